@@ -60,7 +60,7 @@ typedef unsigned __int128 u128;
 static const double E_CHARGE = 1.602176634e-19;
 static const double EPS0 = 8.8541878128e-12;
 static const double TWO_M32 = 2.3283064365386962890625e-10;  /* 2^-32 */
-static const double TWO_M53 = 1.1102230246251565404236316680908203125e-16; /* 2^-53 */
+static const double TWO_M52 = 2.220446049250313080847263336181640625e-16; /* 2^-52 */
 static const double TWO_M40 = 9.094947017729282379150390625e-13; /* 2^-40 */
 static const double TWO_P32 = 4294967296.0;
 static const double TWO_P64 = 18446744073709551616.0;
@@ -134,10 +134,12 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-/* 53-bit uniform in (0,1): (((a<<32|b)>>11)+0.5)*2^-53.  SURVEY 8(c) "R". */
+/* Two-word uniform in (0,1): (((a<<32|b)>>12)+0.5)*2^-52, exact in fp64.
+ * DESIGN.md reading R-U: SURVEY 8(c) "R" wrote >>11 and 2^-53, but w+0.5 then needs
+ * 54 bits and the top value rounds to 1.0; 52 bits keep the stated range (0,1). */
 double orc_u53(uint32_t a, uint32_t b) {
-  uint64_t w = (((uint64_t)a << 32) | (uint64_t)b) >> 11;
-  return ((double)w + 0.5) * TWO_M53;
+  uint64_t w = (((uint64_t)a << 32) | (uint64_t)b) >> 12;
+  return ((double)w + 0.5) * TWO_M52;
 }
 /* 32-bit uniform in (0,1): (a+0.5)*2^-32. */
 double orc_u32(uint32_t a) { return ((double)a + 0.5) * TWO_M32; }
@@ -359,11 +361,18 @@ void orc_phase_deposit(orc *o) {
   }
 }
 
-/* dbl(n) of an int128: (double)(int64)(n>>64) * 2^64 + (double)(uint64)n. */
+/* dbl(n) of an int128: sign(n) * ((double)hi(|n|) * 2^64 + (double)lo(|n|)), hi/lo the unsigned
+ * 64-bit halves of the magnitude.  DESIGN.md reading R-dbl: SURVEY 8(c) "P" converted the two's
+ * complement halves, which loses up to 2^11 units of a small negative n (lo is then near 2^64);
+ * the tridiagonal-solve pin in tests/test_oracle_grid.py exposed it.  Magnitude first keeps the
+ * relative error below 2^-52 for every n. */
 static double dbl128(i128 n) {
-  int64_t hi = (int64_t)(n >> 64);
-  uint64_t lo = (uint64_t)n;
-  return (double)hi * TWO_P64 + (double)lo;
+  int neg = n < 0;
+  u128 a = neg ? (u128)0 - (u128)n : (u128)n;
+  uint64_t hi = (uint64_t)(a >> 64);
+  uint64_t lo = (uint64_t)a;
+  double d = (double)hi * TWO_P64 + (double)lo;
+  return neg ? -d : d;
 }
 
 /* P (Poisson / field): exact integer double prefix sum of rho.
