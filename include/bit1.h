@@ -1,0 +1,184 @@
+/*
+ * bit1.h -- C ABI of libbit1: the data-parallel hot path of a BIT1-style 1D3V
+ * electrostatic PIC-MC timestep on one NVIDIA B200 (sm_100a).
+ *
+ * The operation.  arxiv/paper_2606_28534 states the problem as the PIC cycle
+ * "(i) particle mover ... (ii) deposition to the grid ... (iii) field solver ... (iv) particle force
+ * evaluation ... density smoothing and MC collision handling" (Background), run by the
+ * mover move0/moveb and the arranger arrj/narrj, between two walls that absorb
+ * plasma and take its charge (Table 3), with checkpoint/restart of per-species particle
+ * records plus counts per cell.  The paper prints no equations; the exact arithmetic is
+ * fixed in DESIGN.md ("Readings", "Arithmetic policy") following SURVEY.md section 8(c).
+ *
+ * One step of bit1_step, for every particle in array order: gather E (linear), Boris push, move,
+ * periodic wrap or wall absorption (+ re-injection / pair source), null-collision Monte Carlo against
+ * a uniform neutral background (elastic, ionisation, charge exchange; births appended), then a STABLE
+ * counting sort by cell that drops the dead and merges the born, charge deposition to the 1D grid in
+ * int64 fixed point (unit 2^-40 C), and an exact integer-scan Poisson solve giving phi and E.
+ *
+ * Conventions
+ *  - Plain C, no torch types.  Every pointer argument says HOST or DEVICE.
+ *  - Ownership: the library allocates no device memory.  The caller supplies one DEVICE workspace of
+ *    bit1_workspace_size() bytes, 256-byte aligned, alive until bit1_destroy.  All input arrays and
+ *    tables are copied at the call; the caller keeps them.  Streams are borrowed cudaStream_t handles.
+ *  - Errors: every call returns a bit1_status; nothing throws or aborts; out-parameters are untouched
+ *    on error.  Device-side faults (capacity exceeded, particle escaped the domain, overflow list full)
+ *    set a sticky flag word that bit1_sync and the getters report as BIT1_ERR_DEVICE_FLAG.
+ *  - Threading: one context, one caller thread.
+ *  - There is no CPU fallback: without a CUDA device bit1_create returns BIT1_ERR_CUDA.
+ */
+#ifndef BIT1_H
+#define BIT1_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BIT1_MAX_SPECIES 8
+
+typedef struct bit1_ctx bit1_ctx; /* opaque, host side, owned by the library */
+
+typedef enum {
+  BIT1_OK = 0,
+  BIT1_ERR_INVALID_ARG = 1,
+  BIT1_ERR_RANGE = 2,       /* fixed-point charge Q_s outside [1, 2^31) */
+  BIT1_ERR_CAPACITY = 3,    /* more particles than capacity, or workspace too small */
+  BIT1_ERR_STATE = 4,       /* call out of order (e.g. step before load) */
+  BIT1_ERR_CUDA = 5,        /* a CUDA runtime call failed / no device */
+  BIT1_ERR_CHECKPOINT = 6,  /* blob does not match this context */
+  BIT1_ERR_DEVICE_FLAG = 7  /* sticky device flag set; see bit1_moments.flags */
+} bit1_status;
+
+/* sticky device flag bits (bit1_moments.flags) */
+#define BIT1_FLAG_CAPACITY 1u  /* births beyond capacity were dropped (SURVEY 8(c) "A") */
+#define BIT1_FLAG_ESCAPE 2u    /* a particle crossed more than one domain length (reading A21) */
+#define BIT1_FLAG_OVERFLOW 4u  /* far-mover/birth list full: results after this step are invalid */
+
+/* species process flags */
+#define BIT1_ELASTIC 1u             /* e-D elastic, isotropic (reading A14) */
+#define BIT1_IONISE 2u              /* e-D ionisation (readings A15, A16) */
+#define BIT1_CX 4u                  /* D+-D charge exchange */
+#define BIT1_ION_PRODUCT 8u         /* species that receives ions born by ionisation */
+#define BIT1_ELECTRON_PRODUCT 16u   /* species that receives electrons born by ionisation */
+#define BIT1_TARGET_MAXWELLIAN 32u  /* collision partner sampled from the neutral Maxwellian (A13) */
+
+#define BIT1_SRC_NONE 0 /* absorbed particles die */
+#define BIT1_SRC_SELF 1 /* absorbed particles are re-injected in [src_lo, src_hi) (reading A9) */
+#define BIT1_SRC_PAIR 2 /* as SELF, plus one particle of src_partner born at the same place */
+
+/* Grid ("simulation domain"; 1D, x is the wall normal). */
+typedef struct {
+  int32_t nc;         /* cells, >= 2, < 2^28 */
+  int32_t bc;         /* 0 periodic, 1 absorbing grounded walls (phi = 0 at both, reading A8) */
+  double dx;          /* m */
+  double area;        /* m^2 cross-section that turns the 1D density into coulombs (reading A4) */
+  double Bx, By, Bz;  /* tesla, uniform (reading A7) */
+} bit1_grid;
+
+typedef struct {
+  double q, m;          /* C, kg */
+  double weight;        /* real particles per macro-particle; Q = llrint(e*weight*2^40) in [1, 2^31) */
+  uint32_t flags;       /* BIT1_ELASTIC | ... */
+  int32_t src_mode;     /* BIT1_SRC_* */
+  int32_t src_partner;  /* species index for BIT1_SRC_PAIR, else ignored */
+  int32_t _pad;
+  double src_vth;       /* sqrt(e*T_src/m), m/s per component */
+  double pnull, numax;  /* null-collision probability per step and nu_max (1/s), caller computed (A17) */
+} bit1_species;
+
+typedef struct {
+  uint64_t seed;      /* Philox key */
+  uint64_t capacity;  /* max particles incl. births, < 2^31 */
+  double src_lo, src_hi;          /* re-injection interval, m */
+  double n0, vth_n, E_ion, m_n;   /* neutral density m^-3, sqrt(e*T0/m_n) m/s, threshold eV, neutral mass kg */
+  const double *sig_el, *sig_ion, *sig_cx; /* HOST, n_sig entries each, uniform grid in eV from 0; may be NULL if n_sig == 0 */
+  int32_t n_sig;
+  int32_t n_norm;          /* intervals of the inverse normal CDF table */
+  double dE_eV;
+  const double *inv_norm;  /* HOST, n_norm + 1 entries (reading A18) */
+  void *workspace;         /* DEVICE, bit1_workspace_size() bytes, 256-byte aligned */
+  size_t workspace_bytes;
+  void *compute_stream;    /* cudaStream_t, borrowed; NULL = default stream */
+  void *side_stream;       /* cudaStream_t for checkpoint device->host copies; NULL = compute stream */
+  int32_t checkpoint_staging; /* 1: reserve a device snapshot area so bit1_checkpoint overlaps later steps */
+  int32_t variant;         /* 0 default; 1 = in-place push then scatter ("V1"); 2 = recompute in the scatter pass ("V2") */
+} bit1_options;
+
+typedef struct {
+  uint64_t step, n_live;
+  uint64_t count[BIT1_MAX_SPECIES];
+  double kinetic_J[BIT1_MAX_SPECIES]; /* 0.5 m w sum |v|^2 */
+  double px[BIT1_MAX_SPECIES];        /* m w sum vx */
+  double field_J;                     /* 0.5 eps0 area dx sum g_j E_j^2 */
+  uint64_t wall_count[2][BIT1_MAX_SPECIES];
+  int64_t wall_charge_fixed[2];       /* unit 2^-40 C */
+  int64_t rho_total_fixed;
+  uint32_t flags;                     /* sticky BIT1_FLAG_* */
+  uint32_t next_pid;
+  uint64_t nu_overflow, dir_fallback, escape, births, reinject;
+  uint64_t candidates[BIT1_MAX_SPECIES];
+  uint64_t events[BIT1_MAX_SPECIES][3]; /* elastic, ionise, cx */
+  uint64_t far_movers, max_far_movers_per_step; /* entries that took the sorted side list */
+  double *density[BIT1_MAX_SPECIES];  /* HOST, optional (NULL to skip), ng entries each, m^-3 */
+} bit1_moments;
+
+/* Bytes of device workspace for this configuration (staging: see bit1_options.checkpoint_staging). */
+size_t bit1_workspace_size(const bit1_grid *grid, int nspecies, uint64_t capacity, int checkpoint_staging);
+
+/* Create a context.  grid/species/opt are HOST structs, copied.  BIT1_ERR_RANGE if any Q_s is out of
+ * range; BIT1_ERR_INVALID_ARG for nc < 2, non-positive dx/dt/m/weight, bad species indices, IONISE set
+ * without both product species (of equal weight); BIT1_ERR_CAPACITY if the workspace is too small. */
+bit1_status bit1_create(const bit1_grid *grid, const bit1_species *species, int nspecies, double dt,
+                        const bit1_options *opt, bit1_ctx **out);
+
+/* Load n particles (arrays of n entries; HOST pointers unless ptrs_on_device != 0; pid may be NULL =
+ * 0..n-1).  Requires 0 <= x < nc*dx and species < nspecies.  Afterwards: particles stably sorted by
+ * cell (given order kept inside a cell), rho/phi/E valid, step = 0.  v is v(t = -dt/2) (reading A25). */
+bit1_status bit1_load_particles(bit1_ctx *ctx, uint64_t n, const double *x, const double *vx,
+                                const double *vy, const double *vz, const uint8_t *species,
+                                const uint32_t *pid_or_null, int ptrs_on_device);
+
+/* Enqueue nsteps timesteps on the compute stream; returns without waiting. */
+bit1_status bit1_step(bit1_ctx *ctx, uint64_t nsteps);
+/* Wait for the compute stream; BIT1_ERR_DEVICE_FLAG if the sticky flag word is non-zero. */
+bit1_status bit1_sync(bit1_ctx *ctx);
+
+/* Getters synchronise the compute stream; outputs are caller-allocated HOST buffers. */
+bit1_status bit1_get_count(bit1_ctx *ctx, uint64_t *n_live, uint64_t *step, uint64_t per_species[BIT1_MAX_SPECIES]);
+bit1_status bit1_get_rho(bit1_ctx *ctx, int64_t *rho_fixed_or_null, double *rho_si_or_null); /* ng entries; SI = C/m^3 */
+bit1_status bit1_get_phi(bit1_ctx *ctx, double *phi); /* nc+1 entries (periodic: ghost copy at nc) */
+bit1_status bit1_get_E(bit1_ctx *ctx, double *E);     /* nc+1 entries */
+bit1_status bit1_get_dens(bit1_ctx *ctx, int64_t *dens_fixed); /* nspecies*ng entries, species-major */
+bit1_status bit1_get_moments(bit1_ctx *ctx, bit1_moments *out);
+/* Any pointer may be NULL.  n_live entries each (bit1_get_count), cell_start nc+1 entries. */
+bit1_status bit1_get_particles(bit1_ctx *ctx, double *x, double *vx, double *vy, double *vz,
+                               int32_t *cell, uint32_t *pid, uint8_t *species, int64_t *cell_start_or_null);
+
+/* Test hook: overwrite E (HOST, nc+1 entries) and optionally freeze the field solve (E stays as set
+ * while rho keeps being deposited) -- used by closed-form push tests. */
+bit1_status bit1_set_E(bit1_ctx *ctx, const double *E, int freeze_field);
+/* Test hook: set the step counter (Philox counter words 1-2). */
+bit1_status bit1_set_step(bit1_ctx *ctx, uint64_t step);
+
+/* Checkpoint: header + counts per cell + the SoA particle records, snapshotted on the
+ * compute stream and copied to PINNED HOST memory on the side stream; later bit1_step calls overlap the
+ * copy when the context was created with checkpoint_staging = 1.  The blob is valid after
+ * bit1_checkpoint_wait.  bit1_restart needs a context created with the identical configuration and
+ * reproduces the run bit-identically (BASELINE.json north_star). */
+size_t bit1_checkpoint_size(bit1_ctx *ctx);
+bit1_status bit1_checkpoint(bit1_ctx *ctx, void *pinned_host, size_t cap, size_t *written);
+bit1_status bit1_checkpoint_wait(bit1_ctx *ctx);
+bit1_status bit1_restart(bit1_ctx *ctx, const void *blob_host, size_t bytes);
+
+void bit1_destroy(bit1_ctx *ctx);
+const char *bit1_error_string(bit1_status s);
+/* Kernels launched by this context since create (bench.py's gpu_launches). */
+uint64_t bit1_launch_count(bit1_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BIT1_H */

@@ -1,0 +1,199 @@
+// One particle, one timestep: gather E, Boris push, move, boundary (+ re-injection / pair source),
+// null-collision Monte Carlo.  SURVEY.md 8(c) "G, B, M, W, C, A"; PAPER.md:33 steps (i),(iv) and the
+// "MC routines", PAPER.md:111 mover move0/moveb, PAPER.md:95 wall absorption.
+//
+// EMIT = true  : the pass that owns side effects (wall counters, diagnostics, birth records).
+// EMIT = false : the recompute pass of variant V2 -- same arithmetic, no side effects.
+#pragma once
+#include "device_math.cuh"
+
+namespace bit1 {
+
+__device__ __forceinline__ unsigned long long make_key(int cell, unsigned cls, unsigned long long ord) {
+  return ((unsigned long long)(unsigned)cell << kCellShift) | ((unsigned long long)cls << kClsShift) | ord;
+}
+
+// Append one record (far mover or birth) to the side list.  Order of arrival is irrelevant: k_mid sorts by key.
+static __device__ __noinline__ void emit_record(const Params& P, unsigned long long key, double x, double vx, double vy,
+                                         double vz, unsigned pid, int sp) {
+  const unsigned slot = atomicAdd(&P.st->ovf_count, 1u);
+  if (slot >= P.ovf_cap) {
+    atomicOr(&P.st->flags, kFlagOverflow);
+    return;
+  }
+  P.ovf_key[slot] = key;
+  OvfRec r;
+  r.x = x; r.vx = vx; r.vy = vy; r.vz = vz; r.pid = pid; r.sp = (unsigned)sp;
+  P.ovf_rec[slot] = r;
+}
+
+struct PairBirth {
+  int on;
+  double vx, vy, vz;
+};
+
+// W: wall hit on an absorbing boundary.  Returns alive.
+template <bool EMIT>
+__device__ __noinline__ bool wall_event(const Params& P, const SpeciesP* S, unsigned long long step, int sp,
+                                        unsigned pid, int side, bool escaped, double& x, double& vx, double& vy,
+                                        double& vz, PairBirth& pb) {
+  const SpeciesP& s = S[sp];
+  if (EMIT) {
+    if (escaped) {
+      atomicOr(&P.st->flags, kFlagEscape);
+      atomicAdd(&P.st->escape, 1ull);
+    }
+    atomicAdd(&P.st->wall_count[side][sp], 1ull);
+    atomicAdd((unsigned long long*)&P.st->wall_charge[side], (unsigned long long)((long long)s.sign * s.Q));
+  }
+  if (s.src_mode == kSrcNone) return false;
+  const uint4 w = draw(P, pid, step, 2u);  // slot RJ
+  const double u0 = u32(w.x);
+  x = P.src_lo + u0 * P.src_span;
+  vx = s.src_vth * normal_from_word(P, w.y);
+  vy = s.src_vth * normal_from_word(P, w.z);
+  vz = s.src_vth * normal_from_word(P, w.w);
+  if (EMIT) atomicAdd(&P.st->reinject, 1ull);
+  if (s.src_mode == kSrcPair) {
+    const double pv = S[s.src_partner].src_vth;
+    const uint4 wp = draw(P, pid, step, 13u);  // slot PB
+    pb.on = 1;
+    pb.vx = pv * normal_from_word(P, wp.x);
+    pb.vy = pv * normal_from_word(P, wp.y);
+    pb.vz = pv * normal_from_word(P, wp.z);
+  }
+  return true;
+}
+
+// C: a null-collision candidate (u0 < pnull).  Rewrites v; ionisation emits two births.
+template <bool EMIT>
+__device__ __noinline__ void collide(const Params& P, const SpeciesP* S, unsigned long long step, int sp,
+                                     unsigned pid, unsigned gidx, double u1, double x, int cn, double& vx,
+                                     double& vy, double& vz) {
+  const SpeciesP& s = S[sp];
+  const unsigned fl = s.flags;
+  if (EMIT) atomicAdd(&P.st->candidates[sp], 1ull);
+  double vnx = 0.0, vny = 0.0, vnz = 0.0;
+  if (fl & kTargetMaxwellian) {
+    const uint4 wn = draw(P, pid, step, 1u);  // slot NV
+    vnx = P.vth_n * normal_from_word(P, wn.x);
+    vny = P.vth_n * normal_from_word(P, wn.y);
+    vnz = P.vth_n * normal_from_word(P, wn.z);
+  }
+  const double gx = vx - vnx, gy = vy - vny, gz = vz - vnz;
+  const double g2 = (gx * gx + gy * gy) + gz * gz;
+  const double g = sqrt(g2);
+  const double EeV = s.kin_eV * g2;
+  const double r = u1 * s.numax;
+  double cum = 0.0;
+  int chosen = -1;
+  if (fl & kElastic) {
+    cum = cum + (P.n0 * sigma_lookup(P, P.sig_el, EeV)) * g;
+    if (chosen < 0 && r < cum) chosen = 0;
+  }
+  if (fl & kIonise) {
+    cum = cum + (P.n0 * sigma_lookup(P, P.sig_ion, EeV)) * g;
+    if (chosen < 0 && r < cum) chosen = 1;
+  }
+  if (fl & kCx) {
+    cum = cum + (P.n0 * sigma_lookup(P, P.sig_cx, EeV)) * g;
+    if (chosen < 0 && r < cum) chosen = 2;
+  }
+  if (EMIT && cum > s.numax) atomicAdd(&P.st->nu_overflow, 1ull);
+  if (chosen == 0) {
+    double nn[3];
+    const int fb = direction(P, pid, step, 4u, nn);
+    const double dot = (vx * nn[0] + vy * nn[1]) + vz * nn[2];
+    const double cosx = dot / g;
+    const double gn = g * sqrt(1.0 - s.el_loss * (1.0 - cosx));
+    vx = gn * nn[0]; vy = gn * nn[1]; vz = gn * nn[2];
+    if (EMIT) {
+      if (fb) atomicAdd(&P.st->dir_fallback, 1ull);
+      atomicAdd(&P.st->events[sp][0], 1ull);
+    }
+  } else if (chosen == 1) {
+    const double Er = EeV - P.E_ion;
+    const uint4 ws = draw(P, pid, step, 3u);  // slot SP
+    const double u = u52(ws.x, ws.y);
+    const double E1 = u * Er;
+    const double E2 = Er - E1;
+    double n1[3], n2[3];
+    const int fb1 = direction(P, pid, step, 4u, n1);
+    const double sp1 = sqrt(E1 * s.two_e_over_m);
+    vx = sp1 * n1[0]; vy = sp1 * n1[1]; vz = sp1 * n1[2];
+    if (EMIT) {
+      const int fb2 = direction(P, pid, step, 8u, n2);
+      const double sp2 = sqrt(E2 * S[P.sp_ep].two_e_over_m);
+      const uint4 wb = draw(P, pid, step, 12u);  // slot BI
+      const double ivx = P.vth_n * normal_from_word(P, wb.x);
+      const double ivy = P.vth_n * normal_from_word(P, wb.y);
+      const double ivz = P.vth_n * normal_from_word(P, wb.z);
+      emit_record(P, make_key(cn, 2u, (unsigned long long)gidx * 4ull + 1ull), x, sp2 * n2[0], sp2 * n2[1],
+                  sp2 * n2[2], 0u, P.sp_ep);
+      emit_record(P, make_key(cn, 2u, (unsigned long long)gidx * 4ull + 2ull), x, ivx, ivy, ivz, 0u, P.sp_ip);
+      if (fb1 + fb2) atomicAdd(&P.st->dir_fallback, (unsigned long long)(fb1 + fb2));
+      atomicAdd(&P.st->events[sp][1], 1ull);
+    }
+  } else if (chosen == 2) {
+    vx = vnx; vy = vny; vz = vnz;
+    if (EMIT) atomicAdd(&P.st->events[sp][2], 1ull);
+  }
+}
+
+// The whole per-particle step.  In: state at step k (c = current cell).  Out: state at k+1, c = new cell
+// or -1 when the particle died.  Eptr[c], Eptr[c+1] must be readable (global E or a shared-memory window).
+template <bool EMIT>
+__device__ __forceinline__ void advance(const Params& P, const SpeciesP* S, unsigned long long step,
+                                        const double* Eptr, int sp, unsigned pid, unsigned gidx, double& x,
+                                        double& vx, double& vy, double& vz, int& c) {
+  const SpeciesP& s = S[sp];
+  // G
+  const double f = x * P.inv_dx - (double)c;
+  const double e0 = Eptr[c], e1 = Eptr[c + 1];
+  const double Ex = e0 + f * (e1 - e0);
+  // B
+  const double a = s.h * Ex;
+  const double ux = vx + a, uy = vy, uz = vz;
+  const double px = ux + (uy * s.tz - uz * s.ty);
+  const double py = uy + (uz * s.tx - ux * s.tz);
+  const double pz = uz + (ux * s.ty - uy * s.tx);
+  const double wx = ux + (py * s.sz - pz * s.sy);
+  const double wy = uy + (pz * s.sx - px * s.sz);
+  const double wz = uz + (px * s.sy - py * s.sx);
+  vx = wx + a; vy = wy; vz = wz;
+  // M
+  x = x + vx * P.dt;
+  // W
+  bool alive = true;
+  PairBirth pb;
+  pb.on = 0;
+  if (!P.bc) {
+    if (x < 0.0) x = x + P.L;
+    if (x >= P.L) x = x - P.L;
+    if (!(x >= 0.0 && x < P.L)) {
+      if (EMIT) {
+        atomicOr(&P.st->flags, kFlagEscape);
+        atomicAdd(&P.st->escape, 1ull);
+      }
+      x = 0.0;
+    }
+  } else if (!(x >= 0.0 && x < P.L)) {
+    const int side = (x >= P.L) ? 1 : 0;
+    const bool escaped = !(x < 0.0) && !(x >= P.L);  // NaN
+    alive = wall_event<EMIT>(P, S, step, sp, pid, side, escaped, x, vx, vy, vz, pb);
+  }
+  const int cn = alive ? cell_of(P, x) : -1;
+  // C
+  if (alive && (s.flags & (kElastic | kIonise | kCx))) {
+    const uint4 w = draw(P, pid, step, 0u);  // slot C0
+    const double u0 = u52(w.x, w.y);
+    if (u0 < s.pnull) collide<EMIT>(P, S, step, sp, pid, gidx, u52(w.z, w.w), x, cn, vx, vy, vz);
+  }
+  // A: the pair-source partner is the parent's first birth (ord slot 0)
+  if (EMIT && pb.on)
+    emit_record(P, make_key(cn, 2u, (unsigned long long)gidx * 4ull), x, pb.vx, pb.vy, pb.vz, 0u,
+                s.src_partner);
+  c = cn;
+}
+
+}  // namespace bit1

@@ -1,0 +1,656 @@
+// C ABI of libbit1 (include/bit1.h): argument checking, workspace layout, stream-ordered launches.
+// Every step of the hot path runs in the kernels of step_kernels.cu; nothing here computes on the host
+// beyond the derived constants of DESIGN.md "Derived constants".
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "../../include/bit1.h"
+#include "aux_kernels.h"
+#include "step_kernels.h"
+
+using namespace bit1;
+
+namespace {
+
+constexpr double kECharge = 1.602176634e-19;   // C, CODATA 2018
+constexpr double kEps0 = 8.8541878128e-12;     // F/m
+constexpr double kTwoM40 = 9.094947017729282379150390625e-13;
+constexpr int kMaxSig = 16384;
+constexpr int kMaxNorm = 1 << 20;
+constexpr int kMaxR = 4;
+constexpr size_t kAlign = 256;
+constexpr uint32_t kCkptVersion = 1;
+
+inline size_t align_up(size_t v) { return (v + kAlign - 1) & ~(kAlign - 1); }
+
+struct PartLayout {
+  size_t x, vx, vy, vz, cell, pid, sp, bytes;
+};
+PartLayout part_layout(size_t cap) {
+  PartLayout l;
+  size_t o = 0;
+  l.x = o; o += align_up(cap * 8);
+  l.vx = o; o += align_up(cap * 8);
+  l.vy = o; o += align_up(cap * 8);
+  l.vz = o; o += align_up(cap * 8);
+  l.cell = o; o += align_up(cap * 4);
+  l.pid = o; o += align_up(cap * 4);
+  l.sp = o; o += align_up(cap);
+  l.bytes = o;
+  return l;
+}
+Particles part_at(void* base, const PartLayout& l) {
+  char* b = static_cast<char*>(base);
+  Particles p;
+  p.x = reinterpret_cast<double*>(b + l.x);
+  p.vx = reinterpret_cast<double*>(b + l.vx);
+  p.vy = reinterpret_cast<double*>(b + l.vy);
+  p.vz = reinterpret_cast<double*>(b + l.vz);
+  p.cell = reinterpret_cast<int*>(b + l.cell);
+  p.pid = reinterpret_cast<unsigned*>(b + l.pid);
+  p.sp = reinterpret_cast<unsigned char*>(b + l.sp);
+  return p;
+}
+
+struct CkptLayout {
+  size_t header, state, cell_start, part, bytes;
+};
+CkptLayout ckpt_layout(int nc, size_t cap) {
+  CkptLayout c;
+  c.header = 0;
+  c.state = 256;
+  c.cell_start = c.state + align_up(sizeof(DevState));
+  c.part = c.cell_start + align_up((size_t)(nc + 1) * 4);
+  c.bytes = c.part + part_layout(cap).bytes;
+  return c;
+}
+
+struct Layout {
+  size_t st, tables, dens, rho, phi, E, cell_count, cell_start, cell_base, ovf_before, tile_desc, tile_hist,
+      ovf_key, ovf_idx, ovf_dst, tmp_key, tmp_idx, ovf_rec, part[2], scratch, mom, total;
+  unsigned ovf_cap, ovf_pow2;
+  int max_tiles, ng;
+  size_t scratch_bytes;
+};
+Layout make_layout(int nc, int bc, int ns, size_t cap, int staging) {
+  Layout l;
+  l.ng = bc ? nc + 1 : nc;
+  l.max_tiles = (int)((cap + kTile - 1) / kTile);
+  size_t oc = cap / 16;
+  if (oc < 65536) oc = 65536;
+  l.ovf_cap = (unsigned)oc;
+  unsigned p2 = 1;
+  while (p2 < l.ovf_cap) p2 <<= 1;
+  l.ovf_pow2 = p2;
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes); return at; };
+  l.st = take(sizeof(DevState));
+  l.tables = take(((size_t)3 * kMaxSig + kMaxNorm + 1) * 8);
+  l.dens = take((size_t)ns * l.ng * 8);
+  l.rho = take((size_t)l.ng * 8);
+  l.phi = take((size_t)(nc + 1) * 8);
+  l.E = take((size_t)(nc + 1) * 8);
+  l.cell_count = take((size_t)nc * 4);
+  l.cell_start = take((size_t)(nc + 1) * 4);
+  l.cell_base = take((size_t)nc * 4);
+  l.ovf_before = take((size_t)nc * 4);
+  l.tile_desc = take((size_t)(l.max_tiles + 1) * 8);
+  l.tile_hist = take(((size_t)nc + (size_t)(l.max_tiles + 1) * (2 * kMaxR + 1) + kWCap) * 4);
+  l.ovf_key = take((size_t)p2 * 8);
+  l.tmp_key = take((size_t)p2 * 8);
+  l.ovf_idx = take((size_t)p2 * 4);
+  l.ovf_dst = take((size_t)p2 * 4);
+  l.tmp_idx = take((size_t)p2 * 4);
+  l.ovf_rec = take((size_t)l.ovf_cap * sizeof(OvfRec));
+  const PartLayout pl = part_layout(cap);
+  l.part[0] = take(pl.bytes);
+  l.part[1] = take(pl.bytes);
+  l.scratch_bytes = load_scratch_bytes((unsigned)cap);
+  if (staging) {
+    const size_t cb = ckpt_layout(nc, cap).bytes;
+    if (cb > l.scratch_bytes) l.scratch_bytes = cb;
+  }
+  l.scratch = take(l.scratch_bytes);
+  l.mom = take(moments_scratch_bytes());
+  l.total = o;
+  return l;
+}
+
+struct CkptHeader {
+  char magic[8];
+  uint32_t version;
+  int32_t nc, ns, bc;
+  uint64_t capacity, cfg_hash, bytes;
+};
+
+uint64_t fnv1a(uint64_t h, const void* data, size_t n) {
+  const unsigned char* p = static_cast<const unsigned char*>(data);
+  for (size_t i = 0; i < n; ++i) { h ^= p[i]; h *= 1099511628211ull; }
+  return h;
+}
+
+}  // namespace
+
+struct bit1_ctx {
+  Params P;
+  Layout lay;
+  Particles buf[2];
+  int cur;
+  char* ws;
+  cudaStream_t cs, ss;
+  cudaEvent_t ev_snap, ev_done;
+  bool ckpt_pending, staging, loaded;
+  int variant;
+  uint64_t launches, cfg_hash;
+  double m[BIT1_MAX_SPECIES], weight[BIT1_MAX_SPECIES];
+  double dt;
+};
+
+#define CUDA_OK(call)                              \
+  do {                                             \
+    cudaError_t e_ = (call);                       \
+    if (e_ != cudaSuccess) return BIT1_ERR_CUDA;   \
+  } while (0)
+
+extern "C" {
+
+const char* bit1_error_string(bit1_status s) {
+  switch (s) {
+    case BIT1_OK: return "ok";
+    case BIT1_ERR_INVALID_ARG: return "invalid argument";
+    case BIT1_ERR_RANGE: return "fixed-point charge out of range [1, 2^31)";
+    case BIT1_ERR_CAPACITY: return "capacity or workspace too small";
+    case BIT1_ERR_STATE: return "call out of order";
+    case BIT1_ERR_CUDA: return "CUDA runtime error or no device";
+    case BIT1_ERR_CHECKPOINT: return "checkpoint blob does not match this context";
+    case BIT1_ERR_DEVICE_FLAG: return "sticky device flag set";
+  }
+  return "unknown";
+}
+
+size_t bit1_workspace_size(const bit1_grid* g, int ns, uint64_t capacity, int staging) {
+  if (!g || g->nc < 2 || ns < 1 || ns > BIT1_MAX_SPECIES || capacity == 0 || capacity >= (1ull << 31)) return 0;
+  return make_layout(g->nc, g->bc, ns, (size_t)capacity, staging).total;
+}
+
+bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, double dt, const bit1_options* o,
+                        bit1_ctx** out) {
+  if (!g || !sp || !o || !out) return BIT1_ERR_INVALID_ARG;
+  if (g->nc < 2 || g->nc >= (1 << 28) || (g->bc != 0 && g->bc != 1) || !(g->dx > 0.0) || !(g->area > 0.0) ||
+      !(dt > 0.0) || ns < 1 || ns > BIT1_MAX_SPECIES)
+    return BIT1_ERR_INVALID_ARG;
+  if (o->capacity == 0 || o->capacity >= (1ull << 31)) return BIT1_ERR_INVALID_ARG;
+  if (o->n_sig < 0 || o->n_sig > kMaxSig || o->n_norm < 1 || o->n_norm > kMaxNorm || !o->inv_norm)
+    return BIT1_ERR_INVALID_ARG;
+  if (!o->workspace || (reinterpret_cast<uintptr_t>(o->workspace) & (kAlign - 1))) return BIT1_ERR_INVALID_ARG;
+  int sp_ep = -1, sp_ip = -1;
+  bool any_coll = false, any_ion = false;
+  for (int s = 0; s < ns; ++s) {
+    if (!(sp[s].m > 0.0) || !(sp[s].weight > 0.0)) return BIT1_ERR_INVALID_ARG;
+    if (sp[s].src_mode < 0 || sp[s].src_mode > 2) return BIT1_ERR_INVALID_ARG;
+    if (sp[s].src_mode == BIT1_SRC_PAIR && (sp[s].src_partner < 0 || sp[s].src_partner >= ns))
+      return BIT1_ERR_INVALID_ARG;
+    if ((sp[s].flags & BIT1_ELECTRON_PRODUCT) && sp_ep < 0) sp_ep = s;
+    if ((sp[s].flags & BIT1_ION_PRODUCT) && sp_ip < 0) sp_ip = s;
+    if (sp[s].flags & (BIT1_ELASTIC | BIT1_IONISE | BIT1_CX)) any_coll = true;
+    if (sp[s].flags & BIT1_IONISE) any_ion = true;
+  }
+  if (any_coll && (o->n_sig < 2 || !o->sig_el || !o->sig_ion || !o->sig_cx || !(o->dE_eV > 0.0) || !(o->m_n > 0.0)))
+    return BIT1_ERR_INVALID_ARG;
+  if (any_ion && (sp_ep < 0 || sp_ip < 0 || sp[sp_ep].weight != sp[sp_ip].weight)) return BIT1_ERR_INVALID_ARG;
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return BIT1_ERR_CUDA;
+
+  const int staging = o->checkpoint_staging ? 1 : 0;
+  const Layout lay = make_layout(g->nc, g->bc, ns, (size_t)o->capacity, staging);
+  if (o->workspace_bytes < lay.total) return BIT1_ERR_CAPACITY;
+
+  bit1_ctx* c = new (std::nothrow) bit1_ctx();
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  memset(&c->P, 0, sizeof(Params));
+  c->lay = lay;
+  c->ws = static_cast<char*>(o->workspace);
+  c->cs = static_cast<cudaStream_t>(o->compute_stream);
+  c->ss = o->side_stream ? static_cast<cudaStream_t>(o->side_stream) : c->cs;
+  c->staging = staging != 0;
+  c->variant = o->variant == 1 ? 1 : 2;
+  if (const char* ev = getenv("BIT1_VARIANT")) { if (atoi(ev) == 1) c->variant = 1; else if (atoi(ev) == 2) c->variant = 2; }
+  c->cur = 0; c->loaded = false; c->ckpt_pending = false; c->launches = 0; c->dt = dt;
+
+  Params& P = c->P;
+  P.nc = g->nc; P.bc = g->bc; P.ng = lay.ng; P.ns = ns;
+  P.R = 1;
+  if (const char* ev = getenv("BIT1_WINDOW_R")) { int r = atoi(ev); if (r >= 0 && r <= kMaxR) P.R = r; }
+  P.n_sig = o->n_sig; P.n_norm = o->n_norm; P.sp_ep = sp_ep; P.sp_ip = sp_ip;
+  P.seed_lo = (unsigned)o->seed; P.seed_hi = (unsigned)(o->seed >> 32);
+  P.capacity = (unsigned)o->capacity; P.ovf_cap = lay.ovf_cap; P.ovf_pow2 = lay.ovf_pow2;
+  P.max_tiles = lay.max_tiles;
+  // derived constants, one documented expression each
+  P.inv_dx = 1.0 / g->dx;
+  P.L = (double)g->nc * g->dx;
+  P.dt = dt; P.dx = g->dx; P.area = g->area;
+  P.src_lo = o->src_lo; P.src_span = o->src_hi - o->src_lo;
+  P.n0 = o->n0; P.vth_n = o->vth_n; P.E_ion = o->E_ion; P.dE_eV = o->dE_eV;
+  P.Kphi = (kTwoM40 * g->dx) / ((g->area * kEps0) * (double)g->nc);
+  P.KE = kTwoM40 / (((2.0 * (double)g->nc) * g->area) * kEps0);
+  if (!g->bc) { P.Kphi = P.Kphi / (double)g->nc; P.KE = P.KE / (double)g->nc; }
+  P.field_J_factor = ((0.5 * kEps0) * g->area) * g->dx;
+  P.dep_u32 = 1;
+  const double B[3] = {g->Bx, g->By, g->Bz};
+  for (int s = 0; s < ns; ++s) {
+    SpeciesP& q = P.sp[s];
+    const double h = 0.5 * ((sp[s].q / sp[s].m) * dt);
+    q.h = h;
+    q.tx = h * B[0]; q.ty = h * B[1]; q.tz = h * B[2];
+    const double tt = (q.tx * q.tx + q.ty * q.ty) + q.tz * q.tz;
+    q.sx = (2.0 * q.tx) / (1.0 + tt);
+    q.sy = (2.0 * q.ty) / (1.0 + tt);
+    q.sz = (2.0 * q.tz) / (1.0 + tt);
+    q.src_vth = sp[s].src_vth; q.pnull = sp[s].pnull; q.numax = sp[s].numax;
+    q.kin_eV = (0.5 * sp[s].m) / kECharge;
+    q.two_e_over_m = (2.0 * kECharge) / sp[s].m;
+    q.el_loss = o->m_n > 0.0 ? (2.0 * sp[s].m) / o->m_n : 0.0;
+    q.Q = llrint((kECharge * sp[s].weight) * 1099511627776.0);
+    q.sign = sp[s].q > 0.0 ? 1 : (sp[s].q < 0.0 ? -1 : 0);
+    q.flags = sp[s].flags; q.src_mode = sp[s].src_mode; q.src_partner = sp[s].src_partner;
+    if (q.Q < 1 || q.Q >= (1ll << 31)) { delete c; return BIT1_ERR_RANGE; }
+    if ((unsigned long long)q.Q * (unsigned long long)kTile >= (1ull << 32)) P.dep_u32 = 0;
+    c->m[s] = sp[s].m; c->weight[s] = sp[s].weight;
+  }
+  char* ws = c->ws;
+  P.st = reinterpret_cast<DevState*>(ws + lay.st);
+  double* tab = reinterpret_cast<double*>(ws + lay.tables);
+  P.sig_el = tab; P.sig_ion = tab + kMaxSig; P.sig_cx = tab + 2 * kMaxSig; P.inv_norm = tab + 3 * kMaxSig;
+  P.dens = reinterpret_cast<long long*>(ws + lay.dens);
+  P.rho = reinterpret_cast<long long*>(ws + lay.rho);
+  P.phi = reinterpret_cast<double*>(ws + lay.phi);
+  P.E = reinterpret_cast<double*>(ws + lay.E);
+  P.cell_count = reinterpret_cast<int*>(ws + lay.cell_count);
+  P.cell_start = reinterpret_cast<int*>(ws + lay.cell_start);
+  P.cell_base = reinterpret_cast<int*>(ws + lay.cell_base);
+  P.ovf_before = reinterpret_cast<int*>(ws + lay.ovf_before);
+  P.tile_desc = reinterpret_cast<int2*>(ws + lay.tile_desc);
+  P.tile_hist = reinterpret_cast<unsigned*>(ws + lay.tile_hist);
+  P.ovf_key = reinterpret_cast<unsigned long long*>(ws + lay.ovf_key);
+  P.tmp_key = reinterpret_cast<unsigned long long*>(ws + lay.tmp_key);
+  P.ovf_idx = reinterpret_cast<unsigned*>(ws + lay.ovf_idx);
+  P.ovf_dst = reinterpret_cast<int*>(ws + lay.ovf_dst);
+  P.tmp_idx = reinterpret_cast<unsigned*>(ws + lay.tmp_idx);
+  P.ovf_rec = reinterpret_cast<OvfRec*>(ws + lay.ovf_rec);
+  const PartLayout pl = part_layout((size_t)o->capacity);
+  c->buf[0] = part_at(ws + lay.part[0], pl);
+  c->buf[1] = part_at(ws + lay.part[1], pl);
+
+  // configuration hash for checkpoint validation
+  uint64_t h = 1469598103934665603ull;
+  h = fnv1a(h, g, sizeof(*g));
+  h = fnv1a(h, &dt, sizeof(dt));
+  for (int s = 0; s < ns; ++s) {
+    h = fnv1a(h, &sp[s].q, 8); h = fnv1a(h, &sp[s].m, 8); h = fnv1a(h, &sp[s].weight, 8);
+    h = fnv1a(h, &sp[s].flags, 4); h = fnv1a(h, &sp[s].src_mode, 4); h = fnv1a(h, &sp[s].src_partner, 4);
+    h = fnv1a(h, &sp[s].src_vth, 8); h = fnv1a(h, &sp[s].pnull, 8); h = fnv1a(h, &sp[s].numax, 8);
+  }
+  h = fnv1a(h, &o->seed, 8); h = fnv1a(h, &o->capacity, 8);
+  h = fnv1a(h, &o->src_lo, 8); h = fnv1a(h, &o->src_hi, 8); h = fnv1a(h, &o->n0, 8);
+  h = fnv1a(h, &o->vth_n, 8); h = fnv1a(h, &o->E_ion, 8); h = fnv1a(h, &o->m_n, 8); h = fnv1a(h, &o->dE_eV, 8);
+  if (o->n_sig > 0 && o->sig_el) {
+    h = fnv1a(h, o->sig_el, (size_t)o->n_sig * 8);
+    h = fnv1a(h, o->sig_ion, (size_t)o->n_sig * 8);
+    h = fnv1a(h, o->sig_cx, (size_t)o->n_sig * 8);
+  }
+  h = fnv1a(h, o->inv_norm, (size_t)(o->n_norm + 1) * 8);
+  c->cfg_hash = h;
+
+  bool ok = true;
+  ok = ok && cudaMemsetAsync(ws + lay.st, 0, lay.part[0] - lay.st, c->cs) == cudaSuccess;  // state, grids, lists
+  if (o->n_sig > 0 && o->sig_el) {
+    ok = ok && cudaMemcpyAsync((void*)P.sig_el, o->sig_el, (size_t)o->n_sig * 8, cudaMemcpyHostToDevice, c->cs) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync((void*)P.sig_ion, o->sig_ion, (size_t)o->n_sig * 8, cudaMemcpyHostToDevice, c->cs) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync((void*)P.sig_cx, o->sig_cx, (size_t)o->n_sig * 8, cudaMemcpyHostToDevice, c->cs) == cudaSuccess;
+  }
+  ok = ok && cudaMemcpyAsync((void*)P.inv_norm, o->inv_norm, (size_t)(o->n_norm + 1) * 8, cudaMemcpyHostToDevice, c->cs) == cudaSuccess;
+  ok = ok && cudaStreamSynchronize(c->cs) == cudaSuccess;
+  ok = ok && configure_kernels(ns) == cudaSuccess;
+  ok = ok && cudaEventCreateWithFlags(&c->ev_snap, cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaEventCreateWithFlags(&c->ev_done, cudaEventDisableTiming) == cudaSuccess;
+  if (!ok) { delete c; return BIT1_ERR_CUDA; }
+  *out = c;
+  return BIT1_OK;
+}
+
+void bit1_destroy(bit1_ctx* c) {
+  if (!c) return;
+  cudaStreamSynchronize(c->cs);
+  if (c->ss != c->cs) cudaStreamSynchronize(c->ss);
+  cudaEventDestroy(c->ev_snap);
+  cudaEventDestroy(c->ev_done);
+  delete c;
+}
+
+uint64_t bit1_launch_count(bit1_ctx* c) { return c ? c->launches : 0; }
+
+static bit1_status read_state(bit1_ctx* c, DevState* h) {
+  CUDA_OK(cudaMemcpyAsync(h, c->P.st, sizeof(DevState), cudaMemcpyDeviceToHost, c->cs));
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  return BIT1_OK;
+}
+
+bit1_status bit1_load_particles(bit1_ctx* c, uint64_t n, const double* x, const double* vx, const double* vy,
+                                const double* vz, const uint8_t* sp, const uint32_t* pid, int on_device) {
+  if (!c || (n && (!x || !vx || !vy || !vz || !sp))) return BIT1_ERR_INVALID_ARG;
+  if (n > c->P.capacity) return BIT1_ERR_CAPACITY;
+  if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; }
+  const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  Particles in = c->buf[1], outp = c->buf[0];
+  CUDA_OK(cudaMemsetAsync(c->P.st, 0, sizeof(DevState), c->cs));
+  if (n) {
+    CUDA_OK(cudaMemcpyAsync(in.x, x, n * 8, kind, c->cs));
+    CUDA_OK(cudaMemcpyAsync(in.vx, vx, n * 8, kind, c->cs));
+    CUDA_OK(cudaMemcpyAsync(in.vy, vy, n * 8, kind, c->cs));
+    CUDA_OK(cudaMemcpyAsync(in.vz, vz, n * 8, kind, c->cs));
+    CUDA_OK(cudaMemcpyAsync(in.sp, sp, n, kind, c->cs));
+    if (pid) CUDA_OK(cudaMemcpyAsync(in.pid, pid, n * 4, kind, c->cs));
+  }
+  const unsigned n32 = (unsigned)n;
+  CUDA_OK(cudaMemcpyAsync(&c->P.st->n, &n32, 4, cudaMemcpyHostToDevice, c->cs));
+  c->launches += launch_load_sort(c->P, in, outp, n32, pid ? 1 : 0, c->ws + c->lay.scratch, c->cs);
+  c->cur = 0;
+  c->launches += launch_rebuild(c->P, c->buf[0], c->cs);
+  CUDA_OK(cudaGetLastError());
+  DevState h;
+  bit1_status s = read_state(c, &h);
+  if (s != BIT1_OK) return s;
+  if (h.load_error) { c->loaded = false; return BIT1_ERR_INVALID_ARG; }
+  c->loaded = true;
+  return BIT1_OK;
+}
+
+bit1_status bit1_step(bit1_ctx* c, uint64_t nsteps) {
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  for (uint64_t k = 0; k < nsteps; ++k) {
+    c->launches += launch_step(c->P, c->buf[c->cur], c->buf[c->cur ^ 1], c->variant, c->cs);
+    c->cur ^= 1;
+  }
+  CUDA_OK(cudaGetLastError());
+  return BIT1_OK;
+}
+
+bit1_status bit1_sync(bit1_ctx* c) {
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  DevState h;
+  bit1_status s = read_state(c, &h);
+  if (s != BIT1_OK) return s;
+  return h.flags ? BIT1_ERR_DEVICE_FLAG : BIT1_OK;
+}
+
+static bit1_status fetch(bit1_ctx* c, void* dst, const void* src, size_t bytes) {
+  if (!bytes) return BIT1_OK;
+  CUDA_OK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, c->cs));
+  return BIT1_OK;
+}
+
+bit1_status bit1_get_count(bit1_ctx* c, uint64_t* n_live, uint64_t* step, uint64_t per_species[BIT1_MAX_SPECIES]) {
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  if (per_species) {
+    bit1_moments m;
+    memset(&m, 0, sizeof(m));
+    bit1_status s = bit1_get_moments(c, &m);
+    if (s != BIT1_OK) return s;
+    for (int k = 0; k < BIT1_MAX_SPECIES; ++k) per_species[k] = m.count[k];
+    if (n_live) *n_live = m.n_live;
+    if (step) *step = m.step;
+    return BIT1_OK;
+  }
+  DevState h;
+  bit1_status s = read_state(c, &h);
+  if (s != BIT1_OK) return s;
+  if (h.flags & kFlagOverflow) return BIT1_ERR_DEVICE_FLAG;
+  if (n_live) *n_live = h.n;
+  if (step) *step = h.step;
+  return BIT1_OK;
+}
+
+bit1_status bit1_get_rho(bit1_ctx* c, int64_t* rho_fixed, double* rho_si) {
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  const int ng = c->P.ng;
+  int64_t* tmp = rho_fixed;
+  if (!tmp) tmp = static_cast<int64_t*>(malloc((size_t)ng * 8));
+  if (!tmp) return BIT1_ERR_INVALID_ARG;
+  bit1_status s = fetch(c, tmp, c->P.rho, (size_t)ng * 8);
+  if (s == BIT1_OK && cudaStreamSynchronize(c->cs) != cudaSuccess) s = BIT1_ERR_CUDA;
+  if (s == BIT1_OK && rho_si) {
+    const double f = kTwoM40 / (c->P.area * c->P.dx);
+    for (int j = 0; j < ng; ++j) {
+      double v = (double)tmp[j] * f;
+      if (c->P.bc && (j == 0 || j == c->P.nc)) v = 2.0 * v;
+      rho_si[j] = v;
+    }
+  }
+  if (!rho_fixed) free(tmp);
+  return s;
+}
+
+bit1_status bit1_get_phi(bit1_ctx* c, double* phi) {
+  if (!c || !phi) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  bit1_status s = fetch(c, phi, c->P.phi, (size_t)(c->P.nc + 1) * 8);
+  if (s != BIT1_OK) return s;
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  return BIT1_OK;
+}
+
+bit1_status bit1_get_E(bit1_ctx* c, double* E) {
+  if (!c || !E) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  bit1_status s = fetch(c, E, c->P.E, (size_t)(c->P.nc + 1) * 8);
+  if (s != BIT1_OK) return s;
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  return BIT1_OK;
+}
+
+bit1_status bit1_get_dens(bit1_ctx* c, int64_t* dens) {
+  if (!c || !dens) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  bit1_status s = fetch(c, dens, c->P.dens, (size_t)c->P.ns * c->P.ng * 8);
+  if (s != BIT1_OK) return s;
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  return BIT1_OK;
+}
+
+bit1_status bit1_get_moments(bit1_ctx* c, bit1_moments* out) {
+  if (!c || !out) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  const Params& P = c->P;
+  double* partial = reinterpret_cast<double*>(c->ws + c->lay.mom);
+  double* dres = partial + (size_t)1024 * kMaxSpecies * 3;
+  c->launches += launch_moments(P, c->buf[c->cur], partial, dres, c->cs);
+  double res[kMaxSpecies * 3 + 1];
+  CUDA_OK(cudaMemcpyAsync(res, dres, sizeof(res), cudaMemcpyDeviceToHost, c->cs));
+  DevState h;
+  bit1_status s = read_state(c, &h);
+  if (s != BIT1_OK) return s;
+  double* dens_out[BIT1_MAX_SPECIES];
+  for (int k = 0; k < BIT1_MAX_SPECIES; ++k) dens_out[k] = out->density[k];
+  out->step = h.step; out->n_live = h.n;
+  for (int k = 0; k < BIT1_MAX_SPECIES; ++k) {
+    out->count[k] = 0; out->kinetic_J[k] = 0.0; out->px[k] = 0.0; out->candidates[k] = h.candidates[k];
+    for (int e = 0; e < 3; ++e) out->events[k][e] = h.events[k][e];
+    out->wall_count[0][k] = h.wall_count[0][k];
+    out->wall_count[1][k] = h.wall_count[1][k];
+  }
+  for (int k = 0; k < P.ns; ++k) {
+    out->count[k] = (uint64_t)res[k * 3];
+    out->kinetic_J[k] = ((0.5 * c->m[k]) * c->weight[k]) * res[k * 3 + 1];
+    out->px[k] = (c->m[k] * c->weight[k]) * res[k * 3 + 2];
+  }
+  out->field_J = P.field_J_factor * res[kMaxSpecies * 3];
+  out->wall_charge_fixed[0] = h.wall_charge[0];
+  out->wall_charge_fixed[1] = h.wall_charge[1];
+  out->rho_total_fixed = h.rho_total;
+  out->flags = h.flags; out->next_pid = h.next_pid;
+  out->nu_overflow = h.nu_overflow; out->dir_fallback = h.dir_fallback; out->escape = h.escape;
+  out->births = h.births; out->reinject = h.reinject;
+  out->far_movers = h.far_movers; out->max_far_movers_per_step = h.max_far_movers;
+  bool any = false;
+  for (int k = 0; k < P.ns; ++k) any = any || dens_out[k];
+  if (any) {
+    const size_t ng = (size_t)P.ng;
+    int64_t* tmp = static_cast<int64_t*>(malloc((size_t)P.ns * ng * 8));
+    if (!tmp) return BIT1_ERR_INVALID_ARG;
+    s = bit1_get_dens(c, tmp);
+    if (s == BIT1_OK) {
+      for (int k = 0; k < P.ns; ++k) {
+        if (!dens_out[k]) continue;
+        for (size_t j = 0; j < ng; ++j) {
+          double v = (((double)tmp[k * ng + j] / (double)P.sp[k].Q) * c->weight[k]) / (P.area * P.dx);
+          if (P.bc && (j == 0 || j == (size_t)P.nc)) v = 2.0 * v;
+          dens_out[k][j] = v;
+        }
+      }
+    }
+    free(tmp);
+    if (s != BIT1_OK) return s;
+  }
+  return BIT1_OK;
+}
+
+bit1_status bit1_get_particles(bit1_ctx* c, double* x, double* vx, double* vy, double* vz, int32_t* cell,
+                               uint32_t* pid, uint8_t* sp, int64_t* cell_start) {
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  DevState h;
+  bit1_status s = read_state(c, &h);
+  if (s != BIT1_OK) return s;
+  if (h.flags & kFlagOverflow) return BIT1_ERR_DEVICE_FLAG;
+  const size_t n = h.n;
+  const Particles& p = c->buf[c->cur];
+  if (x) CUDA_OK(cudaMemcpyAsync(x, p.x, n * 8, cudaMemcpyDeviceToHost, c->cs));
+  if (vx) CUDA_OK(cudaMemcpyAsync(vx, p.vx, n * 8, cudaMemcpyDeviceToHost, c->cs));
+  if (vy) CUDA_OK(cudaMemcpyAsync(vy, p.vy, n * 8, cudaMemcpyDeviceToHost, c->cs));
+  if (vz) CUDA_OK(cudaMemcpyAsync(vz, p.vz, n * 8, cudaMemcpyDeviceToHost, c->cs));
+  if (cell) CUDA_OK(cudaMemcpyAsync(cell, p.cell, n * 4, cudaMemcpyDeviceToHost, c->cs));
+  if (pid) CUDA_OK(cudaMemcpyAsync(pid, p.pid, n * 4, cudaMemcpyDeviceToHost, c->cs));
+  if (sp) CUDA_OK(cudaMemcpyAsync(sp, p.sp, n, cudaMemcpyDeviceToHost, c->cs));
+  int32_t* cs32 = nullptr;
+  if (cell_start) {
+    cs32 = static_cast<int32_t*>(malloc((size_t)(c->P.nc + 1) * 4));
+    if (!cs32) return BIT1_ERR_INVALID_ARG;
+    if (cudaMemcpyAsync(cs32, c->P.cell_start, (size_t)(c->P.nc + 1) * 4, cudaMemcpyDeviceToHost, c->cs) != cudaSuccess) {
+      free(cs32);
+      return BIT1_ERR_CUDA;
+    }
+  }
+  cudaError_t e = cudaStreamSynchronize(c->cs);
+  if (cs32) {
+    if (e == cudaSuccess) for (int j = 0; j <= c->P.nc; ++j) cell_start[j] = cs32[j];
+    free(cs32);
+  }
+  return e == cudaSuccess ? BIT1_OK : BIT1_ERR_CUDA;
+}
+
+bit1_status bit1_set_E(bit1_ctx* c, const double* E, int freeze) {
+  if (!c || !E) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  CUDA_OK(cudaMemcpyAsync(c->P.E, E, (size_t)(c->P.nc + 1) * 8, cudaMemcpyHostToDevice, c->cs));
+  const unsigned f = freeze ? 1u : 0u;
+  CUDA_OK(cudaMemcpyAsync(&c->P.st->freeze_field, &f, 4, cudaMemcpyHostToDevice, c->cs));
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  return BIT1_OK;
+}
+
+bit1_status bit1_set_step(bit1_ctx* c, uint64_t step) {
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  CUDA_OK(cudaMemcpyAsync(&c->P.st->step, &step, 8, cudaMemcpyHostToDevice, c->cs));
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  return BIT1_OK;
+}
+
+size_t bit1_checkpoint_size(bit1_ctx* c) {
+  if (!c) return 0;
+  return ckpt_layout(c->P.nc, c->P.capacity).bytes;
+}
+
+bit1_status bit1_checkpoint(bit1_ctx* c, void* host, size_t cap, size_t* written) {
+  if (!c || !host) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  const CkptLayout cl = ckpt_layout(c->P.nc, c->P.capacity);
+  if (cap < cl.bytes) return BIT1_ERR_CAPACITY;
+  const PartLayout pl = part_layout(c->P.capacity);
+  CkptHeader hd;
+  memset(&hd, 0, sizeof(hd));
+  memcpy(hd.magic, "BIT1CKPT", 8);
+  hd.version = kCkptVersion; hd.nc = c->P.nc; hd.ns = c->P.ns; hd.bc = c->P.bc;
+  hd.capacity = c->P.capacity; hd.cfg_hash = c->cfg_hash; hd.bytes = cl.bytes;
+  memset(host, 0, 256);
+  memcpy(host, &hd, sizeof(hd));
+  char* hb = static_cast<char*>(host);
+  const char* live = c->ws + c->lay.part[c->cur];
+  if (c->staging) {
+    // snapshot on the compute stream, copy out on the side stream: later steps overlap the D2H
+    if (c->ckpt_pending) CUDA_OK(cudaStreamWaitEvent(c->cs, c->ev_done, 0));
+    char* sg = c->ws + c->lay.scratch;
+    CUDA_OK(cudaMemcpyAsync(sg + cl.state, c->P.st, sizeof(DevState), cudaMemcpyDeviceToDevice, c->cs));
+    CUDA_OK(cudaMemcpyAsync(sg + cl.cell_start, c->P.cell_start, (size_t)(c->P.nc + 1) * 4, cudaMemcpyDeviceToDevice, c->cs));
+    CUDA_OK(cudaMemcpyAsync(sg + cl.part, live, pl.bytes, cudaMemcpyDeviceToDevice, c->cs));
+    CUDA_OK(cudaEventRecord(c->ev_snap, c->cs));
+    CUDA_OK(cudaStreamWaitEvent(c->ss, c->ev_snap, 0));
+    CUDA_OK(cudaMemcpyAsync(hb + cl.state, sg + cl.state, cl.bytes - cl.state, cudaMemcpyDeviceToHost, c->ss));
+    CUDA_OK(cudaEventRecord(c->ev_done, c->ss));
+  } else {
+    CUDA_OK(cudaMemcpyAsync(hb + cl.state, c->P.st, sizeof(DevState), cudaMemcpyDeviceToHost, c->cs));
+    CUDA_OK(cudaMemcpyAsync(hb + cl.cell_start, c->P.cell_start, (size_t)(c->P.nc + 1) * 4, cudaMemcpyDeviceToHost, c->cs));
+    CUDA_OK(cudaMemcpyAsync(hb + cl.part, live, pl.bytes, cudaMemcpyDeviceToHost, c->cs));
+    CUDA_OK(cudaEventRecord(c->ev_done, c->cs));
+  }
+  c->ckpt_pending = true;
+  if (written) *written = cl.bytes;
+  return BIT1_OK;
+}
+
+bit1_status bit1_checkpoint_wait(bit1_ctx* c) {
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  if (c->ckpt_pending) {
+    CUDA_OK(cudaEventSynchronize(c->ev_done));
+    c->ckpt_pending = false;
+  }
+  return BIT1_OK;
+}
+
+bit1_status bit1_restart(bit1_ctx* c, const void* blob, size_t bytes) {
+  if (!c || !blob) return BIT1_ERR_INVALID_ARG;
+  const CkptLayout cl = ckpt_layout(c->P.nc, c->P.capacity);
+  if (bytes < cl.bytes) return BIT1_ERR_CHECKPOINT;
+  CkptHeader hd;
+  memcpy(&hd, blob, sizeof(hd));
+  if (memcmp(hd.magic, "BIT1CKPT", 8) != 0 || hd.version != kCkptVersion || hd.nc != c->P.nc || hd.ns != c->P.ns ||
+      hd.bc != c->P.bc || hd.capacity != c->P.capacity || hd.cfg_hash != c->cfg_hash || hd.bytes != cl.bytes)
+    return BIT1_ERR_CHECKPOINT;
+  if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; }
+  const PartLayout pl = part_layout(c->P.capacity);
+  const char* hb = static_cast<const char*>(blob);
+  DevState h;
+  memcpy(&h, hb + cl.state, sizeof(DevState));
+  if (h.n > c->P.capacity) return BIT1_ERR_CHECKPOINT;
+  h.ovf_count = 0; h.ovf_valid = 0; h.freeze_field = 0; h.load_error = 0; h.n_next = h.n;
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  CUDA_OK(cudaMemcpyAsync(c->P.st, &h, sizeof(DevState), cudaMemcpyHostToDevice, c->cs));
+  CUDA_OK(cudaStreamSynchronize(c->cs));  // h is a stack object
+  c->cur = 0;
+  CUDA_OK(cudaMemcpyAsync(c->ws + c->lay.part[0], hb + cl.part, pl.bytes, cudaMemcpyHostToDevice, c->cs));
+  c->launches += launch_rebuild(c->P, c->buf[0], c->cs);
+  CUDA_OK(cudaGetLastError());
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  c->loaded = true;
+  return BIT1_OK;
+}
+
+}  // extern "C"

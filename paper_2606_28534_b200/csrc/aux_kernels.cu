@@ -1,0 +1,261 @@
+// Kernels off the per-step path: load (validate, cell index, general stable sort by cell), moments.
+// The load-time sort is a multi-pass LSD radix sort (8-bit digits) on (cell, original index); it is the
+// general counterpart of the banded single-scatter sort of the step kernels and is not timed.
+#include "aux_kernels.h"
+#include "device_math.cuh"
+
+namespace bit1 {
+
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_load_prepare(const __grid_constant__ Params P, Particles in, unsigned n,
+                                                      int have_pid, unsigned* keys, unsigned* vals) {
+  unsigned maxpid = 0;
+  bool bad = false;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const double x = in.x[i];
+    const int s = in.sp[i];
+    if (!(x >= 0.0 && x < P.L) || s >= P.ns) bad = true;
+    const int c = cell_of(P, x);
+    in.cell[i] = c;
+    if (!have_pid) in.pid[i] = (unsigned)i;
+    const unsigned pid = in.pid[i];
+    maxpid = max(maxpid, pid + 1u);
+    keys[i] = (unsigned)c;
+    vals[i] = (unsigned)i;
+  }
+  for (int o = 16; o > 0; o >>= 1) maxpid = max(maxpid, __shfl_xor_sync(0xffffffffu, maxpid, o));
+  if ((threadIdx.x & 31) == 0 && maxpid) atomicMax(&P.st->next_pid, maxpid);
+  if (bad) atomicOr(&P.st->load_error, 1u);
+}
+
+constexpr int kRadixItems = 8;
+constexpr int kRadixChunk = 256 * kRadixItems;
+
+__global__ void __launch_bounds__(256) k_radix_hist(const unsigned* keys, unsigned n, int shift, unsigned* blockhist,
+                                                    unsigned nblocks) {
+  __shared__ unsigned h[256];
+  h[threadIdx.x] = 0;
+  __syncthreads();
+  const unsigned base = blockIdx.x * kRadixChunk;
+  for (int r = 0; r < kRadixItems; ++r) {
+    const unsigned i = base + r * 256 + threadIdx.x;
+    if (i < n) atomicAdd(&h[(keys[i] >> shift) & 255u], 1u);
+  }
+  __syncthreads();
+  blockhist[(size_t)threadIdx.x * nblocks + blockIdx.x] = h[threadIdx.x];
+}
+
+// exclusive scan of a uint array by one CTA of 1024 threads (in place)
+__global__ void __launch_bounds__(1024) k_scan_u32(unsigned* a, size_t n) {
+  __shared__ unsigned s_warp[33];
+  unsigned carry = 0;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (size_t i0 = 0; i0 < n; i0 += 4096) {
+    const size_t i = i0 + (size_t)threadIdx.x * 4;
+    unsigned v[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) v[k] = i + k < n ? a[i + k] : 0u;
+    const unsigned t = v[0] + v[1] + v[2] + v[3];
+    unsigned inc = t;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const unsigned u = __shfl_up_sync(0xffffffffu, inc, d);
+      if (lane >= d) inc += u;
+    }
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+      const unsigned w = s_warp[lane];
+      unsigned winc = w;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const unsigned u = __shfl_up_sync(0xffffffffu, winc, d);
+        if (lane >= d) winc += u;
+      }
+      s_warp[lane] = winc - w;
+      if (lane == 31) s_warp[32] = winc;
+    }
+    __syncthreads();
+    unsigned ex = carry + s_warp[warp] + inc - t;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      if (i + k < n) a[i + k] = ex;
+      ex += v[k];
+    }
+    carry += s_warp[32];
+    __syncthreads();
+  }
+}
+
+__global__ void __launch_bounds__(256) k_radix_scatter(const unsigned* keys, const unsigned* vals, unsigned n, int shift,
+                                                       const unsigned* blockhist, unsigned nblocks, unsigned* keys_out,
+                                                       unsigned* vals_out) {
+  __shared__ unsigned s_cnt[256 * 8];  // [digit][warp]
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned lt = lanemask_lt();
+  for (int k = threadIdx.x; k < 256 * 8; k += 256) s_cnt[k] = 0;
+  __syncthreads();
+  const unsigned base = blockIdx.x * kRadixChunk + warp * (32 * kRadixItems);
+  unsigned key[kRadixItems], val[kRadixItems], rank[kRadixItems];
+#pragma unroll
+  for (int r = 0; r < kRadixItems; ++r) {
+    const unsigned i = base + r * 32 + lane;
+    const bool have = i < n;
+    key[r] = have ? keys[i] : 0u;
+    val[r] = have ? vals[i] : 0u;
+    const unsigned d = have ? ((key[r] >> shift) & 255u) : (0x80000000u | (unsigned)lane);
+    const unsigned m = __match_any_sync(0xffffffffu, d);
+    const int leader = __ffs(m) - 1;
+    unsigned old = 0;
+    if (have && lane == leader) {
+      old = s_cnt[d * 8 + warp];
+      s_cnt[d * 8 + warp] = old + (unsigned)__popc(m);
+    }
+    old = __shfl_sync(0xffffffffu, old, leader);
+    rank[r] = have ? old + (unsigned)__popc(m & lt) : 0xffffffffu;
+    __syncwarp();
+  }
+  __syncthreads();
+  {
+    const unsigned d = threadIdx.x;
+    unsigned run = blockhist[(size_t)d * nblocks + blockIdx.x];
+#pragma unroll
+    for (int w = 0; w < 8; ++w) {
+      const unsigned t = s_cnt[d * 8 + w];
+      s_cnt[d * 8 + w] = run;
+      run += t;
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int r = 0; r < kRadixItems; ++r) {
+    if (rank[r] != 0xffffffffu) {
+      const unsigned d = (key[r] >> shift) & 255u;
+      const unsigned dst = s_cnt[d * 8 + warp] + rank[r];
+      keys_out[dst] = key[r];
+      vals_out[dst] = val[r];
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256) k_gather(Particles in, Particles out, const unsigned* perm, unsigned n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const unsigned j = perm[i];
+    out.x[i] = in.x[j]; out.vx[i] = in.vx[j]; out.vy[i] = in.vy[j]; out.vz[i] = in.vz[j];
+    out.cell[i] = in.cell[j]; out.pid[i] = in.pid[j]; out.sp[i] = in.sp[j];
+  }
+}
+
+int launch_load_sort(const Params& P, const Particles& in, const Particles& out, unsigned n, int have_pid,
+                     void* scratch, cudaStream_t s) {
+  if (n == 0) return 0;
+  int launches = 0;
+  const unsigned nblocks = (n + kRadixChunk - 1) / kRadixChunk;
+  unsigned* k0 = reinterpret_cast<unsigned*>(scratch);
+  unsigned* v0 = k0 + P.capacity;
+  unsigned* k1 = v0 + P.capacity;
+  unsigned* v1 = k1 + P.capacity;
+  unsigned* bh = v1 + P.capacity;
+  k_load_prepare<<<148 * 8, 256, 0, s>>>(P, in, n, have_pid, k0, v0);
+  ++launches;
+  int bits = 0;
+  while ((1ll << bits) < (long long)P.nc) ++bits;
+  for (int shift = 0; shift < bits; shift += 8) {
+    k_radix_hist<<<nblocks, 256, 0, s>>>(k0, n, shift, bh, nblocks);
+    k_scan_u32<<<1, 1024, 0, s>>>(bh, (size_t)256 * nblocks);
+    k_radix_scatter<<<nblocks, 256, 0, s>>>(k0, v0, n, shift, bh, nblocks, k1, v1);
+    launches += 3;
+    unsigned* t = k0; k0 = k1; k1 = t;
+    t = v0; v0 = v1; v1 = t;
+  }
+  k_gather<<<148 * 8, 256, 0, s>>>(in, out, v0, n);
+  return launches + 1;
+}
+
+size_t load_scratch_bytes(unsigned capacity) {
+  const size_t nblocks = ((size_t)capacity + kRadixChunk - 1) / kRadixChunk;
+  return (size_t)capacity * 16 + nblocks * 256 * 4 + 1024;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Moments: fixed-shape reduction, so the result is deterministic run to run.
+constexpr int kMomBlocks = 1024;
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+__global__ void __launch_bounds__(256) k_moments_partial(const __grid_constant__ Params P, Particles cur,
+                                                         double* partial /* [blocks][ns][3] */) {
+  __shared__ double s_red[8][kMaxSpecies * 3];
+  const unsigned n = P.st->n;
+  double acc[kMaxSpecies * 3];
+#pragma unroll
+  for (int k = 0; k < kMaxSpecies * 3; ++k) acc[k] = 0.0;
+  const size_t per = ((size_t)n + gridDim.x - 1) / gridDim.x;
+  const size_t lo = per * blockIdx.x, hi = min((size_t)n, lo + per);
+  for (size_t i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+    const int s = cur.sp[i];
+    const double vx = cur.vx[i], vy = cur.vy[i], vz = cur.vz[i];
+    const double v2 = (vx * vx + vy * vy) + vz * vz;
+#pragma unroll
+    for (int k = 0; k < kMaxSpecies; ++k) {
+      if (k == s) { acc[k * 3] += 1.0; acc[k * 3 + 1] += v2; acc[k * 3 + 2] += vx; }
+    }
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int k = 0; k < P.ns * 3; ++k) {
+    const double v = warp_sum(acc[k]);
+    if (lane == 0) s_red[warp][k] = v;
+  }
+  __syncthreads();
+  if ((int)threadIdx.x < P.ns * 3) {
+    double t = 0.0;
+    for (int w = 0; w < 8; ++w) t += s_red[w][threadIdx.x];
+    partial[(size_t)blockIdx.x * (kMaxSpecies * 3) + threadIdx.x] = t;
+  }
+}
+
+__global__ void __launch_bounds__(1024) k_moments_final(const __grid_constant__ Params P, const double* partial,
+                                                        int nblocks, double* out /* [ns][3] then field */) {
+  __shared__ double s_red[32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int k = 0; k < P.ns * 3; ++k) {
+    double v = 0.0;
+    for (int b = threadIdx.x; b < nblocks; b += blockDim.x) v += partial[(size_t)b * (kMaxSpecies * 3) + k];
+    v = warp_sum(v);
+    if (lane == 0) s_red[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+      double t = s_red[lane];
+      t = warp_sum(t);
+      if (lane == 0) out[k] = t;
+    }
+    __syncthreads();
+  }
+  // field energy sum g_j E_j^2
+  double v = 0.0;
+  for (int j = threadIdx.x; j < P.ng; j += blockDim.x) {
+    const double g = (P.bc && (j == 0 || j == P.nc)) ? 0.5 : 1.0;
+    const double e = P.E[j];
+    v += g * (e * e);
+  }
+  v = warp_sum(v);
+  if (lane == 0) s_red[warp] = v;
+  __syncthreads();
+  if (warp == 0) {
+    double t = warp_sum(s_red[lane]);
+    if (lane == 0) out[kMaxSpecies * 3] = t;
+  }
+}
+
+int launch_moments(const Params& P, const Particles& cur, double* partial, double* out, cudaStream_t s) {
+  k_moments_partial<<<kMomBlocks, 256, 0, s>>>(P, cur, partial);
+  k_moments_final<<<1, 1024, 0, s>>>(P, partial, kMomBlocks, out);
+  return 2;
+}
+size_t moments_scratch_bytes() { return ((size_t)kMomBlocks + 2) * kMaxSpecies * 3 * 8 + 256; }
+
+}  // namespace bit1

@@ -1,0 +1,13 @@
+// Host-callable launchers of the load-time and diagnostic kernels (defined in aux_kernels.cu).
+#pragma once
+#include "common.cuh"
+
+namespace bit1 {
+// validate + cell index + general stable sort by cell of `in` (n particles) into `out`
+int launch_load_sort(const Params& P, const Particles& in, const Particles& out, unsigned n, int have_pid,
+                     void* scratch, cudaStream_t s);
+size_t load_scratch_bytes(unsigned capacity);
+// out: [kMaxSpecies*3] = (count, sum v^2, sum vx) per species, then sum g_j E_j^2
+int launch_moments(const Params& P, const Particles& cur, double* partial, double* out, cudaStream_t s);
+size_t moments_scratch_bytes();
+}  // namespace bit1

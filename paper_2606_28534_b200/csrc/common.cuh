@@ -1,0 +1,111 @@
+// Shared device/host structures of libbit1 (CUDA side only; the CPU oracle shares nothing with this).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace bit1 {
+
+constexpr int kMaxSpecies = 8;
+constexpr int kThreads = 256;             // threads per CTA of the particle kernels
+constexpr int kItems = 8;                 // particles per thread per tile
+constexpr int kTile = kThreads * kItems;  // 2048 particles per tile
+constexpr int kWarps = kThreads / 32;
+constexpr int kWarpSpan = 32 * kItems;    // contiguous particles handled by one warp
+constexpr int kWCap = 512;                // max cells in a tile's window (smem histogram bins)
+
+// overflow ("far mover" / birth) key: cell(28) | cls(2) | ord(34)
+constexpr int kOrdBits = 34;
+constexpr int kClsShift = kOrdBits;
+constexpr int kCellShift = kOrdBits + 2;
+constexpr unsigned long long kInvalidKey = ~0ull;
+
+constexpr unsigned kFlagCapacity = 1u, kFlagEscape = 2u, kFlagOverflow = 4u;
+constexpr unsigned kElastic = 1u, kIonise = 2u, kCx = 4u, kIonProduct = 8u, kElectronProduct = 16u,
+                   kTargetMaxwellian = 32u;
+constexpr int kSrcNone = 0, kSrcSelf = 1, kSrcPair = 2;
+
+struct SpeciesP {
+  double h, tx, ty, tz, sx, sy, sz;
+  double src_vth, pnull, numax, kin_eV, two_e_over_m, el_loss;
+  long long Q;
+  int sign;
+  unsigned flags;
+  int src_mode, src_partner;
+};
+
+// SoA particle store: 41 B per particle.
+struct Particles {
+  double *x, *vx, *vy, *vz;
+  int *cell;
+  unsigned *pid;
+  unsigned char *sp;
+};
+
+struct OvfRec {  // one far mover or birth, full state (48 B)
+  double x, vx, vy, vz;
+  unsigned pid;
+  unsigned sp;
+};
+
+// Mutable device-side counters; every kernel reads n/step from here so that bit1_step never syncs.
+struct DevState {
+  unsigned long long step;
+  unsigned n;         // live particles at step start
+  unsigned n_next;    // live particles after this step's sort
+  unsigned next_pid;
+  unsigned ovf_count; // far movers + births appended this step
+  unsigned flags;     // sticky
+  unsigned freeze_field;
+  unsigned load_error;
+  unsigned ovf_valid; // side-list entries that k_mid placed (ovf_count minus dropped births)
+  unsigned long long wall_count[2][kMaxSpecies];
+  long long wall_charge[2];
+  unsigned long long nu_overflow, dir_fallback, escape, births, reinject;
+  unsigned long long candidates[kMaxSpecies];
+  unsigned long long events[kMaxSpecies][3];
+  unsigned long long far_movers, max_far_movers;
+  long long rho_total;
+};
+
+struct Params {
+  int nc, bc, ng, ns;
+  int R;         // window radius in cells
+  int n_sig, n_norm;
+  int sp_ep, sp_ip;
+  int dep_u32;   // 1: every Q_s * kTile < 2^32, shared-memory deposit counters may be 32-bit
+  unsigned seed_lo, seed_hi;
+  unsigned capacity, ovf_cap, ovf_pow2;
+  int max_tiles;
+  double inv_dx, L, dt, dx, area;
+  double src_lo, src_span;
+  double n0, vth_n, E_ion, dE_eV;
+  double Kphi, KE;
+  double field_J_factor;
+  const double *sig_el, *sig_ion, *sig_cx, *inv_norm;
+  DevState *st;
+  // grids
+  long long *dens;  // ns * ng
+  long long *rho;   // ng
+  double *phi, *E;  // nc + 1
+  int *cell_count;  // nc
+  int *cell_start;  // nc + 1
+  int *cell_base;   // nc: cell_start + far movers placed before the windowed particles
+  int *ovf_before;  // nc
+  // tiles
+  int2 *tile_desc;      // (clo, chi) of each tile at step start
+  unsigned *tile_hist;  // banded histogram rows, row t at clo_t + t*(2R+1)
+  // overflow list
+  unsigned long long *ovf_key;  // ovf_pow2 (unsorted, then sorted in place)
+  unsigned *ovf_idx;            // ovf_pow2: record index of sorted position
+  OvfRec *ovf_rec;              // ovf_cap
+  int *ovf_dst;                 // ovf_pow2: destination slot of sorted position (-1: dropped)
+  unsigned long long *tmp_key;  // ovf_pow2 scratch (birth ordering)
+  unsigned *tmp_idx;            // ovf_pow2 scratch
+  SpeciesP sp[kMaxSpecies];
+};
+
+__host__ __device__ inline size_t tile_row_offset(int clo, int tile, int R) {
+  return (size_t)clo + (size_t)tile * (size_t)(2 * R + 1);
+}
+
+}  // namespace bit1

@@ -1,0 +1,721 @@
+// The four kernels of one timestep:
+//   k_pass_a  mover: advance every particle, banded per-tile histogram of new cells, side list of far
+//             movers and births                                   (PAPER.md:111 move0/moveb)
+//   k_mid     order the side list, counts -> cell_start           (row a4, scan part)
+//   k_pass_b  arranger: stable ranks inside the tile, scatter to the sorted position with the charge
+//             deposition fused                                    (rows a4-a5; PAPER.md:111 arrj/narrj)
+//   k_field   exact integer-scan Poisson solve -> phi, E          (row a6; PAPER.md:33 step (iii))
+#include "advance.cuh"
+#include "step_kernels.h"
+
+namespace bit1 {
+
+// ---------------------------------------------------------------------------------------------
+// tile geometry shared by both passes
+struct TileWin {
+  int clo, chi, wlo, W;
+};
+__device__ __forceinline__ TileWin make_window(int clo, int chi, int R) {
+  TileWin t;
+  t.clo = clo; t.chi = chi; t.wlo = clo - R;
+  const int w = chi - clo + 1 + 2 * R;
+  t.W = w < kWCap ? w : kWCap;
+  return t;
+}
+
+__device__ __forceinline__ void load_species(const Params& P, SpeciesP* s_sp) {
+  const int words = P.ns * (int)(sizeof(SpeciesP) / 8);
+  const unsigned long long* src = reinterpret_cast<const unsigned long long*>(P.sp);
+  unsigned long long* dst = reinterpret_cast<unsigned long long*>(s_sp);
+  for (int i = threadIdx.x; i < words; i += blockDim.x) dst[i] = src[i];
+}
+
+// ---------------------------------------------------------------------------------------------
+// Pass A.  VARIANT 1 writes the advanced state back in place; VARIANT 2 writes nothing per particle.
+template <int VARIANT>
+__global__ void __launch_bounds__(kThreads) k_pass_a(const __grid_constant__ Params P, Particles cur) {
+  __shared__ SpeciesP s_sp[kMaxSpecies];
+  __shared__ unsigned s_hist[kWCap];
+  __shared__ double s_E[kWCap + 2];
+  load_species(P, s_sp);
+  const unsigned n = P.st->n;
+  const unsigned long long step = P.st->step;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+
+  // the deposition of this step accumulates into dens: clear it here (nobody reads it during pass A)
+  {
+    const size_t tot = (size_t)P.ns * (size_t)P.ng;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < tot; i += (size_t)gridDim.x * blockDim.x)
+      P.dens[i] = 0;
+  }
+  const int ntiles = (int)((n + kTile - 1) / kTile);
+  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const unsigned base = (unsigned)tile * kTile;
+    const unsigned cnt = min((unsigned)kTile, n - base);
+    const int clo = cur.cell[base], chi = cur.cell[base + cnt - 1];
+    const TileWin tw = make_window(clo, chi, P.R);
+    for (int k = threadIdx.x; k < tw.W; k += kThreads) s_hist[k] = 0;
+    const int ecount = chi - clo + 2;
+    const bool e_staged = ecount <= kWCap + 2;
+    if (e_staged)
+      for (int k = threadIdx.x; k < ecount; k += kThreads) s_E[k] = P.E[clo + k];
+    const double* Eptr = e_staged ? (s_E - clo) : P.E;
+    __syncthreads();
+
+#pragma unroll 2
+    for (int r = 0; r < kItems; ++r) {
+      const unsigned off = (unsigned)(warp * kWarpSpan + r * 32 + lane);
+      const bool have = off < cnt;
+      unsigned key = 0x80000000u | (unsigned)lane;  // unique: matches nobody
+      if (have) {
+        const unsigned i = base + off;
+        double x = cur.x[i], vx = cur.vx[i], vy = cur.vy[i], vz = cur.vz[i];
+        int c = cur.cell[i];
+        const int sp = cur.sp[i];
+        const unsigned pid = cur.pid[i];
+        advance<true>(P, s_sp, step, Eptr, sp, pid, i, x, vx, vy, vz, c);
+        if (VARIANT == 1) {
+          cur.x[i] = x; cur.vx[i] = vx; cur.vy[i] = vy; cur.vz[i] = vz; cur.cell[i] = c;
+        }
+        if (c >= 0) {
+          const int k = c - tw.wlo;
+          if (k >= 0 && k < tw.W) key = (unsigned)k;
+          else emit_record(P, make_key(c, c < tw.wlo ? 1u : 0u, (unsigned long long)i), x, vx, vy, vz, pid, sp);
+        }
+      }
+      const unsigned m = __match_any_sync(0xffffffffu, key);
+      if (!(key & 0x80000000u) && lane == __ffs(m) - 1) atomicAdd(&s_hist[key], (unsigned)__popc(m));
+    }
+    __syncthreads();
+    unsigned* row = P.tile_hist + tile_row_offset(clo, tile, P.R);
+    for (int k = threadIdx.x; k < tw.W; k += kThreads) {
+      const unsigned h = s_hist[k];
+      row[k] = h;
+      const int c = tw.wlo + k;
+      if (h && c >= 0 && c < P.nc) atomicAdd(&P.cell_count[c], (int)h);
+    }
+    if (threadIdx.x == 0) P.tile_desc[tile] = make_int2(clo, chi);
+    __syncthreads();
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// k_mid: single CTA.
+constexpr int kMidThreads = 1024;
+constexpr int kSortSmem = 2048;
+
+__device__ void cta_bitonic(unsigned long long* key, unsigned* val, unsigned n) {
+  for (unsigned k = 2; k <= n; k <<= 1) {
+    for (unsigned j = k >> 1; j > 0; j >>= 1) {
+      for (unsigned i = threadIdx.x; i < n; i += blockDim.x) {
+        const unsigned ixj = i ^ j;
+        if (ixj > i) {
+          const unsigned long long a = key[i], b = key[ixj];
+          const bool asc = (i & k) == 0;
+          if ((a > b) == asc) {
+            key[i] = b; key[ixj] = a;
+            const unsigned t = val[i]; val[i] = val[ixj]; val[ixj] = t;
+          }
+        }
+      }
+      __syncthreads();
+    }
+  }
+}
+
+__device__ __forceinline__ unsigned next_pow2(unsigned v) {
+  unsigned p = 1;
+  while (p < v) p <<= 1;
+  return p;
+}
+
+__device__ __forceinline__ unsigned lower_bound_u64(const unsigned long long* a, unsigned n, unsigned long long v) {
+  unsigned lo = 0, hi = n;
+  while (lo < hi) {
+    const unsigned mid = (lo + hi) >> 1;
+    if (a[mid] < v) lo = mid + 1; else hi = mid;
+  }
+  return lo;
+}
+
+// sort (key, val) pairs of length P2 (power of two, padded with kInvalidKey) held in global memory
+__device__ void cta_sort(unsigned long long* gkey, unsigned* gval, unsigned P2, unsigned long long* s_key,
+                         unsigned* s_val) {
+  if (P2 <= (unsigned)kSortSmem) {
+    for (unsigned i = threadIdx.x; i < P2; i += blockDim.x) { s_key[i] = gkey[i]; s_val[i] = gval[i]; }
+    __syncthreads();
+    cta_bitonic(s_key, s_val, P2);
+    for (unsigned i = threadIdx.x; i < P2; i += blockDim.x) { gkey[i] = s_key[i]; gval[i] = s_val[i]; }
+    __syncthreads();
+  } else {
+    __syncthreads();
+    cta_bitonic(gkey, gval, P2);  // robustness path: global memory, one CTA
+  }
+}
+
+__device__ int block_exclusive_scan_int(int v, int* s_warp, int* total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int inc = v;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const int t = __shfl_up_sync(0xffffffffu, inc, d);
+    if (lane >= d) inc += t;
+  }
+  if (lane == 31) s_warp[warp] = inc;
+  __syncthreads();
+  if (warp == 0) {
+    int w = lane < (int)(blockDim.x >> 5) ? s_warp[lane] : 0;
+    int winc = w;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int t = __shfl_up_sync(0xffffffffu, winc, d);
+      if (lane >= d) winc += t;
+    }
+    s_warp[lane] = winc - w;
+    if (lane == 31) s_warp[32] = winc;
+  }
+  __syncthreads();
+  const int res = s_warp[warp] + inc - v;
+  *total = s_warp[32];
+  __syncthreads();
+  return res;
+}
+
+__global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Params P) {
+  __shared__ unsigned long long s_key[kSortSmem];
+  __shared__ unsigned s_val[kSortSmem];
+  __shared__ int s_warp[33];
+  __shared__ unsigned s_cnt;
+  DevState* st = P.st;
+  const unsigned n = st->n;
+  unsigned M = st->ovf_count;
+  if (M > P.ovf_cap) M = P.ovf_cap;
+  const unsigned P2 = next_pow2(M > 1 ? M : 1);
+  unsigned Mv = 0;
+
+  if (M > 0) {
+    // (a) births: order by (parent index, kind), assign pid = next_pid + r, drop those beyond capacity
+    unsigned nb_local = 0;
+    for (unsigned i = threadIdx.x; i < P2; i += blockDim.x) {
+      unsigned long long bk = kInvalidKey;
+      if (i < M) {
+        const unsigned long long key = P.ovf_key[i];
+        if (((key >> kClsShift) & 3ull) == 2ull) { bk = key & ((1ull << kOrdBits) - 1ull); nb_local++; }
+      }
+      P.tmp_key[i] = bk;
+      P.tmp_idx[i] = i;
+    }
+    if (threadIdx.x == 0) s_cnt = 0;
+    __syncthreads();
+    if (nb_local) atomicAdd(&s_cnt, nb_local);
+    __syncthreads();
+    const unsigned B = s_cnt;
+    __syncthreads();
+    if (B > 0) {
+      cta_sort(P.tmp_key, P.tmp_idx, P2, s_key, s_val);
+      const unsigned room = P.capacity > n ? P.capacity - n : 0u;
+      const unsigned next_pid = st->next_pid;
+      for (unsigned r = threadIdx.x; r < B; r += blockDim.x) {
+        const unsigned rec = P.tmp_idx[r];
+        if (r < room) P.ovf_rec[rec].pid = next_pid + r;
+        else P.ovf_key[rec] = kInvalidKey;
+      }
+      __syncthreads();
+      if (threadIdx.x == 0) {
+        const unsigned created = B < room ? B : room;
+        st->next_pid = next_pid + created;
+        st->births += created;
+        if (B > room) st->flags |= kFlagCapacity;
+      }
+    }
+    // (b) order the whole list by (cell, class, order)
+    for (unsigned i = threadIdx.x; i < P2; i += blockDim.x) {
+      if (i >= M) P.ovf_key[i] = kInvalidKey;
+      P.ovf_idx[i] = i;
+    }
+    __syncthreads();
+    cta_sort(P.ovf_key, P.ovf_idx, P2, s_key, s_val);
+    Mv = lower_bound_u64(P.ovf_key, P2, kInvalidKey);
+    // (d) groups per cell: rank inside the group, group size joins the cell count
+    for (unsigned p = threadIdx.x; p < Mv; p += blockDim.x) {
+      const unsigned long long key = P.ovf_key[p];
+      const unsigned long long c = key >> kCellShift;
+      const unsigned lb = lower_bound_u64(P.ovf_key, Mv, c << kCellShift);
+      const unsigned ub = lower_bound_u64(P.ovf_key, Mv, (c + 1ull) << kCellShift);
+      const unsigned cls = (unsigned)((key >> kClsShift) & 3ull);
+      if (p == lb) {
+        const unsigned ub0 = lower_bound_u64(P.ovf_key, Mv, (c << kCellShift) | (1ull << kClsShift));
+        P.cell_count[c] += (int)(ub - lb);
+        P.ovf_before[c] = (int)(ub0 - lb);
+      }
+      // class 0 counts from the cell's start, classes 1-2 from the cell's end
+      P.ovf_dst[p] = cls == 0 ? (int)(p - lb) : (int)(p - lb) - (int)(ub - lb);
+    }
+    __syncthreads();
+  }
+
+  // (e) exclusive scan of the cell counts
+  int carry = 0;
+  const int nc = P.nc;
+  for (int c0 = 0; c0 < nc; c0 += kMidThreads * 4) {
+    const int c = c0 + (int)threadIdx.x * 4;
+    int v[4], b[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const bool in = c + k < nc;
+      v[k] = in ? P.cell_count[c + k] : 0;
+      b[k] = in ? P.ovf_before[c + k] : 0;
+    }
+    const int tsum = (v[0] + v[1]) + (v[2] + v[3]);
+    int total;
+    int ex = carry + block_exclusive_scan_int(tsum, s_warp, &total);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      if (c + k < nc) {
+        P.cell_start[c + k] = ex;
+        P.cell_base[c + k] = ex + b[k];
+        P.cell_count[c + k] = 0;
+        P.ovf_before[c + k] = 0;
+      }
+      ex += v[k];
+    }
+    carry += total;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    P.cell_start[nc] = carry;
+    st->n_next = (unsigned)carry;
+    st->ovf_valid = Mv;
+    st->far_movers += M;
+    if (M > st->max_far_movers) st->max_far_movers = M;
+  }
+  // (f) destinations of the side-list entries (reads cell_start written above by this CTA)
+  __threadfence_block();
+  __syncthreads();
+  for (unsigned p = threadIdx.x; p < Mv; p += blockDim.x) {
+    const unsigned long long key = P.ovf_key[p];
+    const int c = (int)(key >> kCellShift);
+    const unsigned cls = (unsigned)((key >> kClsShift) & 3ull);
+    const int rel = P.ovf_dst[p];
+    P.ovf_dst[p] = (cls == 0 ? P.cell_start[c] : P.cell_start[c + 1]) + rel;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Pass B.  Dynamic shared memory: s_wcnt[kWCap][kWarps], s_base[kWCap], s_dens[kWCap+1][ns], s_E.
+template <int VARIANT>
+__global__ void __launch_bounds__(kThreads, 2)
+k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  __shared__ SpeciesP s_sp[kMaxSpecies];
+  unsigned* s_wcnt = reinterpret_cast<unsigned*>(smem_raw);          // [kWCap][kWarps]
+  int* s_base = reinterpret_cast<int*>(s_wcnt + kWarps * kWCap);     // [kWCap]
+  unsigned* s_dens = reinterpret_cast<unsigned*>(s_base + kWCap);    // [kWCap + 1][ns]
+  double* s_E = reinterpret_cast<double*>(s_dens + ((P.ns * (kWCap + 1) + 1) & ~1));  // [kWCap + 2] (V2)
+  load_species(P, s_sp);
+  const unsigned n = P.st->n;
+  const unsigned long long step = P.st->step;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned lt = lanemask_lt();
+  const int ntiles = (int)((n + kTile - 1) / kTile);
+  __syncthreads();
+
+  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const unsigned base = (unsigned)tile * kTile;
+    const unsigned cnt = min((unsigned)kTile, n - base);
+    const int2 d = P.tile_desc[tile];
+    const TileWin tw = make_window(d.x, d.y, P.R);
+    for (int k = threadIdx.x; k < kWarps * tw.W; k += kThreads) s_wcnt[k] = 0;
+    for (int k = threadIdx.x; k < P.ns * (tw.W + 1); k += kThreads) s_dens[k] = 0;
+    const double* Eptr = P.E;
+    if (VARIANT == 2) {
+      const int ecount = tw.chi - tw.clo + 2;
+      if (ecount <= kWCap + 2) {
+        for (int k = threadIdx.x; k < ecount; k += kThreads) s_E[k] = P.E[tw.clo + k];
+        Eptr = s_E - tw.clo;
+      }
+    }
+    __syncthreads();
+
+    // phase 1: load (and, for V2, recompute) every particle of the tile; stable rank inside the warp
+    double x[kItems], vx[kItems], vy[kItems], vz[kItems];
+    unsigned pid[kItems];
+    int key[kItems];        // window-relative new cell, or -1 when the particle is not placed by this tile
+    unsigned rank[kItems];
+    unsigned char sp[kItems];
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) {
+      const unsigned off = (unsigned)(warp * kWarpSpan + r * 32 + lane);
+      key[r] = -1;
+      if (off < cnt) {
+        const unsigned i = base + off;
+        x[r] = cur.x[i]; vx[r] = cur.vx[i]; vy[r] = cur.vy[i]; vz[r] = cur.vz[i];
+        pid[r] = cur.pid[i]; sp[r] = cur.sp[i];
+        int c = cur.cell[i];
+        if (VARIANT == 2) advance<false>(P, s_sp, step, Eptr, sp[r], pid[r], i, x[r], vx[r], vy[r], vz[r], c);
+        if (c >= 0) {
+          const int k = c - tw.wlo;
+          if (k >= 0 && k < tw.W) key[r] = k;
+        }
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) {
+      const unsigned mk = key[r] >= 0 ? (unsigned)key[r] : (0x80000000u | (unsigned)lane);
+      const unsigned m = __match_any_sync(0xffffffffu, mk);
+      const int leader = __ffs(m) - 1;
+      unsigned old = 0;
+      if (key[r] >= 0 && lane == leader) {
+        old = s_wcnt[key[r] * kWarps + warp];
+        s_wcnt[key[r] * kWarps + warp] = old + (unsigned)__popc(m);
+      }
+      old = __shfl_sync(0xffffffffu, old, leader);
+      rank[r] = old + (unsigned)__popc(m & lt);
+      __syncwarp();
+    }
+
+    // look-back: particles that earlier tiles put into each cell of this window
+    for (int k = warp; k < tw.W; k += kWarps) {
+      const int c = tw.wlo + k;
+      int pre = 0;
+      if (c >= 0 && c < P.nc) {
+        for (int t0 = tile - 1; t0 >= 0; t0 -= 32) {
+          const int t = t0 - lane;
+          bool covers = false;
+          if (t >= 0) {
+            const int2 dd = P.tile_desc[t];
+            const TileWin w2 = make_window(dd.x, dd.y, P.R);
+            covers = c < w2.wlo + w2.W;  // wlo is monotone in t, so c >= w2.wlo always holds
+            if (covers) pre += (int)P.tile_hist[tile_row_offset(dd.x, t, P.R) + (size_t)(c - w2.wlo)];
+          }
+          // windows' upper ends are monotone: once a tile misses c every earlier one does
+          if (__any_sync(0xffffffffu, !covers)) break;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) pre += __shfl_xor_sync(0xffffffffu, pre, o);
+        pre += P.cell_base[c];
+      }
+      if (lane == 0) s_base[k] = pre;
+    }
+    __syncthreads();
+    // exclusive scan over the warps of the tile, per cell: s_wcnt becomes the destination base
+    for (int k = threadIdx.x; k < tw.W; k += kThreads) {
+      unsigned run = (unsigned)s_base[k];
+#pragma unroll
+      for (int w = 0; w < kWarps; ++w) {
+        const unsigned t = s_wcnt[k * kWarps + w];
+        s_wcnt[k * kWarps + w] = run;
+        run += t;
+      }
+    }
+    __syncthreads();
+
+    // phase 2: scatter + deposit
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) {
+      if (key[r] >= 0) {
+        const unsigned dst = s_wcnt[key[r] * kWarps + warp] + rank[r];
+        const int c = tw.wlo + key[r];
+        nxt.x[dst] = x[r]; nxt.vx[dst] = vx[r]; nxt.vy[dst] = vy[r]; nxt.vz[dst] = vz[r];
+        nxt.cell[dst] = c; nxt.pid[dst] = pid[r]; nxt.sp[dst] = sp[r];
+        const unsigned Q = (unsigned)s_sp[sp[r]].Q;
+        const unsigned a = deposit_a(x[r], c, P.inv_dx, Q);
+        if (P.dep_u32) {
+          atomicAdd(&s_dens[key[r] * P.ns + sp[r]], Q - a);
+          atomicAdd(&s_dens[(key[r] + 1) * P.ns + sp[r]], a);
+        } else {
+          int j1 = c + 1;
+          if (!P.bc && j1 == P.nc) j1 = 0;
+          atomicAdd((unsigned long long*)&P.dens[(size_t)sp[r] * P.ng + c], (unsigned long long)(Q - a));
+          atomicAdd((unsigned long long*)&P.dens[(size_t)sp[r] * P.ng + j1], (unsigned long long)a);
+        }
+      }
+    }
+    __syncthreads();
+    if (P.dep_u32) {
+      for (int k = threadIdx.x; k < P.ns * (tw.W + 1); k += kThreads) {
+        const unsigned v = s_dens[k];
+        if (v) {
+          const int kk = k / P.ns, s = k - kk * P.ns;
+          int j = tw.wlo + kk;
+          if (!P.bc && j == P.nc) j = 0;
+          atomicAdd((unsigned long long*)&P.dens[(size_t)s * P.ng + j], (unsigned long long)v);
+        }
+      }
+    }
+    __syncthreads();
+  }
+
+  // side list: far movers and births go to the slots k_mid computed for them
+  const unsigned Mv = P.st->ovf_valid;
+  for (unsigned p = blockIdx.x * blockDim.x + threadIdx.x; p < Mv; p += gridDim.x * blockDim.x) {
+    const int dst = P.ovf_dst[p];
+    const OvfRec rec = P.ovf_rec[P.ovf_idx[p]];
+    const int c = (int)(P.ovf_key[p] >> kCellShift);
+    nxt.x[dst] = rec.x; nxt.vx[dst] = rec.vx; nxt.vy[dst] = rec.vy; nxt.vz[dst] = rec.vz;
+    nxt.cell[dst] = c; nxt.pid[dst] = rec.pid; nxt.sp[dst] = (unsigned char)rec.sp;
+    const unsigned Q = (unsigned)s_sp[rec.sp].Q;
+    const unsigned a = deposit_a(rec.x, c, P.inv_dx, Q);
+    int j1 = c + 1;
+    if (!P.bc && j1 == P.nc) j1 = 0;
+    atomicAdd((unsigned long long*)&P.dens[(size_t)rec.sp * P.ng + c], (unsigned long long)(Q - a));
+    atomicAdd((unsigned long long*)&P.dens[(size_t)rec.sp * P.ng + j1], (unsigned long long)a);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Standalone deposit (load / restart; also SURVEY 8(a) row a5 as its own kernel).
+__global__ void __launch_bounds__(kThreads) k_deposit(const __grid_constant__ Params P, Particles cur) {
+  const unsigned n = P.st->n;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const int c = cur.cell[i], s = cur.sp[i];
+    const unsigned Q = (unsigned)P.sp[s].Q;
+    const unsigned a = deposit_a(cur.x[i], c, P.inv_dx, Q);
+    // neighbours in the sorted array mostly share (cell, species): one atomic per run inside the warp
+    const unsigned gk = (unsigned)c * kMaxSpecies + (unsigned)s;
+    const unsigned act = __activemask();
+    const unsigned m = __match_any_sync(act, gk);
+    unsigned long long lo = Q - a, hi = a;
+    // segmented sum over the match group (small groups: loop over members)
+    unsigned long long slo = 0, shi = 0;
+    for (unsigned mm = m; mm; mm &= mm - 1) {
+      const int src = __ffs(mm) - 1;
+      slo += __shfl_sync(m, lo, src);
+      shi += __shfl_sync(m, hi, src);
+    }
+    if ((int)(threadIdx.x & 31) == __ffs(m) - 1) {
+      int j1 = c + 1;
+      if (!P.bc && j1 == P.nc) j1 = 0;
+      atomicAdd((unsigned long long*)&P.dens[(size_t)s * P.ng + c], slo);
+      atomicAdd((unsigned long long*)&P.dens[(size_t)s * P.ng + j1], shi);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// k_field: rho = sum_s sign_s dens_s; exact double prefix sum -> phi, E.  Single CTA.
+constexpr int kFieldThreads = 1024;
+constexpr int kFieldItems = 8;
+typedef __int128 i128;
+
+__device__ __forceinline__ i128 shfl_up_128(i128 v, int d) {
+  unsigned long long lo = (unsigned long long)v, hi = (unsigned long long)((unsigned __int128)v >> 64);
+  lo = __shfl_up_sync(0xffffffffu, lo, d);
+  hi = __shfl_up_sync(0xffffffffu, hi, d);
+  return (i128)(((unsigned __int128)hi << 64) | (unsigned __int128)lo);
+}
+__device__ __forceinline__ i128 shfl_xor_128(i128 v, int d) {
+  unsigned long long lo = (unsigned long long)v, hi = (unsigned long long)((unsigned __int128)v >> 64);
+  lo = __shfl_xor_sync(0xffffffffu, lo, d);
+  hi = __shfl_xor_sync(0xffffffffu, hi, d);
+  return (i128)(((unsigned __int128)hi << 64) | (unsigned __int128)lo);
+}
+
+// exclusive scan over the CTA of one int128 per thread; *total = sum over the CTA
+__device__ i128 block_exclusive_scan_128(i128 v, i128* s_warp, i128* total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  i128 inc = v;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const i128 t = shfl_up_128(inc, d);
+    if (lane >= d) inc += t;
+  }
+  if (lane == 31) s_warp[warp] = inc;
+  __syncthreads();
+  if (warp == 0) {
+    const i128 w = lane < (int)(blockDim.x >> 5) ? s_warp[lane] : (i128)0;
+    i128 winc = w;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const i128 t = shfl_up_128(winc, d);
+      if (lane >= d) winc += t;
+    }
+    s_warp[lane] = winc - w;
+    if (lane == 31) s_warp[32] = winc;
+  }
+  __syncthreads();
+  const i128 res = s_warp[warp] + inc - v;
+  *total = s_warp[32];
+  __syncthreads();
+  return res;
+}
+
+__device__ i128 block_sum_128(i128 v, i128* s_warp) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += shfl_xor_128(v, o);
+  if (lane == 0) s_warp[warp] = v;
+  __syncthreads();
+  i128 t = 0;
+  if (warp == 0) {
+    t = lane < (int)(blockDim.x >> 5) ? s_warp[lane] : (i128)0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += shfl_xor_128(t, o);
+    if (lane == 0) s_warp[32] = t;
+  }
+  __syncthreads();
+  t = s_warp[32];
+  __syncthreads();
+  return t;
+}
+
+__global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__ Params P, int commit_step) {
+  __shared__ i128 s_warp[33];
+  const int nc = P.nc, ng = P.ng, bc = P.bc;
+  DevState* st = P.st;
+  // phase A: rho, total charge, and T_nc = sum_{j=1}^{nc-1} (nc - j) R_j as plain reductions
+  i128 tot = 0, wsum = 0;
+  for (int j = threadIdx.x; j < ng; j += blockDim.x) {
+    long long r = 0;
+    for (int s = 0; s < P.ns; ++s) r += (long long)P.sp[s].sign * P.dens[(size_t)s * ng + j];
+    P.rho[j] = r;
+    tot += (i128)r;
+    if (j >= 1 && j <= nc - 1) wsum += (i128)(nc - j) * (i128)r;
+  }
+  tot = block_sum_128(tot, s_warp);
+  wsum = block_sum_128(wsum, s_warp);
+  if (threadIdx.x == 0) st->rho_total = (long long)tot;
+  const bool frozen = st->freeze_field != 0;
+  if (!frozen) {
+    // periodic: R'_j = nc R_j - tot  =>  T_nc' = nc * wsum - tot * nc (nc - 1) / 2
+    const i128 Tn = bc ? wsum : (i128)nc * wsum - tot * (((i128)nc * (i128)(nc - 1)) / 2);
+    // phase B: S_j = sum_{k=1..j} R_k (S_0 = 0), T_j = sum_{k<j} S_k, chunked over elements j = 1..jmax
+    const int jmax = bc ? nc : nc - 1;
+    i128 carryS = 0, carryT = 0;  // S_{j0-1}, T_{j0} at the chunk's first element j0
+    if (threadIdx.x == 0) {
+      // node 0
+      P.phi[0] = P.Kphi * dbl128((i128)0);
+      if (bc) P.E[0] = P.KE * dbl128(-2 * Tn - 2 * (i128)nc * (i128)P.rho[0]);
+    }
+    for (int j0 = 1; j0 <= jmax; j0 += kFieldThreads * kFieldItems) {
+      const int jb = j0 + (int)threadIdx.x * kFieldItems;
+      i128 R[kFieldItems], Sl[kFieldItems];
+      i128 run = 0;
+#pragma unroll
+      for (int k = 0; k < kFieldItems; ++k) {
+        const int j = jb + k;
+        i128 r = 0;
+        if (j <= jmax) r = bc ? (i128)P.rho[j] : (i128)nc * (i128)P.rho[j] - tot;
+        R[k] = r;
+        run += r;
+        Sl[k] = run;  // inclusive local
+      }
+      i128 chunkS;
+      const i128 exS = carryS + block_exclusive_scan_128(run, s_warp, &chunkS);
+      // S_j = exS + Sl[k]; thread sum of S over its elements
+      i128 tsumS = 0;
+#pragma unroll
+      for (int k = 0; k < kFieldItems; ++k) {
+        const int j = jb + k;
+        Sl[k] = exS + Sl[k];
+        if (j <= jmax) tsumS += Sl[k];
+      }
+      i128 chunkSS;
+      i128 T = carryT + block_exclusive_scan_128(tsumS, s_warp, &chunkSS);  // T at this thread's first element
+#pragma unroll
+      for (int k = 0; k < kFieldItems; ++k) {
+        const int j = jb + k;
+        if (j <= jmax) {
+          const i128 Sj = Sl[k], Sm = Sl[k] - R[k];
+          P.phi[j] = P.Kphi * dbl128((i128)j * Tn - (i128)nc * T);
+          if (bc) {
+            if (j < nc) P.E[j] = P.KE * dbl128((i128)nc * (Sm + Sj) - 2 * Tn);
+            else P.E[nc] = P.KE * dbl128(2 * (i128)nc * Sm - 2 * Tn + 2 * (i128)nc * (i128)P.rho[nc]);
+          } else {
+            P.E[j] = P.KE * dbl128((i128)nc * (Sm + Sj) - 2 * Tn);
+          }
+          T += Sj;
+        }
+      }
+      carryS += chunkS;
+      carryT += chunkSS;
+    }
+    if (!bc && threadIdx.x == 0) {
+      // node 0 of the periodic grid: S_{-1} = S_{nc-1} (= carryS after the loop), S_0 = 0; ghosts at nc
+      P.E[0] = P.KE * dbl128((i128)nc * (carryS + (i128)0) - 2 * Tn);
+      P.E[nc] = P.E[0];
+      P.phi[nc] = P.phi[0];
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    st->n = st->n_next;
+    if (commit_step) st->step += 1ull;
+    st->ovf_count = 0;
+    st->ovf_valid = 0;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host-side launchers
+static int g_sms = 0;
+static int sm_count() {
+  if (!g_sms) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (g_sms <= 0) g_sms = 148;
+  }
+  return g_sms;
+}
+
+size_t pass_b_smem_bytes(int ns) {
+  size_t words = (size_t)kWarps * kWCap + kWCap + (((size_t)ns * (kWCap + 1) + 1) & ~(size_t)1);
+  return words * 4 + (size_t)(kWCap + 2) * 8;
+}
+
+int particle_grid(const Params& P, int ctas_per_sm) {
+  const int want = sm_count() * ctas_per_sm;
+  return P.max_tiles < want ? (P.max_tiles > 0 ? P.max_tiles : 1) : want;
+}
+
+cudaError_t configure_kernels(int ns) {
+  const int bytes = (int)pass_b_smem_bytes(ns);
+  cudaError_t e = cudaFuncSetAttribute(k_pass_b<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_pass_b<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int variant, cudaStream_t s) {
+  const int ga = particle_grid(P, 4), gb = particle_grid(P, 2);
+  const size_t smem_b = pass_b_smem_bytes(P.ns);
+  if (variant == 2) {
+    k_pass_a<2><<<ga, kThreads, 0, s>>>(P, cur);
+    k_mid<<<1, kMidThreads, 0, s>>>(P);
+    k_pass_b<2><<<gb, kThreads, smem_b, s>>>(P, cur, nxt);
+  } else {
+    k_pass_a<1><<<ga, kThreads, 0, s>>>(P, cur);
+    k_mid<<<1, kMidThreads, 0, s>>>(P);
+    k_pass_b<1><<<gb, kThreads, smem_b, s>>>(P, cur, nxt);
+  }
+  k_field<<<1, kFieldThreads, 0, s>>>(P, 1);
+  return 4;
+}
+
+// load / restart: counts -> cell_start, deposit, field (no push).  cur must be sorted by cell.
+__global__ void __launch_bounds__(kThreads) k_count_cells(const __grid_constant__ Params P, Particles cur) {
+  const unsigned n = P.st->n;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    atomicAdd(&P.cell_count[cur.cell[i]], 1);
+}
+__global__ void k_clear_grids(const __grid_constant__ Params P) {
+  const size_t tot = (size_t)P.ns * (size_t)P.ng;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < tot; i += (size_t)gridDim.x * blockDim.x)
+    P.dens[i] = 0;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < (size_t)P.nc; i += (size_t)gridDim.x * blockDim.x) {
+    P.cell_count[i] = 0;
+    P.ovf_before[i] = 0;
+  }
+}
+
+int launch_rebuild(const Params& P, const Particles& cur, cudaStream_t s) {
+  const int g = sm_count() * 4;
+  k_clear_grids<<<g, 256, 0, s>>>(P);
+  k_count_cells<<<g, kThreads, 0, s>>>(P, cur);
+  k_mid<<<1, kMidThreads, 0, s>>>(P);   // ovf_count == 0: plain scan; n_next = n
+  k_deposit<<<g, kThreads, 0, s>>>(P, cur);
+  k_field<<<1, kFieldThreads, 0, s>>>(P, 0);  // commits n = n_next, leaves the step counter alone
+  return 5;
+}
+
+}  // namespace bit1

@@ -1,0 +1,12 @@
+// Host-callable launchers of the step kernels (defined in step_kernels.cu).
+#pragma once
+#include "common.cuh"
+
+namespace bit1 {
+cudaError_t configure_kernels(int ns);
+// one timestep on stream s; returns the number of kernels launched
+int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int variant, cudaStream_t s);
+// counts per cell -> cell_start, deposit, field solve for particles already sorted in cur
+int launch_rebuild(const Params& P, const Particles& cur, cudaStream_t s);
+size_t pass_b_smem_bytes(int ns);
+}  // namespace bit1
