@@ -175,6 +175,13 @@ bit1_status bit1_restart(bit1_ctx *ctx, const void *blob_host, size_t bytes);
 
 void bit1_destroy(bit1_ctx *ctx);
 const char *bit1_error_string(bit1_status s);
+/* Per-kernel device timing for the roofline report.  While enabled, bit1_step
+ * records CUDA events on the compute stream around each of its four kernels (first 4096 steps kept).
+ * bit1_get_profile waits for the stream and returns the summed milliseconds of
+ * [mover pass A, side-list + cell scan, arranger pass B, field solve] and the number of steps they
+ * cover, then clears the record. */
+bit1_status bit1_profile(bit1_ctx *ctx, int enable);
+bit1_status bit1_get_profile(bit1_ctx *ctx, double ms[4], uint64_t *steps);
 /* Kernels launched by this context since create (bench.py's gpu_launches). */
 uint64_t bit1_launch_count(bit1_ctx *ctx);
 

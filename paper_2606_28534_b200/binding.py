@@ -105,6 +105,10 @@ def load_library(path: Optional[str] = None):
     L.bit1_destroy.argtypes = [vp]
     L.bit1_error_string.restype = C.c_char_p
     L.bit1_error_string.argtypes = [C.c_int]
+    L.bit1_profile.restype = C.c_int
+    L.bit1_profile.argtypes = [vp, C.c_int]
+    L.bit1_get_profile.restype = C.c_int
+    L.bit1_get_profile.argtypes = [vp, C.POINTER(C.c_double * 4), C.POINTER(C.c_uint64)]
     L.bit1_launch_count.restype = C.c_uint64
     L.bit1_launch_count.argtypes = [vp]
     if path is None:
@@ -321,6 +325,15 @@ class Bit1:
 
     def restart(self, blob):
         _check(self.lib.bit1_restart(self.h, blob.data_ptr(), blob.numel()), "bit1_restart")
+
+    def profile(self, enable: bool = True):
+        _check(self.lib.bit1_profile(self.h, int(enable)), "bit1_profile")
+
+    def get_profile(self):
+        ms = (C.c_double * 4)()
+        steps = C.c_uint64()
+        _check(self.lib.bit1_get_profile(self.h, C.byref(ms), C.byref(steps)), "bit1_get_profile")
+        return dict(zip(("pass_a", "mid", "pass_b", "field"), [float(v) for v in ms])), int(steps.value)
 
     def launch_count(self) -> int:
         return int(self.lib.bit1_launch_count(self.h))

@@ -7,6 +7,7 @@
 #include <string.h>
 
 #include <new>
+#include <vector>
 
 #include "../../include/bit1.h"
 #include "aux_kernels.h"
@@ -148,7 +149,11 @@ struct bit1_ctx {
   uint64_t launches, cfg_hash;
   double m[BIT1_MAX_SPECIES], weight[BIT1_MAX_SPECIES];
   double dt;
+  bool profiling;
+  std::vector<cudaEvent_t> prof_ev;  // 5 per timed step
+  size_t prof_steps;
 };
+constexpr size_t kMaxProfSteps = 4096;
 
 #define CUDA_OK(call)                              \
   do {                                             \
@@ -221,6 +226,7 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   c->variant = o->variant == 1 ? 1 : 2;
   if (const char* ev = getenv("BIT1_VARIANT")) { if (atoi(ev) == 1) c->variant = 1; else if (atoi(ev) == 2) c->variant = 2; }
   c->cur = 0; c->loaded = false; c->ckpt_pending = false; c->launches = 0; c->dt = dt;
+  c->profiling = false; c->prof_steps = 0;
 
   Params& P = c->P;
   P.nc = g->nc; P.bc = g->bc; P.ng = lay.ng; P.ns = ns;
@@ -329,10 +335,34 @@ void bit1_destroy(bit1_ctx* c) {
   if (c->ss != c->cs) cudaStreamSynchronize(c->ss);
   cudaEventDestroy(c->ev_snap);
   cudaEventDestroy(c->ev_done);
+  for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
   delete c;
 }
 
 uint64_t bit1_launch_count(bit1_ctx* c) { return c ? c->launches : 0; }
+
+bit1_status bit1_profile(bit1_ctx* c, int enable) {
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  c->profiling = enable != 0;
+  c->prof_steps = 0;
+  return BIT1_OK;
+}
+
+bit1_status bit1_get_profile(bit1_ctx* c, double ms[4], uint64_t* steps) {
+  if (!c || !ms) return BIT1_ERR_INVALID_ARG;
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  double acc[4] = {0, 0, 0, 0};
+  for (size_t k = 0; k < c->prof_steps; ++k)
+    for (int j = 0; j < 4; ++j) {
+      float t = 0.f;
+      CUDA_OK(cudaEventElapsedTime(&t, c->prof_ev[k * 5 + j], c->prof_ev[k * 5 + j + 1]));
+      acc[j] += (double)t;
+    }
+  for (int j = 0; j < 4; ++j) ms[j] = acc[j];
+  if (steps) *steps = c->prof_steps;
+  c->prof_steps = 0;
+  return BIT1_OK;
+}
 
 static bit1_status read_state(bit1_ctx* c, DevState* h) {
   CUDA_OK(cudaMemcpyAsync(h, c->P.st, sizeof(DevState), cudaMemcpyDeviceToHost, c->cs));
@@ -374,7 +404,17 @@ bit1_status bit1_step(bit1_ctx* c, uint64_t nsteps) {
   if (!c) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
   for (uint64_t k = 0; k < nsteps; ++k) {
-    c->launches += launch_step(c->P, c->buf[c->cur], c->buf[c->cur ^ 1], c->variant, c->cs);
+    cudaEvent_t* ev = nullptr;
+    if (c->profiling && c->prof_steps < kMaxProfSteps) {
+      while (c->prof_ev.size() < (c->prof_steps + 1) * 5) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) return BIT1_ERR_CUDA;
+        c->prof_ev.push_back(e);
+      }
+      ev = &c->prof_ev[c->prof_steps * 5];
+      c->prof_steps++;
+    }
+    c->launches += launch_step(c->P, c->buf[c->cur], c->buf[c->cur ^ 1], c->variant, c->cs, ev);
     c->cur ^= 1;
   }
   CUDA_OK(cudaGetLastError());

@@ -676,19 +676,21 @@ cudaError_t configure_kernels(int ns) {
   return cudaFuncSetAttribute(k_pass_b<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
 }
 
-int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int variant, cudaStream_t s) {
+int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int variant, cudaStream_t s,
+                cudaEvent_t* ev) {
   const int ga = particle_grid(P, 4), gb = particle_grid(P, 2);
   const size_t smem_b = pass_b_smem_bytes(P.ns);
-  if (variant == 2) {
-    k_pass_a<2><<<ga, kThreads, 0, s>>>(P, cur);
-    k_mid<<<1, kMidThreads, 0, s>>>(P);
-    k_pass_b<2><<<gb, kThreads, smem_b, s>>>(P, cur, nxt);
-  } else {
-    k_pass_a<1><<<ga, kThreads, 0, s>>>(P, cur);
-    k_mid<<<1, kMidThreads, 0, s>>>(P);
-    k_pass_b<1><<<gb, kThreads, smem_b, s>>>(P, cur, nxt);
-  }
+  if (ev) cudaEventRecord(ev[0], s);
+  if (variant == 2) k_pass_a<2><<<ga, kThreads, 0, s>>>(P, cur);
+  else k_pass_a<1><<<ga, kThreads, 0, s>>>(P, cur);
+  if (ev) cudaEventRecord(ev[1], s);
+  k_mid<<<1, kMidThreads, 0, s>>>(P);
+  if (ev) cudaEventRecord(ev[2], s);
+  if (variant == 2) k_pass_b<2><<<gb, kThreads, smem_b, s>>>(P, cur, nxt);
+  else k_pass_b<1><<<gb, kThreads, smem_b, s>>>(P, cur, nxt);
+  if (ev) cudaEventRecord(ev[3], s);
   k_field<<<1, kFieldThreads, 0, s>>>(P, 1);
+  if (ev) cudaEventRecord(ev[4], s);
   return 4;
 }
 

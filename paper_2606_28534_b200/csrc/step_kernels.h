@@ -5,7 +5,9 @@
 namespace bit1 {
 cudaError_t configure_kernels(int ns);
 // one timestep on stream s; returns the number of kernels launched
-int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int variant, cudaStream_t s);
+// ev: NULL, or 5 events recorded before/between/after the four kernels (per-kernel timing)
+int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int variant, cudaStream_t s,
+                cudaEvent_t* ev);
 // counts per cell -> cell_start, deposit, field solve for particles already sorted in cur
 int launch_rebuild(const Params& P, const Particles& cur, cudaStream_t s);
 size_t pass_b_smem_bytes(int ns);

@@ -242,22 +242,17 @@ def make_config(cfg: int, scale: float = 1.0, *, n0_scale: float = 1.0, pair_sou
     )
     if not particles:
         return w
-    rng = np.random.Generator(np.random.Philox(gen_seed if gen_seed is not None else 2606285340 + cfg))
+    gseed = gen_seed if gen_seed is not None else 2606285340 + cfg
     xs, vxs, vys, vzs, tags = [], [], [], [], []
     x_e = None
     for k, s in enumerate(sp):
+        Tk = T0 if s.name == "D" else T
+        x, vx, vy, vz = _species_arrays(gseed, k, n_per, L, c["profile"], _vth(Tk, s.m))
         if cfg == 1 and k == 1:
             x = x_e.copy()  # ions on top of electrons: rho == 0 at step 0
-        else:
-            x = _positions(rng, n_per, L, c["profile"])
         if k == 0:
             x_e = x
-        Tk = T0 if s.name == "D" else T
-        vth = _vth(Tk, s.m)
-        xs.append(x)
-        vxs.append(vth * rng.standard_normal(n_per))
-        vys.append(vth * rng.standard_normal(n_per))
-        vzs.append(vth * rng.standard_normal(n_per))
+        xs.append(x); vxs.append(vx); vys.append(vy); vzs.append(vz)
         tags.append(np.full(n_per, k, dtype=np.uint8))
     w.x = np.ascontiguousarray(np.concatenate(xs))
     w.vx = np.ascontiguousarray(np.concatenate(vxs))
@@ -265,6 +260,34 @@ def make_config(cfg: int, scale: float = 1.0, *, n0_scale: float = 1.0, pair_sou
     w.vz = np.ascontiguousarray(np.concatenate(vzs))
     w.sp = np.ascontiguousarray(np.concatenate(tags))
     return w
+
+
+_CHUNK = 1 << 21
+
+
+def _species_arrays(gseed: int, k: int, n: int, L: float, profile: str, vth: float):
+    """Positions and velocities of one species, generated in fixed chunks of 2^21 particles, each chunk from
+    its own Philox key (gseed, species, chunk) -- the arrays do not depend on how many threads fill them."""
+    from concurrent.futures import ThreadPoolExecutor
+    import os
+
+    x = np.empty(n); vx = np.empty(n); vy = np.empty(n); vz = np.empty(n)
+
+    def fill(j):
+        lo, hi = j * _CHUNK, min(n, (j + 1) * _CHUNK)
+        rng = np.random.Generator(np.random.Philox(key=[gseed, (k << 32) | j]))
+        x[lo:hi] = _positions(rng, hi - lo, L, profile)
+        vx[lo:hi] = vth * rng.standard_normal(hi - lo)
+        vy[lo:hi] = vth * rng.standard_normal(hi - lo)
+        vz[lo:hi] = vth * rng.standard_normal(hi - lo)
+
+    nchunks = (n + _CHUNK - 1) // _CHUNK
+    if nchunks <= 1:
+        fill(0)
+    else:
+        with ThreadPoolExecutor(max_workers=min(32, os.cpu_count() or 1)) as ex:
+            list(ex.map(fill, range(nchunks)))
+    return x, vx, vy, vz
 
 
 def make_custom(nc: int, dx: float, bc: int, dt: float, species: List[Species], *, B=(0.0, 0.0, 0.0),
