@@ -6,6 +6,7 @@
 // EMIT = false : the recompute pass of variant V2 -- same arithmetic, no side effects.
 #pragma once
 #include "device_math.cuh"
+#include "pipeline.cuh"
 
 namespace bit1 {
 
@@ -194,6 +195,40 @@ __device__ __forceinline__ void advance(const Params& P, const SpeciesP* S, unsi
     emit_record(P, make_key(cn, 2u, (unsigned long long)gidx * 4ull), x, pb.vx, pb.vy, pb.vz, 0u,
                 s.src_partner);
   c = cn;
+}
+
+// G, B, M only: the part of the step that every particle takes.  Same expressions, same order as advance().
+// Returns true when the moved particle is inside [0, L) -- no wall hit, no periodic wrap.
+__device__ __forceinline__ bool push_fast(const Params& P, const SpeciesP& s, const double* Eptr, int c, double& x,
+                                          double& vx, double& vy, double& vz) {
+  const double f = x * P.inv_dx - (double)c;
+  const double e0 = Eptr[c], e1 = Eptr[c + 1];
+  const double Ex = e0 + f * (e1 - e0);
+  const double a = s.h * Ex;
+  const double ux = vx + a, uy = vy, uz = vz;
+  const double px = ux + (uy * s.tz - uz * s.ty);
+  const double py = uy + (uz * s.tx - ux * s.tz);
+  const double pz = uz + (ux * s.ty - uy * s.tx);
+  const double wx = ux + (py * s.sz - pz * s.sy);
+  const double wy = uy + (pz * s.sx - px * s.sz);
+  const double wz = uz + (px * s.sy - py * s.sx);
+  vx = wx + a; vy = wy; vz = wz;
+  x = x + vx * P.dt;
+  return x >= 0.0 && x < P.L;
+}
+
+// The rare path (wall hit, periodic wrap, null-collision candidate): redo the whole step of particle `off` of
+// the staged tile from its stored state, write the new state back into the stage and return the new cell
+// (-1: dead).  Taking the state from shared memory keeps every by-reference argument of the rare code out of
+// the callers' registers and stack.
+template <bool EMIT>
+static __device__ __noinline__ int slow_advance(const Params& P, const SpeciesP* S, unsigned long long step,
+                                                const double* Eptr, Stage* st, int off, unsigned gidx) {
+  double x = st->x[off], vx = st->vx[off], vy = st->vy[off], vz = st->vz[off];
+  int c = st->cell[off];
+  advance<EMIT>(P, S, step, Eptr, (int)st->sp[off], st->pid[off], gidx, x, vx, vy, vz, c);
+  st->x[off] = x; st->vx[off] = vx; st->vy[off] = vy; st->vz[off] = vz;
+  return c;
 }
 
 }  // namespace bit1

@@ -29,10 +29,13 @@ constexpr uint32_t kCkptVersion = 1;
 inline size_t align_up(size_t v) { return (v + kAlign - 1) & ~(kAlign - 1); }
 
 struct PartLayout {
-  size_t x, vx, vy, vz, cell, pid, sp, bytes;
+  size_t x, vx, vy, vz, cell, pid, sp, desc, bytes;
 };
-PartLayout part_layout(size_t cap) {
+// every array holds a whole number of tiles: the bulk-async loads always fetch whole tiles
+PartLayout part_layout(size_t cap_in) {
   PartLayout l;
+  const size_t tiles = (cap_in + kTile - 1) / kTile;
+  const size_t cap = tiles * kTile;
   size_t o = 0;
   l.x = o; o += align_up(cap * 8);
   l.vx = o; o += align_up(cap * 8);
@@ -41,6 +44,7 @@ PartLayout part_layout(size_t cap) {
   l.cell = o; o += align_up(cap * 4);
   l.pid = o; o += align_up(cap * 4);
   l.sp = o; o += align_up(cap);
+  l.desc = o; o += align_up((tiles + 1) * 8);
   l.bytes = o;
   return l;
 }
@@ -54,6 +58,7 @@ Particles part_at(void* base, const PartLayout& l) {
   p.cell = reinterpret_cast<int*>(b + l.cell);
   p.pid = reinterpret_cast<unsigned*>(b + l.pid);
   p.sp = reinterpret_cast<unsigned char*>(b + l.sp);
+  p.desc = reinterpret_cast<int2*>(b + l.desc);
   return p;
 }
 
@@ -71,7 +76,7 @@ CkptLayout ckpt_layout(int nc, size_t cap) {
 }
 
 struct Layout {
-  size_t st, tables, dens, rho, phi, E, cell_count, cell_start, cell_base, ovf_before, tile_desc, tile_hist,
+  size_t st, tables, dens, rho, phi, E, cell_count, cell_start, cell_base, ovf_before, tile_hist, tile_base, evt,
       ovf_key, ovf_idx, ovf_dst, tmp_key, tmp_idx, ovf_rec, part[2], scratch, mom, total;
   unsigned ovf_cap, ovf_pow2;
   int max_tiles, ng;
@@ -94,13 +99,14 @@ Layout make_layout(int nc, int bc, int ns, size_t cap, int staging) {
   l.dens = take((size_t)ns * l.ng * 8);
   l.rho = take((size_t)l.ng * 8);
   l.phi = take((size_t)(nc + 1) * 8);
-  l.E = take((size_t)(nc + 1) * 8);
+  l.E = take((size_t)(nc + 4) * 8);  // the E window of a tile is copied in 16-byte units
   l.cell_count = take((size_t)nc * 4);
   l.cell_start = take((size_t)(nc + 1) * 4);
   l.cell_base = take((size_t)nc * 4);
   l.ovf_before = take((size_t)nc * 4);
-  l.tile_desc = take((size_t)(l.max_tiles + 1) * 8);
   l.tile_hist = take(((size_t)nc + (size_t)(l.max_tiles + 1) * (2 * kMaxR + 1) + kWCap) * 4);
+  l.tile_base = take(((size_t)nc + (size_t)(l.max_tiles + 1) * (2 * kMaxR + 1) + kWCap) * 4);
+  l.evt = take((size_t)(l.max_tiles + 1) * (kTile / 8));
   l.ovf_key = take((size_t)p2 * 8);
   l.tmp_key = take((size_t)p2 * 8);
   l.ovf_idx = take((size_t)p2 * 4);
@@ -145,7 +151,7 @@ struct bit1_ctx {
   cudaStream_t cs, ss;
   cudaEvent_t ev_snap, ev_done;
   bool ckpt_pending, staging, loaded;
-  int variant;
+  int variant, threads;
   uint64_t launches, cfg_hash;
   double m[BIT1_MAX_SPECIES], weight[BIT1_MAX_SPECIES];
   double dt;
@@ -225,6 +231,8 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   c->staging = staging != 0;
   c->variant = o->variant == 1 ? 1 : 2;
   if (const char* ev = getenv("BIT1_VARIANT")) { if (atoi(ev) == 1) c->variant = 1; else if (atoi(ev) == 2) c->variant = 2; }
+  c->threads = 512;
+  if (const char* ev = getenv("BIT1_THREADS")) { if (atoi(ev) == 1024) c->threads = 1024; }
   c->cur = 0; c->loaded = false; c->ckpt_pending = false; c->launches = 0; c->dt = dt;
   c->profiling = false; c->prof_steps = 0;
 
@@ -265,7 +273,7 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
     q.sign = sp[s].q > 0.0 ? 1 : (sp[s].q < 0.0 ? -1 : 0);
     q.flags = sp[s].flags; q.src_mode = sp[s].src_mode; q.src_partner = sp[s].src_partner;
     if (q.Q < 1 || q.Q >= (1ll << 31)) { delete c; return BIT1_ERR_RANGE; }
-    if ((unsigned long long)q.Q * (unsigned long long)kTile >= (1ull << 32)) P.dep_u32 = 0;
+    if ((unsigned long long)q.Q * (unsigned long long)kTile >= (1ull << 32)) P.dep_u32 = 0;  // => Q < 2^21
     c->m[s] = sp[s].m; c->weight[s] = sp[s].weight;
   }
   char* ws = c->ws;
@@ -280,7 +288,8 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   P.cell_start = reinterpret_cast<int*>(ws + lay.cell_start);
   P.cell_base = reinterpret_cast<int*>(ws + lay.cell_base);
   P.ovf_before = reinterpret_cast<int*>(ws + lay.ovf_before);
-  P.tile_desc = reinterpret_cast<int2*>(ws + lay.tile_desc);
+  P.tile_base = reinterpret_cast<int*>(ws + lay.tile_base);
+  P.evt = reinterpret_cast<unsigned*>(ws + lay.evt);
   P.tile_hist = reinterpret_cast<unsigned*>(ws + lay.tile_hist);
   P.ovf_key = reinterpret_cast<unsigned long long*>(ws + lay.ovf_key);
   P.tmp_key = reinterpret_cast<unsigned long long*>(ws + lay.tmp_key);
@@ -321,7 +330,7 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   }
   ok = ok && cudaMemcpyAsync((void*)P.inv_norm, o->inv_norm, (size_t)(o->n_norm + 1) * 8, cudaMemcpyHostToDevice, c->cs) == cudaSuccess;
   ok = ok && cudaStreamSynchronize(c->cs) == cudaSuccess;
-  ok = ok && configure_kernels(ns) == cudaSuccess;
+  ok = ok && configure_kernels() == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&c->ev_snap, cudaEventDisableTiming) == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&c->ev_done, cudaEventDisableTiming) == cudaSuccess;
   if (!ok) { delete c; return BIT1_ERR_CUDA; }
@@ -414,7 +423,7 @@ bit1_status bit1_step(bit1_ctx* c, uint64_t nsteps) {
       ev = &c->prof_ev[c->prof_steps * 5];
       c->prof_steps++;
     }
-    c->launches += launch_step(c->P, c->buf[c->cur], c->buf[c->cur ^ 1], c->variant, c->cs, ev);
+    c->launches += launch_step(c->P, c->buf[c->cur], c->buf[c->cur ^ 1], c->variant, c->threads, c->cs, ev);
     c->cur ^= 1;
   }
   CUDA_OK(cudaGetLastError());

@@ -6,12 +6,8 @@
 namespace bit1 {
 
 constexpr int kMaxSpecies = 8;
-constexpr int kThreads = 256;             // threads per CTA of the particle kernels
-constexpr int kItems = 8;                 // particles per thread per tile
-constexpr int kTile = kThreads * kItems;  // 2048 particles per tile
-constexpr int kWarps = kThreads / 32;
-constexpr int kWarpSpan = 32 * kItems;    // contiguous particles handled by one warp
-constexpr int kWCap = 512;                // max cells in a tile's window (smem histogram bins)
+constexpr int kTile = 2048;               // particles per tile (one TMA stage)
+constexpr int kWCap = 256;                // max cells in a tile's window (smem histogram bins)
 
 // overflow ("far mover" / birth) key: cell(28) | cls(2) | ord(34)
 constexpr int kOrdBits = 34;
@@ -24,9 +20,9 @@ constexpr unsigned kElastic = 1u, kIonise = 2u, kCx = 4u, kIonProduct = 8u, kEle
                    kTargetMaxwellian = 32u;
 constexpr int kSrcNone = 0, kSrcSelf = 1, kSrcPair = 2;
 
-struct SpeciesP {
-  double h, tx, ty, tz, sx, sy, sz;
-  double src_vth, pnull, numax, kin_eV, two_e_over_m, el_loss;
+struct __align__(16) SpeciesP {
+  double h, tx, ty, tz, sx, sy, sz, pnull;   // the per-particle fast path reads these eight (four 128-bit loads)
+  double src_vth, numax, kin_eV, two_e_over_m, el_loss;
   long long Q;
   int sign;
   unsigned flags;
@@ -39,6 +35,7 @@ struct Particles {
   int *cell;
   unsigned *pid;
   unsigned char *sp;
+  int2 *desc;  // per tile of this buffer: (cell of its first particle, cell of its last particle)
 };
 
 struct OvfRec {  // one far mover or birth, full state (48 B)
@@ -92,8 +89,9 @@ struct Params {
   int *cell_base;   // nc: cell_start + far movers placed before the windowed particles
   int *ovf_before;  // nc
   // tiles
-  int2 *tile_desc;      // (clo, chi) of each tile at step start
   unsigned *tile_hist;  // banded histogram rows, row t at clo_t + t*(2R+1)
+  int *tile_base;       // same layout: destination of the tile's first particle of each window cell
+  unsigned *evt;        // one bit per particle slot: pass B must take the slow path (wall hit / MC candidate)
   // overflow list
   unsigned long long *ovf_key;  // ovf_pow2 (unsorted, then sorted in place)
   unsigned *ovf_idx;            // ovf_pow2: record index of sorted position

@@ -1,10 +1,13 @@
-// The four kernels of one timestep:
-//   k_pass_a  mover: advance every particle, banded per-tile histogram of new cells, side list of far
-//             movers and births                                   (PAPER.md:111 move0/moveb)
-//   k_mid     order the side list, counts -> cell_start           (row a4, scan part)
-//   k_pass_b  arranger: stable ranks inside the tile, scatter to the sorted position with the charge
-//             deposition fused                                    (rows a4-a5; PAPER.md:111 arrj/narrj)
-//   k_field   exact integer-scan Poisson solve -> phi, E          (row a6; PAPER.md:33 step (iii))
+// The kernels of one timestep:
+//   k_pass_a   mover: advance every particle, banded per-tile histogram of new cells, event bits, side list of
+//              far movers and births                               (PAPER.md:111 move0/moveb)
+//   k_mid      order the side list, counts -> cell_start           (row a4, scan part)
+//   k_colscan  banded column scan: destination base of every (tile, window cell)
+//   k_pass_b   arranger: stable ranks inside the tile, scatter to the sorted position with the charge
+//              deposition fused                                    (rows a4-a5; PAPER.md:111 arrj/narrj)
+//   k_field    exact integer-scan Poisson solve -> phi, E          (row a6; PAPER.md:33 step (iii))
+// Both particle passes are persistent (one CTA per SM) and read their tiles through the two-stage bulk-async
+// pipeline of pipeline.cuh.
 #include "advance.cuh"
 #include "step_kernels.h"
 
@@ -30,71 +33,128 @@ __device__ __forceinline__ void load_species(const Params& P, SpeciesP* s_sp) {
   for (int i = threadIdx.x; i < words; i += blockDim.x) dst[i] = src[i];
 }
 
+constexpr int kAuxThreads = 256;
+constexpr unsigned kCollMask = kElastic | kIonise | kCx;
+
+// dynamic shared memory of both passes: [2 x Stage][pass-specific arrays][species][2 barriers]
+template <int THREADS>
+struct PassSmem {
+  static constexpr int kWarps = THREADS / 32;
+  static constexpr size_t stages = 2 * sizeof(Stage);
+  static constexpr size_t a_hist = stages;                                  // unsigned[kWCap]
+  static constexpr size_t a_sp = a_hist + kWCap * 4;                        // SpeciesP[kMaxSpecies]
+  static constexpr size_t a_bar = a_sp + kMaxSpecies * sizeof(SpeciesP);    // 2 x u64
+  static constexpr size_t a_total = a_bar + 16;
+  static constexpr size_t b_wcnt = stages;                                  // unsigned[kWCap][kWarps]
+  static constexpr size_t b_dens = b_wcnt + (size_t)kWCap * kWarps * 4;     // unsigned[kWCap + 1][kMaxSpecies]
+  static constexpr size_t b_sp = b_dens + (size_t)(kWCap + 1) * kMaxSpecies * 4 + 32;
+  static constexpr size_t b_bar = (b_sp + kMaxSpecies * sizeof(SpeciesP) + 15) & ~(size_t)15;
+  static constexpr size_t b_total = b_bar + 16;
+};
+
 // ---------------------------------------------------------------------------------------------
-// Pass A.  VARIANT 1 writes the advanced state back in place; VARIANT 2 writes nothing per particle.
-template <int VARIANT>
-__global__ void __launch_bounds__(kThreads) k_pass_a(const __grid_constant__ Params P, Particles cur) {
-  __shared__ SpeciesP s_sp[kMaxSpecies];
-  __shared__ unsigned s_hist[kWCap];
-  __shared__ double s_E[kWCap + 2];
-  load_species(P, s_sp);
+// Pass A.  VARIANT 1 writes the advanced state back in place; VARIANT 2 writes one event bit per particle.
+template <int VARIANT, int THREADS>
+__global__ void __launch_bounds__(THREADS, 1) k_pass_a(const __grid_constant__ Params P, Particles cur) {
+  constexpr int kItems = kTile / THREADS, kWarpSpan = 32 * kItems;
+  typedef PassSmem<THREADS> SM;
+  extern __shared__ __align__(128) unsigned char smem[];
+  Stage* stg = reinterpret_cast<Stage*>(smem);
+  unsigned* s_hist = reinterpret_cast<unsigned*>(smem + SM::a_hist);
+  SpeciesP* s_sp = reinterpret_cast<SpeciesP*>(smem + SM::a_sp);
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem + SM::a_bar);
+
   const unsigned n = P.st->n;
   const unsigned long long step = P.st->step;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int ntiles = (int)((n + kTile - 1) / kTile);
+  const int G = gridDim.x;
 
+  if (threadIdx.x == 0) {
+    mbar_init(&bar[0], 1);
+    mbar_init(&bar[1], 1);
+    mbar_fence_init();
+    fence_proxy_async();
+    for (int k = 0; k < 2; ++k) {
+      const int t = blockIdx.x + k * G;
+      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, cur.desc[t], false, true);
+    }
+  }
+  load_species(P, s_sp);
+  for (int k = threadIdx.x; k < kWCap; k += THREADS) s_hist[k] = 0;
   // the deposition of this step accumulates into dens: clear it here (nobody reads it during pass A)
   {
     const size_t tot = (size_t)P.ns * (size_t)P.ng;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < tot; i += (size_t)gridDim.x * blockDim.x)
-      P.dens[i] = 0;
+    for (size_t i = (size_t)blockIdx.x * THREADS + threadIdx.x; i < tot; i += (size_t)G * THREADS) P.dens[i] = 0;
   }
-  const int ntiles = (int)((n + kTile - 1) / kTile);
-  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+  __syncthreads();
+
+  int it = 0;
+  for (int tile = blockIdx.x; tile < ntiles; tile += G, ++it) {
+    Stage* S = &stg[it & 1];
     const unsigned base = (unsigned)tile * kTile;
     const unsigned cnt = min((unsigned)kTile, n - base);
-    const int clo = cur.cell[base], chi = cur.cell[base + cnt - 1];
-    const TileWin tw = make_window(clo, chi, P.R);
-    for (int k = threadIdx.x; k < tw.W; k += kThreads) s_hist[k] = 0;
-    const int ecount = chi - clo + 2;
-    const bool e_staged = ecount <= kWCap + 2;
-    if (e_staged)
-      for (int k = threadIdx.x; k < ecount; k += kThreads) s_E[k] = P.E[clo + k];
-    const double* Eptr = e_staged ? (s_E - clo) : P.E;
-    __syncthreads();
+    // descriptor of the tile after next (its load is issued at the end of this iteration)
+    int2 dn = make_int2(0, 0);
+    const int tnext = tile + 2 * G;
+    if (threadIdx.x == 0 && tnext < ntiles) dn = cur.desc[tnext];
+    mbar_wait(&bar[it & 1], (unsigned)(it >> 1) & 1u);
 
-#pragma unroll 2
+    const int clo = S->cell[0], chi = S->cell[cnt - 1];
+    const TileWin tw = make_window(clo, chi, P.R);
+    int e0, ne;
+    const double* Eptr = e_window(clo, chi, e0, ne) ? (S->E - e0) : P.E;
+
+#pragma unroll
     for (int r = 0; r < kItems; ++r) {
-      const unsigned off = (unsigned)(warp * kWarpSpan + r * 32 + lane);
-      const bool have = off < cnt;
+      const int off = warp * kWarpSpan + r * 32 + lane;
+      const bool have = (unsigned)off < cnt;
       unsigned key = 0x80000000u | (unsigned)lane;  // unique: matches nobody
+      bool evt = false;
       if (have) {
-        const unsigned i = base + off;
-        double x = cur.x[i], vx = cur.vx[i], vy = cur.vy[i], vz = cur.vz[i];
-        int c = cur.cell[i];
-        const int sp = cur.sp[i];
-        const unsigned pid = cur.pid[i];
-        advance<true>(P, s_sp, step, Eptr, sp, pid, i, x, vx, vy, vz, c);
+        const unsigned i = base + (unsigned)off;
+        const int sp = S->sp[off];
+        const SpeciesP& s = s_sp[sp];
+        int c = S->cell[off];
+        double x = S->x[off], vx = S->vx[off], vy = S->vy[off], vz = S->vz[off];
+        evt = !push_fast(P, s, Eptr, c, x, vx, vy, vz);
+        if (!evt && (s.flags & kCollMask)) {
+          const uint4 w = draw(P, S->pid[off], step, 0u);  // slot C0
+          evt = u52(w.x, w.y) < s.pnull;
+        }
+        if (evt) {
+          c = slow_advance<true>(P, s_sp, step, Eptr, S, off, i);
+          x = S->x[off]; vx = S->vx[off]; vy = S->vy[off]; vz = S->vz[off];
+        } else {
+          c = cell_of(P, x);
+        }
         if (VARIANT == 1) {
           cur.x[i] = x; cur.vx[i] = vx; cur.vy[i] = vy; cur.vz[i] = vz; cur.cell[i] = c;
         }
         if (c >= 0) {
           const int k = c - tw.wlo;
           if (k >= 0 && k < tw.W) key = (unsigned)k;
-          else emit_record(P, make_key(c, c < tw.wlo ? 1u : 0u, (unsigned long long)i), x, vx, vy, vz, pid, sp);
+          else emit_record(P, make_key(c, c < tw.wlo ? 1u : 0u, (unsigned long long)i), x, vx, vy, vz, S->pid[off], sp);
         }
+      }
+      if (VARIANT == 2) {
+        const unsigned eb = __ballot_sync(0xffffffffu, evt);
+        if (lane == 0) P.evt[(base >> 5) + (unsigned)(warp * kItems + r)] = eb;
       }
       const unsigned m = __match_any_sync(0xffffffffu, key);
       if (!(key & 0x80000000u) && lane == __ffs(m) - 1) atomicAdd(&s_hist[key], (unsigned)__popc(m));
     }
+    fence_proxy_async();
     __syncthreads();
     unsigned* row = P.tile_hist + tile_row_offset(clo, tile, P.R);
-    for (int k = threadIdx.x; k < tw.W; k += kThreads) {
+    for (int k = threadIdx.x; k < tw.W; k += THREADS) {
       const unsigned h = s_hist[k];
+      s_hist[k] = 0;
       row[k] = h;
       const int c = tw.wlo + k;
       if (h && c >= 0 && c < P.nc) atomicAdd(&P.cell_count[c], (int)h);
     }
-    if (threadIdx.x == 0) P.tile_desc[tile] = make_int2(clo, chi);
+    if (threadIdx.x == 0 && tnext < ntiles) issue_tile(P, cur, S, &bar[it & 1], tnext, dn, false, true);
     __syncthreads();
   }
 }
@@ -302,65 +362,120 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
 }
 
 // ---------------------------------------------------------------------------------------------
-// Pass B.  Dynamic shared memory: s_wcnt[kWCap][kWarps], s_base[kWCap], s_dens[kWCap+1][ns], s_E.
-template <int VARIANT>
-__global__ void __launch_bounds__(kThreads, 2)
-k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  __shared__ SpeciesP s_sp[kMaxSpecies];
-  unsigned* s_wcnt = reinterpret_cast<unsigned*>(smem_raw);          // [kWCap][kWarps]
-  int* s_base = reinterpret_cast<int*>(s_wcnt + kWarps * kWCap);     // [kWCap]
-  unsigned* s_dens = reinterpret_cast<unsigned*>(s_base + kWCap);    // [kWCap + 1][ns]
-  double* s_E = reinterpret_cast<double*>(s_dens + ((P.ns * (kWCap + 1) + 1) & ~1));  // [kWCap + 2] (V2)
-  load_species(P, s_sp);
+// k_colscan: for every tile t and every cell c of its window, the destination of the first particle that tile t
+// sends to c:  cell_base[c] + sum of tile_hist over the earlier tiles whose window holds c.  Windows' lower and
+// upper ends are monotone in t, so those tiles are the contiguous range just before t.  One warp per tile.
+constexpr int kColThreads = 256;
+
+__global__ void __launch_bounds__(kColThreads) k_colscan(const __grid_constant__ Params P, Particles cur) {
   const unsigned n = P.st->n;
+  const int ntiles = (int)((n + kTile - 1) / kTile);
+  const int lane = threadIdx.x & 31;
+  const int wpb = kColThreads / 32;
+  for (int tile = blockIdx.x * wpb + (threadIdx.x >> 5); tile < ntiles; tile += gridDim.x * wpb) {
+    const int2 d = cur.desc[tile];
+    const TileWin tw = make_window(d.x, d.y, P.R);
+    int* out = P.tile_base + tile_row_offset(d.x, tile, P.R);
+    for (int k = lane; k < tw.W; k += 32) {
+      const int c = tw.wlo + k;
+      int pre = 0;
+      if (c >= 0 && c < P.nc) {
+        pre = P.cell_base[c];
+        for (int t = tile - 1; t >= 0; --t) {
+          const int2 dd = cur.desc[t];
+          const TileWin w2 = make_window(dd.x, dd.y, P.R);
+          if (c >= w2.wlo + w2.W) break;  // c >= w2.wlo always holds (wlo is monotone in t)
+          pre += (int)P.tile_hist[tile_row_offset(dd.x, t, P.R) + (size_t)(c - w2.wlo)];
+        }
+      }
+      out[k] = pre;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Pass B.
+template <int VARIANT, int THREADS>
+__global__ void __launch_bounds__(THREADS, 1)
+k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
+  constexpr int kItems = kTile / THREADS, kWarpSpan = 32 * kItems, kWarps = THREADS / 32;
+  typedef PassSmem<THREADS> SM;
+  extern __shared__ __align__(128) unsigned char smem[];
+  Stage* stg = reinterpret_cast<Stage*>(smem);
+  unsigned* s_wcnt = reinterpret_cast<unsigned*>(smem + SM::b_wcnt);   // [kWCap][kWarps]
+  unsigned* s_dens = reinterpret_cast<unsigned*>(smem + SM::b_dens);   // [kWCap + 1][ns]
+  SpeciesP* s_sp = reinterpret_cast<SpeciesP*>(smem + SM::b_sp);
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem + SM::b_bar);
+
+  const unsigned n = P.st->n, n_next = P.st->n_next;
   const unsigned long long step = P.st->step;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned lt = lanemask_lt();
   const int ntiles = (int)((n + kTile - 1) / kTile);
+  const int G = gridDim.x;
+  const int ns = P.ns;
+
+  if (threadIdx.x == 0) {
+    mbar_init(&bar[0], 1);
+    mbar_init(&bar[1], 1);
+    mbar_fence_init();
+    fence_proxy_async();
+    for (int k = 0; k < 2; ++k) {
+      const int t = blockIdx.x + k * G;
+      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, cur.desc[t], VARIANT == 2, VARIANT == 2);
+    }
+  }
+  load_species(P, s_sp);
+  for (int k = threadIdx.x; k < kWCap * kWarps; k += THREADS) s_wcnt[k] = 0;
+  for (int k = threadIdx.x; k < (kWCap + 1) * kMaxSpecies; k += THREADS) s_dens[k] = 0;
   __syncthreads();
 
-  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+  int it = 0;
+  for (int tile = blockIdx.x; tile < ntiles; tile += G, ++it) {
+    Stage* S = &stg[it & 1];
     const unsigned base = (unsigned)tile * kTile;
     const unsigned cnt = min((unsigned)kTile, n - base);
-    const int2 d = P.tile_desc[tile];
+    const int2 d = cur.desc[tile];
     const TileWin tw = make_window(d.x, d.y, P.R);
-    for (int k = threadIdx.x; k < kWarps * tw.W; k += kThreads) s_wcnt[k] = 0;
-    for (int k = threadIdx.x; k < P.ns * (tw.W + 1); k += kThreads) s_dens[k] = 0;
-    const double* Eptr = P.E;
-    if (VARIANT == 2) {
-      const int ecount = tw.chi - tw.clo + 2;
-      if (ecount <= kWCap + 2) {
-        for (int k = threadIdx.x; k < ecount; k += kThreads) s_E[k] = P.E[tw.clo + k];
-        Eptr = s_E - tw.clo;
-      }
-    }
-    __syncthreads();
+    int2 dn = make_int2(0, 0);
+    const int tnext = tile + 2 * G;
+    if (threadIdx.x == 0 && tnext < ntiles) dn = cur.desc[tnext];
+    // destination bases of this tile's window (consumed after phase 1: the load stays in flight meanwhile)
+    int mybase = 0;
+    if ((int)threadIdx.x < tw.W) mybase = P.tile_base[tile_row_offset(d.x, tile, P.R) + threadIdx.x];
+    mbar_wait(&bar[it & 1], (unsigned)(it >> 1) & 1u);
 
-    // phase 1: load (and, for V2, recompute) every particle of the tile; stable rank inside the warp
+    int e0, ne;
+    const double* Eptr = e_window(d.x, d.y, e0, ne) ? (S->E - e0) : P.E;
+
+    // phase 1: new state of every particle of the tile (V2: recomputed), stable rank inside the warp, deposit
     double x[kItems], vx[kItems], vy[kItems], vz[kItems];
-    unsigned pid[kItems];
     int key[kItems];        // window-relative new cell, or -1 when the particle is not placed by this tile
     unsigned rank[kItems];
-    unsigned char sp[kItems];
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
-      const unsigned off = (unsigned)(warp * kWarpSpan + r * 32 + lane);
+      const int off = warp * kWarpSpan + r * 32 + lane;
       key[r] = -1;
-      if (off < cnt) {
-        const unsigned i = base + off;
-        x[r] = cur.x[i]; vx[r] = cur.vx[i]; vy[r] = cur.vy[i]; vz[r] = cur.vz[i];
-        pid[r] = cur.pid[i]; sp[r] = cur.sp[i];
-        int c = cur.cell[i];
-        if (VARIANT == 2) advance<false>(P, s_sp, step, Eptr, sp[r], pid[r], i, x[r], vx[r], vy[r], vz[r], c);
+      int sp = 0;
+      if ((unsigned)off < cnt) {
+        sp = S->sp[off];
+        int c = S->cell[off];
+        x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off];
+        if (VARIANT == 2) {
+          const bool evt = (S->evt[warp * kItems + r] >> lane) & 1u;
+          if (evt) {
+            c = slow_advance<false>(P, s_sp, step, Eptr, S, off, base + (unsigned)off);
+            x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off];
+          } else {
+            push_fast(P, s_sp[sp], Eptr, c, x[r], vx[r], vy[r], vz[r]);
+            c = cell_of(P, x[r]);
+          }
+        }
         if (c >= 0) {
           const int k = c - tw.wlo;
           if (k >= 0 && k < tw.W) key[r] = k;
         }
       }
-    }
-#pragma unroll
-    for (int r = 0; r < kItems; ++r) {
       const unsigned mk = key[r] >= 0 ? (unsigned)key[r] : (0x80000000u | (unsigned)lane);
       const unsigned m = __match_any_sync(0xffffffffu, mk);
       const int leader = __ffs(m) - 1;
@@ -371,36 +486,35 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
       }
       old = __shfl_sync(0xffffffffu, old, leader);
       rank[r] = old + (unsigned)__popc(m & lt);
-      __syncwarp();
-    }
-
-    // look-back: particles that earlier tiles put into each cell of this window
-    for (int k = warp; k < tw.W; k += kWarps) {
-      const int c = tw.wlo + k;
-      int pre = 0;
-      if (c >= 0 && c < P.nc) {
-        for (int t0 = tile - 1; t0 >= 0; t0 -= 32) {
-          const int t = t0 - lane;
-          bool covers = false;
-          if (t >= 0) {
-            const int2 dd = P.tile_desc[t];
-            const TileWin w2 = make_window(dd.x, dd.y, P.R);
-            covers = c < w2.wlo + w2.W;  // wlo is monotone in t, so c >= w2.wlo always holds
-            if (covers) pre += (int)P.tile_hist[tile_row_offset(dd.x, t, P.R) + (size_t)(c - w2.wlo)];
+      // deposit (SURVEY 8(c) "D"): one shared-memory atomic pair per (cell, species) run of the warp
+      if (key[r] >= 0) {
+        const unsigned Q = (unsigned)s_sp[sp].Q;
+        const unsigned a = deposit_a(x[r], tw.wlo + key[r], P.inv_dx, Q);
+        if (P.dep_u32) {
+          // Q < 2^21 here: sum of a over a warp < 2^26, the count (<= 32) rides in bits 26..31
+          for (int s = 0; s < ns; ++s) {
+            const unsigned packed = __reduce_add_sync(m, sp == s ? (a + (1u << 26)) : 0u);
+            if (lane == leader && packed) {
+              const unsigned num = packed >> 26, sa = packed & ((1u << 26) - 1u);
+              atomicAdd(&s_dens[key[r] * ns + s], num * (unsigned)s_sp[s].Q - sa);
+              atomicAdd(&s_dens[(key[r] + 1) * ns + s], sa);
+            }
           }
-          // windows' upper ends are monotone: once a tile misses c every earlier one does
-          if (__any_sync(0xffffffffu, !covers)) break;
+        } else {
+          const int c = tw.wlo + key[r];
+          int j1 = c + 1;
+          if (!P.bc && j1 == P.nc) j1 = 0;
+          atomicAdd((unsigned long long*)&P.dens[(size_t)sp * P.ng + c], (unsigned long long)(Q - a));
+          atomicAdd((unsigned long long*)&P.dens[(size_t)sp * P.ng + j1], (unsigned long long)a);
         }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) pre += __shfl_xor_sync(0xffffffffu, pre, o);
-        pre += P.cell_base[c];
       }
-      if (lane == 0) s_base[k] = pre;
+      __syncwarp();
     }
     __syncthreads();
     // exclusive scan over the warps of the tile, per cell: s_wcnt becomes the destination base
-    for (int k = threadIdx.x; k < tw.W; k += kThreads) {
-      unsigned run = (unsigned)s_base[k];
+    if ((int)threadIdx.x < tw.W) {
+      unsigned run = (unsigned)mybase;
+      const int k = threadIdx.x;
 #pragma unroll
       for (int w = 0; w < kWarps; ++w) {
         const unsigned t = s_wcnt[k * kWarps + w];
@@ -410,50 +524,50 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     }
     __syncthreads();
 
-    // phase 2: scatter + deposit
+    // phase 2: scatter (pid and species are read again from the stage)
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
       if (key[r] >= 0) {
+        const int off = warp * kWarpSpan + r * 32 + lane;
         const unsigned dst = s_wcnt[key[r] * kWarps + warp] + rank[r];
         const int c = tw.wlo + key[r];
         nxt.x[dst] = x[r]; nxt.vx[dst] = vx[r]; nxt.vy[dst] = vy[r]; nxt.vz[dst] = vz[r];
-        nxt.cell[dst] = c; nxt.pid[dst] = pid[r]; nxt.sp[dst] = sp[r];
-        const unsigned Q = (unsigned)s_sp[sp[r]].Q;
-        const unsigned a = deposit_a(x[r], c, P.inv_dx, Q);
-        if (P.dep_u32) {
-          atomicAdd(&s_dens[key[r] * P.ns + sp[r]], Q - a);
-          atomicAdd(&s_dens[(key[r] + 1) * P.ns + sp[r]], a);
-        } else {
-          int j1 = c + 1;
-          if (!P.bc && j1 == P.nc) j1 = 0;
-          atomicAdd((unsigned long long*)&P.dens[(size_t)sp[r] * P.ng + c], (unsigned long long)(Q - a));
-          atomicAdd((unsigned long long*)&P.dens[(size_t)sp[r] * P.ng + j1], (unsigned long long)a);
-        }
+        nxt.cell[dst] = c; nxt.pid[dst] = S->pid[off]; nxt.sp[dst] = S->sp[off];
+        if ((dst & (kTile - 1)) == 0) nxt.desc[dst / kTile].x = c;
+        if ((dst & (kTile - 1)) == kTile - 1 || dst == n_next - 1) nxt.desc[dst / kTile].y = c;
       }
     }
+    fence_proxy_async();
     __syncthreads();
+    // flush the tile's deposit and clear the per-tile arrays
     if (P.dep_u32) {
-      for (int k = threadIdx.x; k < P.ns * (tw.W + 1); k += kThreads) {
+      for (int k = threadIdx.x; k < ns * (tw.W + 1); k += THREADS) {
         const unsigned v = s_dens[k];
         if (v) {
-          const int kk = k / P.ns, s = k - kk * P.ns;
+          s_dens[k] = 0;
+          const int kk = k / ns, s = k - kk * ns;
           int j = tw.wlo + kk;
           if (!P.bc && j == P.nc) j = 0;
           atomicAdd((unsigned long long*)&P.dens[(size_t)s * P.ng + j], (unsigned long long)v);
         }
       }
     }
+    for (int k = threadIdx.x; k < kWarps * tw.W; k += THREADS) s_wcnt[k] = 0;
+    if (threadIdx.x == 0 && tnext < ntiles)
+      issue_tile(P, cur, S, &bar[it & 1], tnext, dn, VARIANT == 2, VARIANT == 2);
     __syncthreads();
   }
 
   // side list: far movers and births go to the slots k_mid computed for them
   const unsigned Mv = P.st->ovf_valid;
-  for (unsigned p = blockIdx.x * blockDim.x + threadIdx.x; p < Mv; p += gridDim.x * blockDim.x) {
+  for (unsigned p = blockIdx.x * THREADS + threadIdx.x; p < Mv; p += G * THREADS) {
     const int dst = P.ovf_dst[p];
     const OvfRec rec = P.ovf_rec[P.ovf_idx[p]];
     const int c = (int)(P.ovf_key[p] >> kCellShift);
     nxt.x[dst] = rec.x; nxt.vx[dst] = rec.vx; nxt.vy[dst] = rec.vy; nxt.vz[dst] = rec.vz;
     nxt.cell[dst] = c; nxt.pid[dst] = rec.pid; nxt.sp[dst] = (unsigned char)rec.sp;
+    if (((unsigned)dst & (kTile - 1)) == 0) nxt.desc[dst / kTile].x = c;
+    if (((unsigned)dst & (kTile - 1)) == kTile - 1 || (unsigned)dst == n_next - 1) nxt.desc[dst / kTile].y = c;
     const unsigned Q = (unsigned)s_sp[rec.sp].Q;
     const unsigned a = deposit_a(rec.x, c, P.inv_dx, Q);
     int j1 = c + 1;
@@ -465,7 +579,7 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
 
 // ---------------------------------------------------------------------------------------------
 // Standalone deposit (load / restart; also SURVEY 8(a) row a5 as its own kernel).
-__global__ void __launch_bounds__(kThreads) k_deposit(const __grid_constant__ Params P, Particles cur) {
+__global__ void __launch_bounds__(kAuxThreads) k_deposit(const __grid_constant__ Params P, Particles cur) {
   const unsigned n = P.st->n;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
     const int c = cur.cell[i], s = cur.sp[i];
@@ -659,46 +773,71 @@ static int sm_count() {
   return g_sms;
 }
 
-size_t pass_b_smem_bytes(int ns) {
-  size_t words = (size_t)kWarps * kWCap + kWCap + (((size_t)ns * (kWCap + 1) + 1) & ~(size_t)1);
-  return words * 4 + (size_t)(kWCap + 2) * 8;
-}
-
-int particle_grid(const Params& P, int ctas_per_sm) {
-  const int want = sm_count() * ctas_per_sm;
+// persistent grid: one CTA per SM (or one per tile when there are fewer tiles than SMs)
+static int particle_grid(const Params& P) {
+  const int want = sm_count();
   return P.max_tiles < want ? (P.max_tiles > 0 ? P.max_tiles : 1) : want;
 }
 
-cudaError_t configure_kernels(int ns) {
-  const int bytes = (int)pass_b_smem_bytes(ns);
-  cudaError_t e = cudaFuncSetAttribute(k_pass_b<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+template <int THREADS>
+static cudaError_t configure_threads() {
+  typedef PassSmem<THREADS> SM;
+  cudaError_t e;
+  e = cudaFuncSetAttribute(k_pass_a<1, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::a_total);
   if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(k_pass_b<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  e = cudaFuncSetAttribute(k_pass_a<2, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::a_total);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_pass_b<1, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::b_total);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_pass_b<2, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::b_total);
 }
 
-int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int variant, cudaStream_t s,
-                cudaEvent_t* ev) {
-  const int ga = particle_grid(P, 4), gb = particle_grid(P, 2);
-  const size_t smem_b = pass_b_smem_bytes(P.ns);
+cudaError_t configure_kernels() {
+  cudaError_t e = configure_threads<512>();
+  if (e != cudaSuccess) return e;
+  return configure_threads<1024>();
+}
+
+template <int THREADS>
+static void launch_passes(const Params& P, const Particles& cur, const Particles& nxt, int variant, cudaStream_t s,
+                          cudaEvent_t* ev) {
+  typedef PassSmem<THREADS> SM;
+  const int g = particle_grid(P);
+  const int gc = (P.max_tiles + (kColThreads / 32) - 1) / (kColThreads / 32);
   if (ev) cudaEventRecord(ev[0], s);
-  if (variant == 2) k_pass_a<2><<<ga, kThreads, 0, s>>>(P, cur);
-  else k_pass_a<1><<<ga, kThreads, 0, s>>>(P, cur);
+  if (variant == 2) k_pass_a<2, THREADS><<<g, THREADS, SM::a_total, s>>>(P, cur);
+  else k_pass_a<1, THREADS><<<g, THREADS, SM::a_total, s>>>(P, cur);
   if (ev) cudaEventRecord(ev[1], s);
   k_mid<<<1, kMidThreads, 0, s>>>(P);
+  k_colscan<<<gc < 1 ? 1 : (gc > 16384 ? 16384 : gc), kColThreads, 0, s>>>(P, cur);
   if (ev) cudaEventRecord(ev[2], s);
-  if (variant == 2) k_pass_b<2><<<gb, kThreads, smem_b, s>>>(P, cur, nxt);
-  else k_pass_b<1><<<gb, kThreads, smem_b, s>>>(P, cur, nxt);
+  if (variant == 2) k_pass_b<2, THREADS><<<g, THREADS, SM::b_total, s>>>(P, cur, nxt);
+  else k_pass_b<1, THREADS><<<g, THREADS, SM::b_total, s>>>(P, cur, nxt);
   if (ev) cudaEventRecord(ev[3], s);
   k_field<<<1, kFieldThreads, 0, s>>>(P, 1);
   if (ev) cudaEventRecord(ev[4], s);
-  return 4;
+}
+
+int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int variant, int threads,
+                cudaStream_t s, cudaEvent_t* ev) {
+  if (threads == 1024) launch_passes<1024>(P, cur, nxt, variant, s, ev);
+  else launch_passes<512>(P, cur, nxt, variant, s, ev);
+  return 5;
 }
 
 // load / restart: counts -> cell_start, deposit, field (no push).  cur must be sorted by cell.
-__global__ void __launch_bounds__(kThreads) k_count_cells(const __grid_constant__ Params P, Particles cur) {
+__global__ void __launch_bounds__(kAuxThreads) k_count_cells(const __grid_constant__ Params P, Particles cur) {
   const unsigned n = P.st->n;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
     atomicAdd(&P.cell_count[cur.cell[i]], 1);
+}
+__global__ void __launch_bounds__(kAuxThreads) k_tile_desc(const __grid_constant__ Params P, Particles cur) {
+  const unsigned n = P.st->n;
+  const unsigned ntiles = (n + kTile - 1) / kTile;
+  for (unsigned t = blockIdx.x * blockDim.x + threadIdx.x; t < ntiles; t += gridDim.x * blockDim.x) {
+    const unsigned last = min(n, (t + 1) * (unsigned)kTile) - 1u;
+    cur.desc[t] = make_int2(cur.cell[(size_t)t * kTile], cur.cell[last]);
+  }
 }
 __global__ void k_clear_grids(const __grid_constant__ Params P) {
   const size_t tot = (size_t)P.ns * (size_t)P.ng;
@@ -713,11 +852,12 @@ __global__ void k_clear_grids(const __grid_constant__ Params P) {
 int launch_rebuild(const Params& P, const Particles& cur, cudaStream_t s) {
   const int g = sm_count() * 4;
   k_clear_grids<<<g, 256, 0, s>>>(P);
-  k_count_cells<<<g, kThreads, 0, s>>>(P, cur);
+  k_count_cells<<<g, kAuxThreads, 0, s>>>(P, cur);
+  k_tile_desc<<<g, kAuxThreads, 0, s>>>(P, cur);
   k_mid<<<1, kMidThreads, 0, s>>>(P);   // ovf_count == 0: plain scan; n_next = n
-  k_deposit<<<g, kThreads, 0, s>>>(P, cur);
+  k_deposit<<<g, kAuxThreads, 0, s>>>(P, cur);
   k_field<<<1, kFieldThreads, 0, s>>>(P, 0);  // commits n = n_next, leaves the step counter alone
-  return 5;
+  return 6;
 }
 
 }  // namespace bit1
