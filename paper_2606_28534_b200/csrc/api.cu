@@ -151,7 +151,7 @@ struct bit1_ctx {
   cudaStream_t cs, ss;
   cudaEvent_t ev_snap, ev_done;
   bool ckpt_pending, staging, loaded;
-  int variant, threads;
+  int variant;
   uint64_t launches, cfg_hash;
   double m[BIT1_MAX_SPECIES], weight[BIT1_MAX_SPECIES];
   double dt;
@@ -231,8 +231,6 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   c->staging = staging != 0;
   c->variant = o->variant == 1 ? 1 : 2;
   if (const char* ev = getenv("BIT1_VARIANT")) { if (atoi(ev) == 1) c->variant = 1; else if (atoi(ev) == 2) c->variant = 2; }
-  c->threads = 512;
-  if (const char* ev = getenv("BIT1_THREADS")) { if (atoi(ev) == 1024) c->threads = 1024; }
   c->cur = 0; c->loaded = false; c->ckpt_pending = false; c->launches = 0; c->dt = dt;
   c->profiling = false; c->prof_steps = 0;
 
@@ -266,6 +264,14 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
     q.sy = (2.0 * q.ty) / (1.0 + tt);
     q.sz = (2.0 * q.tz) / (1.0 + tt);
     q.src_vth = sp[s].src_vth; q.pnull = sp[s].pnull; q.numax = sp[s].numax;
+    // integer form of the candidate test: the uniform is u = (w + 0.5) * 2^-52 with a 52-bit integer w (exact),
+    // so u < pnull  <=>  w + 0.5 < y = pnull * 2^52 (exact scaling)  <=>  w < floor(y) + (frac(y) > 0.5)
+    q.pthr = 0;
+    if ((sp[s].flags & (BIT1_ELASTIC | BIT1_IONISE | BIT1_CX)) && sp[s].pnull > 0.0) {
+      const double y = (sp[s].pnull < 1.0 ? sp[s].pnull : 1.0) * 4503599627370496.0;
+      const double fl = floor(y);
+      q.pthr = (unsigned long long)fl + ((y - fl) > 0.5 ? 1ull : 0ull);
+    }
     q.kin_eV = (0.5 * sp[s].m) / kECharge;
     q.two_e_over_m = (2.0 * kECharge) / sp[s].m;
     q.el_loss = o->m_n > 0.0 ? (2.0 * sp[s].m) / o->m_n : 0.0;
@@ -273,7 +279,7 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
     q.sign = sp[s].q > 0.0 ? 1 : (sp[s].q < 0.0 ? -1 : 0);
     q.flags = sp[s].flags; q.src_mode = sp[s].src_mode; q.src_partner = sp[s].src_partner;
     if (q.Q < 1 || q.Q >= (1ll << 31)) { delete c; return BIT1_ERR_RANGE; }
-    if ((unsigned long long)q.Q * (unsigned long long)kTile >= (1ull << 32)) P.dep_u32 = 0;  // => Q < 2^21
+    if ((unsigned long long)q.Q * (unsigned long long)kTile >= (1ull << 32) || q.Q >= (1ll << 21)) P.dep_u32 = 0;
     c->m[s] = sp[s].m; c->weight[s] = sp[s].weight;
   }
   char* ws = c->ws;
@@ -423,7 +429,7 @@ bit1_status bit1_step(bit1_ctx* c, uint64_t nsteps) {
       ev = &c->prof_ev[c->prof_steps * 5];
       c->prof_steps++;
     }
-    c->launches += launch_step(c->P, c->buf[c->cur], c->buf[c->cur ^ 1], c->variant, c->threads, c->cs, ev);
+    c->launches += launch_step(c->P, c->buf[c->cur], c->buf[c->cur ^ 1], c->variant, c->cs, ev);
     c->cur ^= 1;
   }
   CUDA_OK(cudaGetLastError());

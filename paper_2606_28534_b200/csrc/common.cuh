@@ -6,8 +6,27 @@
 namespace bit1 {
 
 constexpr int kMaxSpecies = 8;
-constexpr int kTile = 2048;               // particles per tile (one TMA stage)
-constexpr int kWCap = 256;                // max cells in a tile's window (smem histogram bins)
+// Geometry of the two particle passes (compile-time).  Two CTAs of 256 threads share an SM,
+// each streaming tiles of 1024 particles: while one CTA sits at a barrier or waits for its tile, the other issues.
+#ifndef BIT1_THREADS
+#define BIT1_THREADS 256
+#endif
+#ifndef BIT1_ITEMS
+#define BIT1_ITEMS 4
+#endif
+#ifndef BIT1_MINBLOCKS
+#define BIT1_MINBLOCKS 2
+#endif
+#ifndef BIT1_WCAP
+#define BIT1_WCAP 128
+#endif
+constexpr int kThreads = BIT1_THREADS;    // threads per CTA of the particle passes
+constexpr int kItems = BIT1_ITEMS;        // particles per thread and tile
+constexpr int kMinBlocks = BIT1_MINBLOCKS;  // CTAs per SM the passes are compiled and launched for
+constexpr int kTile = kThreads * kItems;  // particles per tile (one TMA stage)
+constexpr int kWCap = BIT1_WCAP;          // max cells in a tile's window (smem histogram bins)
+constexpr int kWarps = kThreads / 32;
+static_assert(kWCap <= kThreads && (32 % kWarps == 0 || kWarps % 32 == 0), "pass geometry");
 
 // overflow ("far mover" / birth) key: cell(28) | cls(2) | ord(34)
 constexpr int kOrdBits = 34;
@@ -21,7 +40,9 @@ constexpr unsigned kElastic = 1u, kIonise = 2u, kCx = 4u, kIonProduct = 8u, kEle
 constexpr int kSrcNone = 0, kSrcSelf = 1, kSrcPair = 2;
 
 struct __align__(16) SpeciesP {
-  double h, tx, ty, tz, sx, sy, sz, pnull;   // the per-particle fast path reads these eight (four 128-bit loads)
+  double h, tx, ty, tz, sx, sy, sz;          // the per-particle fast path reads these seven and pthr
+  unsigned long long pthr;                   // u52(w) < pnull  <=>  w < pthr  (52-bit w; exact, see api.cu)
+  double pnull;
   double src_vth, numax, kin_eV, two_e_over_m, el_loss;
   long long Q;
   int sign;

@@ -1,6 +1,6 @@
-// Tile staging for the two particle passes: one tile (2048 particles, all seven SoA arrays, its event bits and
+// Tile staging for the two particle passes: one tile (kTile particles, all seven SoA arrays, its event bits and
 // its window of E) is brought into shared memory by 1D bulk-async copies (TMA, SASS UBLKCP) that complete on an
-// mbarrier, two stages deep, so that the next tile's 86 KB are in flight while the current tile is computed.
+// mbarrier, two stages deep, so that the next tile's 41 B x kTile are in flight while the current tile is computed.
 // bytes in flight per SM are decoupled from registers and occupancy.
 #pragma once
 #include "common.cuh"
@@ -14,6 +14,7 @@ struct __align__(128) Stage {
   unsigned char sp[kTile];
   unsigned evt[kTile / 32];
   double E[kWCap + 4];  // E[e0 .. ], e0 = clo & ~1 (16-byte aligned source)
+  int2 d;               // (first, last) old cell of the staged tile; plain store by the issuing thread
 };
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -65,6 +66,7 @@ __device__ __forceinline__ void issue_tile(const Params& P, const Particles& cur
   unsigned bytes = 4u * kTile * 8u + 2u * kTile * 4u + kTile;
   if (with_evt) bytes += kTile / 8;
   if (stage_E) bytes += (unsigned)ne * 8u;
+  st->d = d;
   mbar_expect_tx(bar, bytes);
   bulk_g2s(st->x, cur.x + base, kTile * 8, bar);
   bulk_g2s(st->vx, cur.vx + base, kTile * 8, bar);

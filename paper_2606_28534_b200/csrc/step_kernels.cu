@@ -6,8 +6,8 @@
 //   k_pass_b   arranger: stable ranks inside the tile, scatter to the sorted position with the charge
 //              deposition fused                                    (rows a4-a5; PAPER.md:111 arrj/narrj)
 //   k_field    exact integer-scan Poisson solve -> phi, E          (row a6; PAPER.md:33 step (iii))
-// Both particle passes are persistent (one CTA per SM) and read their tiles through the two-stage bulk-async
-// pipeline of pipeline.cuh.
+// Both particle passes are persistent (kMinBlocks CTAs per SM) and read their tiles through the two-stage
+// bulk-async pipeline of pipeline.cuh.
 #include "advance.cuh"
 #include "step_kernels.h"
 
@@ -37,30 +37,47 @@ constexpr int kAuxThreads = 256;
 constexpr unsigned kCollMask = kElastic | kIonise | kCx;
 
 // dynamic shared memory of both passes: [2 x Stage][pass-specific arrays][species][2 barriers]
-template <int THREADS>
 struct PassSmem {
-  static constexpr int kWarps = THREADS / 32;
   static constexpr size_t stages = 2 * sizeof(Stage);
-  static constexpr size_t a_hist = stages;                                  // unsigned[kWCap]
-  static constexpr size_t a_sp = a_hist + kWCap * 4;                        // SpeciesP[kMaxSpecies]
-  static constexpr size_t a_bar = a_sp + kMaxSpecies * sizeof(SpeciesP);    // 2 x u64
+  static constexpr size_t a_hist = stages;                                  // unsigned[2][kWCap]
+  static constexpr size_t a_sp = a_hist + 2 * kWCap * 4;                    // SpeciesP[kMaxSpecies]
+  static constexpr size_t a_bar = (a_sp + kMaxSpecies * sizeof(SpeciesP) + 15) & ~(size_t)15;  // 2 x u64
   static constexpr size_t a_total = a_bar + 16;
   static constexpr size_t b_wcnt = stages;                                  // unsigned[kWCap][kWarps]
-  static constexpr size_t b_dens = b_wcnt + (size_t)kWCap * kWarps * 4;     // unsigned[kWCap + 1][kMaxSpecies]
+  static constexpr size_t b_base = b_wcnt + (size_t)kWCap * kWarps * 4;     // unsigned[kWCap][kWarps]
+  static constexpr size_t b_tb = b_base + (size_t)kWCap * kWarps * 4;       // int[kWCap]
+  static constexpr size_t b_dens = b_tb + (size_t)kWCap * 4;                // unsigned[kWCap + 1][kMaxSpecies]
   static constexpr size_t b_sp = b_dens + (size_t)(kWCap + 1) * kMaxSpecies * 4 + 32;
   static constexpr size_t b_bar = (b_sp + kMaxSpecies * sizeof(SpeciesP) + 15) & ~(size_t)15;
   static constexpr size_t b_total = b_bar + 16;
 };
 
+// (cell of the first particle, cell of the last particle) of tile t, read from the sorted cell array itself
+__device__ __forceinline__ int2 tile_cells(const Particles& cur, int t, unsigned n) {
+  const size_t first = (size_t)t * kTile;
+  const size_t end = first + kTile;
+  const size_t last = (end < (size_t)n ? end : (size_t)n) - 1;
+  return make_int2(cur.cell[first], cur.cell[last]);
+}
+
+// first 52 bits of the two-word uniform of slot C0 as an integer: u52(a, b) = (w + 0.5) * 2^-52
+__device__ __forceinline__ unsigned long long w52(unsigned a, unsigned b) {
+  return (((unsigned long long)a << 32) | (unsigned long long)b) >> 12;
+}
+
 // ---------------------------------------------------------------------------------------------
 // Pass A.  VARIANT 1 writes the advanced state back in place; VARIANT 2 writes one event bit per particle.
-template <int VARIANT, int THREADS>
-__global__ void __launch_bounds__(THREADS, 1) k_pass_a(const __grid_constant__ Params P, Particles cur) {
-  constexpr int kItems = kTile / THREADS, kWarpSpan = 32 * kItems;
-  typedef PassSmem<THREADS> SM;
+// Per tile: phase 1 is straight-line arithmetic over the thread's kItems particles (no warp-wide operation in
+// it, so the compiler interleaves the independent dependency chains); phase 2 redoes the rare particles (wall
+// hit, periodic wrap, null-collision candidate, move beyond the window) through the full advance(); phase 3
+// builds the banded histogram.  One CTA barrier per tile: the histogram is double-buffered.
+template <int VARIANT>
+__global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_constant__ Params P, Particles cur) {
+  constexpr int kWarpSpan = 32 * kItems;
+  typedef PassSmem SM;
   extern __shared__ __align__(128) unsigned char smem[];
   Stage* stg = reinterpret_cast<Stage*>(smem);
-  unsigned* s_hist = reinterpret_cast<unsigned*>(smem + SM::a_hist);
+  unsigned* s_hist2 = reinterpret_cast<unsigned*>(smem + SM::a_hist);
   SpeciesP* s_sp = reinterpret_cast<SpeciesP*>(smem + SM::a_sp);
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem + SM::a_bar);
 
@@ -77,68 +94,103 @@ __global__ void __launch_bounds__(THREADS, 1) k_pass_a(const __grid_constant__ P
     fence_proxy_async();
     for (int k = 0; k < 2; ++k) {
       const int t = blockIdx.x + k * G;
-      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, cur.desc[t], false, true);
+      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, tile_cells(cur, t, n), false, true);
     }
   }
   load_species(P, s_sp);
-  for (int k = threadIdx.x; k < kWCap; k += THREADS) s_hist[k] = 0;
+  for (int k = threadIdx.x; k < 2 * kWCap; k += kThreads) s_hist2[k] = 0;
   // the deposition of this step accumulates into dens: clear it here (nobody reads it during pass A)
   {
     const size_t tot = (size_t)P.ns * (size_t)P.ng;
-    for (size_t i = (size_t)blockIdx.x * THREADS + threadIdx.x; i < tot; i += (size_t)G * THREADS) P.dens[i] = 0;
+    for (size_t i = (size_t)blockIdx.x * kThreads + threadIdx.x; i < tot; i += (size_t)G * kThreads) P.dens[i] = 0;
   }
   __syncthreads();
 
   int it = 0;
   for (int tile = blockIdx.x; tile < ntiles; tile += G, ++it) {
     Stage* S = &stg[it & 1];
+    unsigned* s_hist = s_hist2 + (it & 1) * kWCap;
     const unsigned base = (unsigned)tile * kTile;
     const unsigned cnt = min((unsigned)kTile, n - base);
-    // descriptor of the tile after next (its load is issued at the end of this iteration)
+    // cells of the tile after next (its load is issued at the end of this iteration)
     int2 dn = make_int2(0, 0);
     const int tnext = tile + 2 * G;
-    if (threadIdx.x == 0 && tnext < ntiles) dn = cur.desc[tnext];
+    if (threadIdx.x == 0 && tnext < ntiles) dn = tile_cells(cur, tnext, n);
     mbar_wait(&bar[it & 1], (unsigned)(it >> 1) & 1u);
 
-    const int clo = S->cell[0], chi = S->cell[cnt - 1];
+    const int clo = S->d.x, chi = S->d.y;
+    if (threadIdx.x == 0) cur.desc[tile] = S->d;   // read by k_colscan and by pass B's issuing thread
     const TileWin tw = make_window(clo, chi, P.R);
     int e0, ne;
     const double* Eptr = e_window(clo, chi, e0, ne) ? (S->E - e0) : P.E;
 
+    // phase 1
+    int cn[kItems];
+    double x[kItems], vx[kItems], vy[kItems], vz[kItems];
+    unsigned long long thr[kItems];
+    unsigned evm = 0;
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) {
+      const int off = warp * kWarpSpan + r * 32 + lane;
+      const bool have = (unsigned)off < cnt;
+      const int sp = have ? (int)S->sp[off] : 0;
+      const SpeciesP& s = s_sp[sp];
+      const int c = have ? S->cell[off] : clo;
+      x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off];
+      const bool inside = push_fast(P, s, Eptr, c, x[r], vx[r], vy[r], vz[r]);
+      cn[r] = cell_of(P, x[r]);
+      const int k = cn[r] - tw.wlo;
+      thr[r] = have ? s.pthr : 0ull;
+      if (have && !(inside && k >= 0 && k < tw.W)) evm |= 1u << r;
+    }
+    unsigned long long any = 0;
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) any |= thr[r];
+    if (any) {
+#pragma unroll
+      for (int r = 0; r < kItems; ++r) {
+        const int off = warp * kWarpSpan + r * 32 + lane;
+        const uint4 w = draw(P, S->pid[off], step, 0u);  // slot C0
+        if (w52(w.x, w.y) < thr[r]) evm |= 1u << r;
+      }
+    }
+    // phase 2
+    if (evm) {
+#pragma unroll
+      for (int r = 0; r < kItems; ++r) {
+        if ((evm >> r) & 1u) {
+          const int off = warp * kWarpSpan + r * 32 + lane;
+          const unsigned i = base + (unsigned)off;
+          const int c = slow_advance<true>(P, s_sp, step, Eptr, S, off, i);
+          cn[r] = c;
+          if (VARIANT == 1) { x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off]; }
+          if (c >= 0) {
+            const int k = c - tw.wlo;
+            if (!(k >= 0 && k < tw.W)) {
+              emit_record(P, make_key(c, c < tw.wlo ? 1u : 0u, (unsigned long long)i), S->x[off], S->vx[off],
+                          S->vy[off], S->vz[off], S->pid[off], (int)S->sp[off]);
+              cn[r] = -2;  // placed through the side list
+            }
+          }
+        }
+      }
+    }
+    // phase 3
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
       const int off = warp * kWarpSpan + r * 32 + lane;
       const bool have = (unsigned)off < cnt;
       unsigned key = 0x80000000u | (unsigned)lane;  // unique: matches nobody
-      bool evt = false;
       if (have) {
-        const unsigned i = base + (unsigned)off;
-        const int sp = S->sp[off];
-        const SpeciesP& s = s_sp[sp];
-        int c = S->cell[off];
-        double x = S->x[off], vx = S->vx[off], vy = S->vy[off], vz = S->vz[off];
-        evt = !push_fast(P, s, Eptr, c, x, vx, vy, vz);
-        if (!evt && (s.flags & kCollMask)) {
-          const uint4 w = draw(P, S->pid[off], step, 0u);  // slot C0
-          evt = u52(w.x, w.y) < s.pnull;
-        }
-        if (evt) {
-          c = slow_advance<true>(P, s_sp, step, Eptr, S, off, i);
-          x = S->x[off]; vx = S->vx[off]; vy = S->vy[off]; vz = S->vz[off];
-        } else {
-          c = cell_of(P, x);
-        }
         if (VARIANT == 1) {
-          cur.x[i] = x; cur.vx[i] = vx; cur.vy[i] = vy; cur.vz[i] = vz; cur.cell[i] = c;
+          const unsigned i = base + (unsigned)off;
+          cur.x[i] = x[r]; cur.vx[i] = vx[r]; cur.vy[i] = vy[r]; cur.vz[i] = vz[r];
+          cur.cell[i] = cn[r] == -2 ? -1 : cn[r];   // side-list particles are not placed by pass B's tile loop
         }
-        if (c >= 0) {
-          const int k = c - tw.wlo;
-          if (k >= 0 && k < tw.W) key = (unsigned)k;
-          else emit_record(P, make_key(c, c < tw.wlo ? 1u : 0u, (unsigned long long)i), x, vx, vy, vz, S->pid[off], sp);
-        }
+        if (cn[r] >= 0) key = (unsigned)(cn[r] - tw.wlo);
       }
       if (VARIANT == 2) {
-        const unsigned eb = __ballot_sync(0xffffffffu, evt);
+        const unsigned eb = __ballot_sync(0xffffffffu, (evm >> r) & 1u);
         if (lane == 0) P.evt[(base >> 5) + (unsigned)(warp * kItems + r)] = eb;
       }
       const unsigned m = __match_any_sync(0xffffffffu, key);
@@ -147,7 +199,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_pass_a(const __grid_constant__ P
     fence_proxy_async();
     __syncthreads();
     unsigned* row = P.tile_hist + tile_row_offset(clo, tile, P.R);
-    for (int k = threadIdx.x; k < tw.W; k += THREADS) {
+    for (int k = threadIdx.x; k < tw.W; k += kThreads) {
       const unsigned h = s_hist[k];
       s_hist[k] = 0;
       row[k] = h;
@@ -155,7 +207,6 @@ __global__ void __launch_bounds__(THREADS, 1) k_pass_a(const __grid_constant__ P
       if (h && c >= 0 && c < P.nc) atomicAdd(&P.cell_count[c], (int)h);
     }
     if (threadIdx.x == 0 && tnext < ntiles) issue_tile(P, cur, S, &bar[it & 1], tnext, dn, false, true);
-    __syncthreads();
   }
 }
 
@@ -394,20 +445,25 @@ __global__ void __launch_bounds__(kColThreads) k_colscan(const __grid_constant__
 }
 
 // ---------------------------------------------------------------------------------------------
-// Pass B.
-template <int VARIANT, int THREADS>
-__global__ void __launch_bounds__(THREADS, 1)
+// Pass B.  Per tile: phase 1 recomputes the push (V2) as straight-line arithmetic, phase 1b redoes the particles
+// pass A flagged through the full advance(), phase 2 ranks the particles inside (warp, new cell) and deposits;
+// after barrier 1 a segmented warp scan turns the per-warp counts into destinations while the other threads
+// flush the tile's deposit; after barrier 2 the scatter; barrier 3 frees the stage for the next load.
+template <int VARIANT>
+__global__ void __launch_bounds__(kThreads, kMinBlocks)
 k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
-  constexpr int kItems = kTile / THREADS, kWarpSpan = 32 * kItems, kWarps = THREADS / 32;
-  typedef PassSmem<THREADS> SM;
+  constexpr int kWarpSpan = 32 * kItems;
+  typedef PassSmem SM;
   extern __shared__ __align__(128) unsigned char smem[];
   Stage* stg = reinterpret_cast<Stage*>(smem);
-  unsigned* s_wcnt = reinterpret_cast<unsigned*>(smem + SM::b_wcnt);   // [kWCap][kWarps]
+  unsigned* s_wcnt = reinterpret_cast<unsigned*>(smem + SM::b_wcnt);   // [kWCap][kWarps] counts, zero between tiles
+  unsigned* s_base = reinterpret_cast<unsigned*>(smem + SM::b_base);   // [kWCap][kWarps] destinations
+  int* s_tb = reinterpret_cast<int*>(smem + SM::b_tb);                 // [kWCap] this tile's row of tile_base
   unsigned* s_dens = reinterpret_cast<unsigned*>(smem + SM::b_dens);   // [kWCap + 1][ns]
   SpeciesP* s_sp = reinterpret_cast<SpeciesP*>(smem + SM::b_sp);
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem + SM::b_bar);
 
-  const unsigned n = P.st->n, n_next = P.st->n_next;
+  const unsigned n = P.st->n;
   const unsigned long long step = P.st->step;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned lt = lanemask_lt();
@@ -426,8 +482,8 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     }
   }
   load_species(P, s_sp);
-  for (int k = threadIdx.x; k < kWCap * kWarps; k += THREADS) s_wcnt[k] = 0;
-  for (int k = threadIdx.x; k < (kWCap + 1) * kMaxSpecies; k += THREADS) s_dens[k] = 0;
+  for (int k = threadIdx.x; k < kWCap * kWarps; k += kThreads) s_wcnt[k] = 0;
+  for (int k = threadIdx.x; k < (kWCap + 1) * kMaxSpecies; k += kThreads) s_dens[k] = 0;
   __syncthreads();
 
   int it = 0;
@@ -435,12 +491,12 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     Stage* S = &stg[it & 1];
     const unsigned base = (unsigned)tile * kTile;
     const unsigned cnt = min((unsigned)kTile, n - base);
-    const int2 d = cur.desc[tile];
+    const int2 d = S->d;
     const TileWin tw = make_window(d.x, d.y, P.R);
     int2 dn = make_int2(0, 0);
     const int tnext = tile + 2 * G;
     if (threadIdx.x == 0 && tnext < ntiles) dn = cur.desc[tnext];
-    // destination bases of this tile's window (consumed after phase 1: the load stays in flight meanwhile)
+    // destination bases of this tile's window (consumed after barrier 1: the load stays in flight meanwhile)
     int mybase = 0;
     if ((int)threadIdx.x < tw.W) mybase = P.tile_base[tile_row_offset(d.x, tile, P.R) + threadIdx.x];
     mbar_wait(&bar[it & 1], (unsigned)(it >> 1) & 1u);
@@ -448,34 +504,42 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     int e0, ne;
     const double* Eptr = e_window(d.x, d.y, e0, ne) ? (S->E - e0) : P.E;
 
-    // phase 1: new state of every particle of the tile (V2: recomputed), stable rank inside the warp, deposit
+    // phase 1: new state of every particle of the tile
     double x[kItems], vx[kItems], vy[kItems], vz[kItems];
     int key[kItems];        // window-relative new cell, or -1 when the particle is not placed by this tile
-    unsigned rank[kItems];
+    unsigned evm = 0;
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
       const int off = warp * kWarpSpan + r * 32 + lane;
-      key[r] = -1;
-      int sp = 0;
-      if ((unsigned)off < cnt) {
-        sp = S->sp[off];
-        int c = S->cell[off];
-        x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off];
-        if (VARIANT == 2) {
-          const bool evt = (S->evt[warp * kItems + r] >> lane) & 1u;
-          if (evt) {
-            c = slow_advance<false>(P, s_sp, step, Eptr, S, off, base + (unsigned)off);
-            x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off];
-          } else {
-            push_fast(P, s_sp[sp], Eptr, c, x[r], vx[r], vy[r], vz[r]);
-            c = cell_of(P, x[r]);
-          }
-        }
-        if (c >= 0) {
+      const bool have = (unsigned)off < cnt;
+      int c = have ? S->cell[off] : d.x;
+      x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off];
+      if (VARIANT == 2) {
+        const int sp = have ? (int)S->sp[off] : 0;
+        if (have && ((S->evt[warp * kItems + r] >> lane) & 1u)) evm |= 1u << r;
+        push_fast(P, s_sp[sp], Eptr, c, x[r], vx[r], vy[r], vz[r]);
+        c = cell_of(P, x[r]);
+      }
+      const int k = c - tw.wlo;
+      key[r] = (have && c >= 0 && k >= 0 && k < tw.W) ? k : -1;
+    }
+    // phase 1b (V2): the particles pass A flagged take the full step again, side effects off
+    if (VARIANT == 2 && evm) {
+#pragma unroll
+      for (int r = 0; r < kItems; ++r) {
+        if ((evm >> r) & 1u) {
+          const int off = warp * kWarpSpan + r * 32 + lane;
+          const int c = slow_advance<false>(P, s_sp, step, Eptr, S, off, base + (unsigned)off);
+          x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off];
           const int k = c - tw.wlo;
-          if (k >= 0 && k < tw.W) key[r] = k;
+          key[r] = (c >= 0 && k >= 0 && k < tw.W) ? k : -1;
         }
       }
+    }
+    // phase 2: stable rank inside (warp, cell), per-warp counts, deposit
+    unsigned rank[kItems];
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) {
       const unsigned mk = key[r] >= 0 ? (unsigned)key[r] : (0x80000000u | (unsigned)lane);
       const unsigned m = __match_any_sync(0xffffffffu, mk);
       const int leader = __ffs(m) - 1;
@@ -488,6 +552,8 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
       rank[r] = old + (unsigned)__popc(m & lt);
       // deposit (SURVEY 8(c) "D"): one shared-memory atomic pair per (cell, species) run of the warp
       if (key[r] >= 0) {
+        const int off = warp * kWarpSpan + r * 32 + lane;
+        const int sp = (int)S->sp[off];
         const unsigned Q = (unsigned)s_sp[sp].Q;
         const unsigned a = deposit_a(x[r], tw.wlo + key[r], P.inv_dx, Q);
         if (P.dep_u32) {
@@ -510,64 +576,66 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
       }
       __syncwarp();
     }
-    __syncthreads();
-    // exclusive scan over the warps of the tile, per cell: s_wcnt becomes the destination base
-    if ((int)threadIdx.x < tw.W) {
-      unsigned run = (unsigned)mybase;
-      const int k = threadIdx.x;
+    if ((int)threadIdx.x < tw.W) s_tb[threadIdx.x] = mybase;
+    __syncthreads();  // barrier 1
+    // per cell, exclusive scan over the warps of the tile (groups of kWarps lanes) -> destination of each
+    // (cell, warp) run; the counts are zeroed for the next tile on the way
+    {
+      const int tot = tw.W * kWarps;
+      for (int b0 = warp * 32; b0 < tot; b0 += kThreads) {
+        const int idx = b0 + lane;
+        const unsigned v = idx < tot ? s_wcnt[idx] : 0u;
+        unsigned inc = v;
 #pragma unroll
-      for (int w = 0; w < kWarps; ++w) {
-        const unsigned t = s_wcnt[k * kWarps + w];
-        s_wcnt[k * kWarps + w] = run;
-        run += t;
+        for (int dd = 1; dd < (kWarps < 32 ? kWarps : 32); dd <<= 1) {
+          const unsigned t = __shfl_up_sync(0xffffffffu, inc, dd, kWarps < 32 ? kWarps : 32);
+          if ((lane & (kWarps - 1)) >= dd) inc += t;
+        }
+        if (idx < tot) {
+          s_wcnt[idx] = 0;
+          s_base[idx] = (unsigned)s_tb[idx / kWarps] + (inc - v);
+        }
+      }
+      // flush the tile's deposit
+      if (P.dep_u32) {
+        for (int k = threadIdx.x; k < ns * (tw.W + 1); k += kThreads) {
+          const unsigned v = s_dens[k];
+          if (v) {
+            s_dens[k] = 0;
+            const int kk = k / ns, s = k - kk * ns;
+            int j = tw.wlo + kk;
+            if (!P.bc && j == P.nc) j = 0;
+            atomicAdd((unsigned long long*)&P.dens[(size_t)s * P.ng + j], (unsigned long long)v);
+          }
+        }
       }
     }
-    __syncthreads();
+    __syncthreads();  // barrier 2
 
-    // phase 2: scatter (pid and species are read again from the stage)
+    // phase 3: scatter (pid and species are read again from the stage)
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
       if (key[r] >= 0) {
         const int off = warp * kWarpSpan + r * 32 + lane;
-        const unsigned dst = s_wcnt[key[r] * kWarps + warp] + rank[r];
-        const int c = tw.wlo + key[r];
+        const unsigned dst = s_base[key[r] * kWarps + warp] + rank[r];
         nxt.x[dst] = x[r]; nxt.vx[dst] = vx[r]; nxt.vy[dst] = vy[r]; nxt.vz[dst] = vz[r];
-        nxt.cell[dst] = c; nxt.pid[dst] = S->pid[off]; nxt.sp[dst] = S->sp[off];
-        if ((dst & (kTile - 1)) == 0) nxt.desc[dst / kTile].x = c;
-        if ((dst & (kTile - 1)) == kTile - 1 || dst == n_next - 1) nxt.desc[dst / kTile].y = c;
+        nxt.cell[dst] = tw.wlo + key[r]; nxt.pid[dst] = S->pid[off]; nxt.sp[dst] = S->sp[off];
       }
     }
     fence_proxy_async();
-    __syncthreads();
-    // flush the tile's deposit and clear the per-tile arrays
-    if (P.dep_u32) {
-      for (int k = threadIdx.x; k < ns * (tw.W + 1); k += THREADS) {
-        const unsigned v = s_dens[k];
-        if (v) {
-          s_dens[k] = 0;
-          const int kk = k / ns, s = k - kk * ns;
-          int j = tw.wlo + kk;
-          if (!P.bc && j == P.nc) j = 0;
-          atomicAdd((unsigned long long*)&P.dens[(size_t)s * P.ng + j], (unsigned long long)v);
-        }
-      }
-    }
-    for (int k = threadIdx.x; k < kWarps * tw.W; k += THREADS) s_wcnt[k] = 0;
+    __syncthreads();  // barrier 3: the stage may be overwritten
     if (threadIdx.x == 0 && tnext < ntiles)
       issue_tile(P, cur, S, &bar[it & 1], tnext, dn, VARIANT == 2, VARIANT == 2);
-    __syncthreads();
   }
 
   // side list: far movers and births go to the slots k_mid computed for them
   const unsigned Mv = P.st->ovf_valid;
-  for (unsigned p = blockIdx.x * THREADS + threadIdx.x; p < Mv; p += G * THREADS) {
+  for (unsigned p = blockIdx.x * kThreads + threadIdx.x; p < Mv; p += G * kThreads) {
     const int dst = P.ovf_dst[p];
     const OvfRec rec = P.ovf_rec[P.ovf_idx[p]];
     const int c = (int)(P.ovf_key[p] >> kCellShift);
     nxt.x[dst] = rec.x; nxt.vx[dst] = rec.vx; nxt.vy[dst] = rec.vy; nxt.vz[dst] = rec.vz;
     nxt.cell[dst] = c; nxt.pid[dst] = rec.pid; nxt.sp[dst] = (unsigned char)rec.sp;
-    if (((unsigned)dst & (kTile - 1)) == 0) nxt.desc[dst / kTile].x = c;
-    if (((unsigned)dst & (kTile - 1)) == kTile - 1 || (unsigned)dst == n_next - 1) nxt.desc[dst / kTile].y = c;
     const unsigned Q = (unsigned)s_sp[rec.sp].Q;
     const unsigned a = deposit_a(rec.x, c, P.inv_dx, Q);
     int j1 = c + 1;
@@ -773,71 +841,50 @@ static int sm_count() {
   return g_sms;
 }
 
-// persistent grid: one CTA per SM (or one per tile when there are fewer tiles than SMs)
+// persistent grid: kMinBlocks CTAs per SM (or one per tile when there are fewer tiles than that)
 static int particle_grid(const Params& P) {
-  const int want = sm_count();
+  const int want = sm_count() * kMinBlocks;
   return P.max_tiles < want ? (P.max_tiles > 0 ? P.max_tiles : 1) : want;
 }
 
-template <int THREADS>
-static cudaError_t configure_threads() {
-  typedef PassSmem<THREADS> SM;
-  cudaError_t e;
-  e = cudaFuncSetAttribute(k_pass_a<1, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::a_total);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_pass_a<2, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::a_total);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_pass_b<1, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::b_total);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(k_pass_b<2, THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::b_total);
-}
-
 cudaError_t configure_kernels() {
-  cudaError_t e = configure_threads<512>();
+  typedef PassSmem SM;
+  cudaError_t e;
+  e = cudaFuncSetAttribute(k_pass_a<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::a_total);
   if (e != cudaSuccess) return e;
-  return configure_threads<1024>();
+  e = cudaFuncSetAttribute(k_pass_a<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::a_total);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_pass_b<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::b_total);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(k_pass_b<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::b_total);
 }
 
-template <int THREADS>
-static void launch_passes(const Params& P, const Particles& cur, const Particles& nxt, int variant, cudaStream_t s,
-                          cudaEvent_t* ev) {
-  typedef PassSmem<THREADS> SM;
+int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int variant, cudaStream_t s,
+                cudaEvent_t* ev) {
+  typedef PassSmem SM;
   const int g = particle_grid(P);
   const int gc = (P.max_tiles + (kColThreads / 32) - 1) / (kColThreads / 32);
   if (ev) cudaEventRecord(ev[0], s);
-  if (variant == 2) k_pass_a<2, THREADS><<<g, THREADS, SM::a_total, s>>>(P, cur);
-  else k_pass_a<1, THREADS><<<g, THREADS, SM::a_total, s>>>(P, cur);
+  if (variant == 2) k_pass_a<2><<<g, kThreads, SM::a_total, s>>>(P, cur);
+  else k_pass_a<1><<<g, kThreads, SM::a_total, s>>>(P, cur);
   if (ev) cudaEventRecord(ev[1], s);
   k_mid<<<1, kMidThreads, 0, s>>>(P);
   k_colscan<<<gc < 1 ? 1 : (gc > 16384 ? 16384 : gc), kColThreads, 0, s>>>(P, cur);
   if (ev) cudaEventRecord(ev[2], s);
-  if (variant == 2) k_pass_b<2, THREADS><<<g, THREADS, SM::b_total, s>>>(P, cur, nxt);
-  else k_pass_b<1, THREADS><<<g, THREADS, SM::b_total, s>>>(P, cur, nxt);
+  if (variant == 2) k_pass_b<2><<<g, kThreads, SM::b_total, s>>>(P, cur, nxt);
+  else k_pass_b<1><<<g, kThreads, SM::b_total, s>>>(P, cur, nxt);
   if (ev) cudaEventRecord(ev[3], s);
   k_field<<<1, kFieldThreads, 0, s>>>(P, 1);
   if (ev) cudaEventRecord(ev[4], s);
-}
-
-int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int variant, int threads,
-                cudaStream_t s, cudaEvent_t* ev) {
-  if (threads == 1024) launch_passes<1024>(P, cur, nxt, variant, s, ev);
-  else launch_passes<512>(P, cur, nxt, variant, s, ev);
   return 5;
 }
 
-// load / restart: counts -> cell_start, deposit, field (no push).  cur must be sorted by cell.
+// load / restart: counts -> cell_start, deposit, field (no push).  cur must be sorted by cell.  (The tile
+// descriptors are not part of the state: pass A reads them off the sorted cell array.)
 __global__ void __launch_bounds__(kAuxThreads) k_count_cells(const __grid_constant__ Params P, Particles cur) {
   const unsigned n = P.st->n;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
     atomicAdd(&P.cell_count[cur.cell[i]], 1);
-}
-__global__ void __launch_bounds__(kAuxThreads) k_tile_desc(const __grid_constant__ Params P, Particles cur) {
-  const unsigned n = P.st->n;
-  const unsigned ntiles = (n + kTile - 1) / kTile;
-  for (unsigned t = blockIdx.x * blockDim.x + threadIdx.x; t < ntiles; t += gridDim.x * blockDim.x) {
-    const unsigned last = min(n, (t + 1) * (unsigned)kTile) - 1u;
-    cur.desc[t] = make_int2(cur.cell[(size_t)t * kTile], cur.cell[last]);
-  }
 }
 __global__ void k_clear_grids(const __grid_constant__ Params P) {
   const size_t tot = (size_t)P.ns * (size_t)P.ng;
@@ -853,11 +900,10 @@ int launch_rebuild(const Params& P, const Particles& cur, cudaStream_t s) {
   const int g = sm_count() * 4;
   k_clear_grids<<<g, 256, 0, s>>>(P);
   k_count_cells<<<g, kAuxThreads, 0, s>>>(P, cur);
-  k_tile_desc<<<g, kAuxThreads, 0, s>>>(P, cur);
   k_mid<<<1, kMidThreads, 0, s>>>(P);   // ovf_count == 0: plain scan; n_next = n
   k_deposit<<<g, kAuxThreads, 0, s>>>(P, cur);
   k_field<<<1, kFieldThreads, 0, s>>>(P, 0);  // commits n = n_next, leaves the step counter alone
-  return 6;
+  return 5;
 }
 
 }  // namespace bit1

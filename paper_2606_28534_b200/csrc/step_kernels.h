@@ -5,10 +5,9 @@
 namespace bit1 {
 cudaError_t configure_kernels();
 // one timestep on stream s; returns the number of kernels launched
-// threads: 512 or 1024 threads per CTA of the two particle passes
 // ev: NULL, or 5 events recorded before/between/after the kernels (per-kernel timing; k_mid + k_colscan share one)
-int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int variant, int threads,
-                cudaStream_t s, cudaEvent_t* ev);
-// counts per cell -> cell_start, tile descriptors, deposit, field solve for particles already sorted in cur
+int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int variant, cudaStream_t s,
+                cudaEvent_t* ev);
+// counts per cell -> cell_start, deposit, field solve for particles already sorted in cur
 int launch_rebuild(const Params& P, const Particles& cur, cudaStream_t s);
 }  // namespace bit1
