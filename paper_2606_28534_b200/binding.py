@@ -61,7 +61,7 @@ def load_library(path: Optional[str] = None):
     global _lib
     if _lib is not None and path is None:
         return _lib
-    p = path or LIB_PATH
+    p = path or os.environ.get("BIT1_LIB") or LIB_PATH   # BIT1_LIB: a libbit1.so built with other tile geometry
     if not os.path.exists(p):
         raise RuntimeError(f"{p} not found: build it with `python -m paper_2606_28534_b200.build` "
                            "(there is no CPU fallback)")

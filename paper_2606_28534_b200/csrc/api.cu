@@ -26,6 +26,13 @@ constexpr int kMaxR = 4;
 constexpr size_t kAlign = 256;
 constexpr uint32_t kCkptVersion = 1;
 
+// sort window radius in cells (reading R-win); BIT1_WINDOW_R overrides it for the tests
+inline int window_R() {
+  int R = 1;
+  if (const char* ev = getenv("BIT1_WINDOW_R")) { const int r = atoi(ev); if (r >= 0 && r <= kMaxR) R = r; }
+  return R;
+}
+
 inline size_t align_up(size_t v) { return (v + kAlign - 1) & ~(kAlign - 1); }
 
 struct PartLayout {
@@ -76,7 +83,7 @@ CkptLayout ckpt_layout(int nc, size_t cap) {
 }
 
 struct Layout {
-  size_t st, tables, dens, rho, phi, E, cell_count, cell_start, cell_base, ovf_before, tile_hist, tile_base, evt,
+  size_t st, tables, dens, rho, phi, E, cell_count, cell_start, cell_base, ovf_before, tile_hist, tile_base, tile_pre, evt,
       ovf_key, ovf_idx, ovf_dst, tmp_key, tmp_idx, ovf_rec, part[2], scratch, mom, total;
   unsigned ovf_cap, ovf_pow2;
   int max_tiles, ng;
@@ -104,8 +111,10 @@ Layout make_layout(int nc, int bc, int ns, size_t cap, int staging) {
   l.cell_start = take((size_t)(nc + 1) * 4);
   l.cell_base = take((size_t)nc * 4);
   l.ovf_before = take((size_t)nc * 4);
-  l.tile_hist = take(((size_t)nc + (size_t)(l.max_tiles + 1) * (2 * kMaxR + 1) + kWCap) * 4);
-  l.tile_base = take(((size_t)nc + (size_t)(l.max_tiles + 1) * (2 * kMaxR + 1) + kWCap) * 4);
+  const size_t rw = tile_row_words(nc, l.max_tiles, window_R());
+  l.tile_hist = take(rw * 4);
+  l.tile_base = take(rw * 4);
+  l.tile_pre = take(rw * 4 * kWarps);
   l.evt = take((size_t)(l.max_tiles + 1) * (kTile / 8));
   l.ovf_key = take((size_t)p2 * 8);
   l.tmp_key = take((size_t)p2 * 8);
@@ -236,8 +245,7 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
 
   Params& P = c->P;
   P.nc = g->nc; P.bc = g->bc; P.ng = lay.ng; P.ns = ns;
-  P.R = 1;
-  if (const char* ev = getenv("BIT1_WINDOW_R")) { int r = atoi(ev); if (r >= 0 && r <= kMaxR) P.R = r; }
+  P.R = window_R();
   P.n_sig = o->n_sig; P.n_norm = o->n_norm; P.sp_ep = sp_ep; P.sp_ip = sp_ip;
   P.seed_lo = (unsigned)o->seed; P.seed_hi = (unsigned)(o->seed >> 32);
   P.capacity = (unsigned)o->capacity; P.ovf_cap = lay.ovf_cap; P.ovf_pow2 = lay.ovf_pow2;
@@ -297,6 +305,7 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   P.tile_base = reinterpret_cast<int*>(ws + lay.tile_base);
   P.evt = reinterpret_cast<unsigned*>(ws + lay.evt);
   P.tile_hist = reinterpret_cast<unsigned*>(ws + lay.tile_hist);
+  P.tile_pre = reinterpret_cast<unsigned*>(ws + lay.tile_pre);
   P.ovf_key = reinterpret_cast<unsigned long long*>(ws + lay.ovf_key);
   P.tmp_key = reinterpret_cast<unsigned long long*>(ws + lay.tmp_key);
   P.ovf_idx = reinterpret_cast<unsigned*>(ws + lay.ovf_idx);

@@ -110,8 +110,10 @@ struct Params {
   int *cell_base;   // nc: cell_start + far movers placed before the windowed particles
   int *ovf_before;  // nc
   // tiles
-  unsigned *tile_hist;  // banded histogram rows, row t at clo_t + t*(2R+1)
+  unsigned *tile_hist;  // banded histogram rows: row t (one count per window cell) at tile_row_offset(clo_t, t, R)
   int *tile_base;       // same layout: destination of the tile's first particle of each window cell
+  unsigned *tile_pre;   // row t at kWarps * tile_row_offset: per (window cell, warp of pass A/B) the number of the
+                        // tile's particles for that cell held by earlier warps of the tile
   unsigned *evt;        // one bit per particle slot: pass B must take the slow path (wall hit / MC candidate)
   // overflow list
   unsigned long long *ovf_key;  // ovf_pow2 (unsorted, then sorted in place)
@@ -123,8 +125,13 @@ struct Params {
   SpeciesP sp[kMaxSpecies];
 };
 
+// Rows never overlap: clo is monotone in the tile index and a row holds chi - clo + 1 + 2R <= the distance to the
+// next row's start.  Offsets are multiples of 4 words so that a row can be fetched by a 16-byte bulk copy.
 __host__ __device__ inline size_t tile_row_offset(int clo, int tile, int R) {
-  return (size_t)clo + (size_t)tile * (size_t)(2 * R + 1);
+  return ((size_t)clo + (size_t)tile * (size_t)(2 * R + 4) + 3) & ~(size_t)3;
+}
+__host__ __device__ inline size_t tile_row_words(int nc, int max_tiles, int R) {
+  return (size_t)nc + (size_t)(max_tiles + 1) * (size_t)(2 * R + 4) + (size_t)kWCap + 16;
 }
 
 }  // namespace bit1

@@ -14,6 +14,8 @@ struct __align__(128) Stage {
   unsigned char sp[kTile];
   unsigned evt[kTile / 32];
   double E[kWCap + 4];  // E[e0 .. ], e0 = clo & ~1 (16-byte aligned source)
+  int tb[kWCap];                  // pass B: the tile's row of tile_base
+  unsigned pre[kWCap * kWarps];   // pass B: the tile's row of tile_pre
   int2 d;               // (first, last) old cell of the staged tile; plain store by the issuing thread
 };
 
@@ -59,13 +61,18 @@ __device__ __forceinline__ bool e_window(int clo, int chi, int& e0, int& ne) {
 // One elected thread: arm the stage's barrier and issue the copies of tile `tile` (always whole tiles: the
 // arrays are padded to a multiple of kTile, the tail of the last tile is never used).
 __device__ __forceinline__ void issue_tile(const Params& P, const Particles& cur, Stage* st, unsigned long long* bar,
-                                           int tile, int2 d, bool with_evt, bool with_E) {
+                                           int tile, int2 d, bool with_evt, bool with_E, bool with_rank) {
   const size_t base = (size_t)tile * kTile;
   int e0 = 0, ne = 0;
   const bool stage_E = with_E && e_window(d.x, d.y, e0, ne);
   unsigned bytes = 4u * kTile * 8u + 2u * kTile * 4u + kTile;
   if (with_evt) bytes += kTile / 8;
   if (stage_E) bytes += (unsigned)ne * 8u;
+  // window of the tile, rounded up to whole 16-byte units (the rows are padded, see tile_row_offset)
+  int w = d.y - d.x + 1 + 2 * P.R;
+  w = ((w < kWCap ? w : kWCap) + 3) & ~3;
+  const size_t row = tile_row_offset(d.x, tile, P.R);
+  if (with_rank) bytes += (unsigned)w * 4u * (1u + (unsigned)kWarps);
   st->d = d;
   mbar_expect_tx(bar, bytes);
   bulk_g2s(st->x, cur.x + base, kTile * 8, bar);
@@ -77,6 +84,10 @@ __device__ __forceinline__ void issue_tile(const Params& P, const Particles& cur
   bulk_g2s(st->sp, cur.sp + base, kTile, bar);
   if (with_evt) bulk_g2s(st->evt, P.evt + base / 32, kTile / 8, bar);
   if (stage_E) bulk_g2s(st->E, P.E + e0, (unsigned)ne * 8u, bar);
+  if (with_rank) {
+    bulk_g2s(st->tb, P.tile_base + row, (unsigned)w * 4u, bar);
+    bulk_g2s(st->pre, P.tile_pre + row * kWarps, (unsigned)w * 4u * (unsigned)kWarps, bar);
+  }
 }
 
 }  // namespace bit1

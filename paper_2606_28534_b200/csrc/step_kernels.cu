@@ -34,20 +34,18 @@ __device__ __forceinline__ void load_species(const Params& P, SpeciesP* s_sp) {
 }
 
 constexpr int kAuxThreads = 256;
-constexpr unsigned kCollMask = kElastic | kIonise | kCx;
 
 // dynamic shared memory of both passes: [2 x Stage][pass-specific arrays][species][2 barriers]
+constexpr int kDensWords = (kWCap + 1) * kMaxSpecies;
 struct PassSmem {
   static constexpr size_t stages = 2 * sizeof(Stage);
-  static constexpr size_t a_hist = stages;                                  // unsigned[2][kWCap]
-  static constexpr size_t a_sp = a_hist + 2 * kWCap * 4;                    // SpeciesP[kMaxSpecies]
+  static constexpr size_t a_hist = stages;                                  // unsigned[2][kWCap][kWarps]
+  static constexpr size_t a_sp = a_hist + 2 * (size_t)kWCap * kWarps * 4;   // SpeciesP[kMaxSpecies]
   static constexpr size_t a_bar = (a_sp + kMaxSpecies * sizeof(SpeciesP) + 15) & ~(size_t)15;  // 2 x u64
   static constexpr size_t a_total = a_bar + 16;
-  static constexpr size_t b_wcnt = stages;                                  // unsigned[kWCap][kWarps]
-  static constexpr size_t b_base = b_wcnt + (size_t)kWCap * kWarps * 4;     // unsigned[kWCap][kWarps]
-  static constexpr size_t b_tb = b_base + (size_t)kWCap * kWarps * 4;       // int[kWCap]
-  static constexpr size_t b_dens = b_tb + (size_t)kWCap * 4;                // unsigned[kWCap + 1][kMaxSpecies]
-  static constexpr size_t b_sp = b_dens + (size_t)(kWCap + 1) * kMaxSpecies * 4 + 32;
+  static constexpr size_t b_wc = stages;                                    // unsigned[kWarps][kWCap]
+  static constexpr size_t b_dens = b_wc + (size_t)kWCap * kWarps * 4;       // unsigned[2][kWCap + 1][kMaxSpecies]
+  static constexpr size_t b_sp = b_dens + 2 * (size_t)kDensWords * 4;
   static constexpr size_t b_bar = (b_sp + kMaxSpecies * sizeof(SpeciesP) + 15) & ~(size_t)15;
   static constexpr size_t b_total = b_bar + 16;
 };
@@ -94,11 +92,11 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
     fence_proxy_async();
     for (int k = 0; k < 2; ++k) {
       const int t = blockIdx.x + k * G;
-      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, tile_cells(cur, t, n), false, true);
+      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, tile_cells(cur, t, n), false, true, false);
     }
   }
   load_species(P, s_sp);
-  for (int k = threadIdx.x; k < 2 * kWCap; k += kThreads) s_hist2[k] = 0;
+  for (int k = threadIdx.x; k < 2 * kWCap * kWarps; k += kThreads) s_hist2[k] = 0;
   // the deposition of this step accumulates into dens: clear it here (nobody reads it during pass A)
   {
     const size_t tot = (size_t)P.ns * (size_t)P.ng;
@@ -109,7 +107,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
   int it = 0;
   for (int tile = blockIdx.x; tile < ntiles; tile += G, ++it) {
     Stage* S = &stg[it & 1];
-    unsigned* s_hist = s_hist2 + (it & 1) * kWCap;
+    unsigned* s_hist = s_hist2 + (it & 1) * (kWCap * kWarps);   // [window cell][warp]
     const unsigned base = (unsigned)tile * kTile;
     const unsigned cnt = min((unsigned)kTile, n - base);
     // cells of the tile after next (its load is issued at the end of this iteration)
@@ -194,19 +192,29 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
         if (lane == 0) P.evt[(base >> 5) + (unsigned)(warp * kItems + r)] = eb;
       }
       const unsigned m = __match_any_sync(0xffffffffu, key);
-      if (!(key & 0x80000000u) && lane == __ffs(m) - 1) atomicAdd(&s_hist[key], (unsigned)__popc(m));
+      if (!(key & 0x80000000u) && lane == __ffs(m) - 1) s_hist[key * kWarps + warp] += (unsigned)__popc(m);
+      __syncwarp();
     }
     fence_proxy_async();
     __syncthreads();
-    unsigned* row = P.tile_hist + tile_row_offset(clo, tile, P.R);
+    // per window cell: the warps' counts become exclusive prefixes (tile_pre, read back by pass B: this warp's
+    // particles for that cell start that far into the tile's run), their sum is the tile's count
+    const size_t rowo = tile_row_offset(clo, tile, P.R);
     for (int k = threadIdx.x; k < tw.W; k += kThreads) {
-      const unsigned h = s_hist[k];
-      s_hist[k] = 0;
-      row[k] = h;
+      unsigned run = 0;
+      unsigned* pre = P.tile_pre + (rowo + (size_t)k) * kWarps;
+#pragma unroll
+      for (int w = 0; w < kWarps; ++w) {
+        const unsigned t = s_hist[k * kWarps + w];
+        s_hist[k * kWarps + w] = 0;
+        pre[w] = run;
+        run += t;
+      }
+      P.tile_hist[rowo + k] = run;
       const int c = tw.wlo + k;
-      if (h && c >= 0 && c < P.nc) atomicAdd(&P.cell_count[c], (int)h);
+      if (run && c >= 0 && c < P.nc) atomicAdd(&P.cell_count[c], (int)run);
     }
-    if (threadIdx.x == 0 && tnext < ntiles) issue_tile(P, cur, S, &bar[it & 1], tnext, dn, false, true);
+    if (threadIdx.x == 0 && tnext < ntiles) issue_tile(P, cur, S, &bar[it & 1], tnext, dn, false, true, false);
   }
 }
 
@@ -445,10 +453,12 @@ __global__ void __launch_bounds__(kColThreads) k_colscan(const __grid_constant__
 }
 
 // ---------------------------------------------------------------------------------------------
-// Pass B.  Per tile: phase 1 recomputes the push (V2) as straight-line arithmetic, phase 1b redoes the particles
-// pass A flagged through the full advance(), phase 2 ranks the particles inside (warp, new cell) and deposits;
-// after barrier 1 a segmented warp scan turns the per-warp counts into destinations while the other threads
-// flush the tile's deposit; after barrier 2 the scatter; barrier 3 frees the stage for the next load.
+// Pass B.  A tile arrives with its particles, its window of E, its row of tile_base (destination of the tile's
+// first particle of every window cell, from k_colscan) and its row of tile_pre (how many of those belong to
+// earlier warps, from pass A).  So every warp knows where its own particles of each cell start and works alone:
+// phase 1 recomputes the push (V2) as straight-line arithmetic, phase 1b redoes the particles pass A flagged
+// through the full advance(), phase 2 ranks inside (warp, cell), deposits and scatters.  One CTA barrier per
+// tile (it frees the stage); the tile's deposit is double-buffered and flushed after it.
 template <int VARIANT>
 __global__ void __launch_bounds__(kThreads, kMinBlocks)
 k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
@@ -456,10 +466,8 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
   typedef PassSmem SM;
   extern __shared__ __align__(128) unsigned char smem[];
   Stage* stg = reinterpret_cast<Stage*>(smem);
-  unsigned* s_wcnt = reinterpret_cast<unsigned*>(smem + SM::b_wcnt);   // [kWCap][kWarps] counts, zero between tiles
-  unsigned* s_base = reinterpret_cast<unsigned*>(smem + SM::b_base);   // [kWCap][kWarps] destinations
-  int* s_tb = reinterpret_cast<int*>(smem + SM::b_tb);                 // [kWCap] this tile's row of tile_base
-  unsigned* s_dens = reinterpret_cast<unsigned*>(smem + SM::b_dens);   // [kWCap + 1][ns]
+  unsigned* s_wc = reinterpret_cast<unsigned*>(smem + SM::b_wc);        // [kWarps][kWCap] next destination
+  unsigned* s_dens2 = reinterpret_cast<unsigned*>(smem + SM::b_dens);   // [2][kWCap + 1][ns]
   SpeciesP* s_sp = reinterpret_cast<SpeciesP*>(smem + SM::b_sp);
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem + SM::b_bar);
 
@@ -470,6 +478,7 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
   const int ntiles = (int)((n + kTile - 1) / kTile);
   const int G = gridDim.x;
   const int ns = P.ns;
+  unsigned* wc = s_wc + warp * kWCap;
 
   if (threadIdx.x == 0) {
     mbar_init(&bar[0], 1);
@@ -478,17 +487,17 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     fence_proxy_async();
     for (int k = 0; k < 2; ++k) {
       const int t = blockIdx.x + k * G;
-      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, cur.desc[t], VARIANT == 2, VARIANT == 2);
+      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, cur.desc[t], VARIANT == 2, VARIANT == 2, true);
     }
   }
   load_species(P, s_sp);
-  for (int k = threadIdx.x; k < kWCap * kWarps; k += kThreads) s_wcnt[k] = 0;
-  for (int k = threadIdx.x; k < (kWCap + 1) * kMaxSpecies; k += kThreads) s_dens[k] = 0;
+  for (int k = threadIdx.x; k < 2 * kDensWords; k += kThreads) s_dens2[k] = 0;
   __syncthreads();
 
   int it = 0;
   for (int tile = blockIdx.x; tile < ntiles; tile += G, ++it) {
     Stage* S = &stg[it & 1];
+    unsigned* s_dens = s_dens2 + (it & 1) * kDensWords;
     const unsigned base = (unsigned)tile * kTile;
     const unsigned cnt = min((unsigned)kTile, n - base);
     const int2 d = S->d;
@@ -496,10 +505,11 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     int2 dn = make_int2(0, 0);
     const int tnext = tile + 2 * G;
     if (threadIdx.x == 0 && tnext < ntiles) dn = cur.desc[tnext];
-    // destination bases of this tile's window (consumed after barrier 1: the load stays in flight meanwhile)
-    int mybase = 0;
-    if ((int)threadIdx.x < tw.W) mybase = P.tile_base[tile_row_offset(d.x, tile, P.R) + threadIdx.x];
     mbar_wait(&bar[it & 1], (unsigned)(it >> 1) & 1u);
+
+    // destination of this warp's first particle of every window cell
+    for (int k = lane; k < tw.W; k += 32) wc[k] = (unsigned)S->tb[k] + S->pre[k * kWarps + warp];
+    __syncwarp();
 
     int e0, ne;
     const double* Eptr = e_window(d.x, d.y, e0, ne) ? (S->E - e0) : P.E;
@@ -536,96 +546,62 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
         }
       }
     }
-    // phase 2: stable rank inside (warp, cell), per-warp counts, deposit
-    unsigned rank[kItems];
+    // phase 2: stable rank inside (warp, cell) -> destination; deposit; scatter
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
-      const unsigned mk = key[r] >= 0 ? (unsigned)key[r] : (0x80000000u | (unsigned)lane);
+      const int off = warp * kWarpSpan + r * 32 + lane;
+      const bool valid = key[r] >= 0;
+      const int sp = valid ? (int)S->sp[off] : 0;
+      const unsigned mk = valid ? (unsigned)key[r] : (0x80000000u | (unsigned)lane);
       const unsigned m = __match_any_sync(0xffffffffu, mk);
       const int leader = __ffs(m) - 1;
       unsigned old = 0;
-      if (key[r] >= 0 && lane == leader) {
-        old = s_wcnt[key[r] * kWarps + warp];
-        s_wcnt[key[r] * kWarps + warp] = old + (unsigned)__popc(m);
+      if (valid && lane == leader) {
+        old = wc[key[r]];
+        wc[key[r]] = old + (unsigned)__popc(m);
       }
       old = __shfl_sync(0xffffffffu, old, leader);
-      rank[r] = old + (unsigned)__popc(m & lt);
+      const unsigned dst = old + (unsigned)__popc(m & lt);
       // deposit (SURVEY 8(c) "D"): one shared-memory atomic pair per (cell, species) run of the warp
-      if (key[r] >= 0) {
-        const int off = warp * kWarpSpan + r * 32 + lane;
-        const int sp = (int)S->sp[off];
-        const unsigned Q = (unsigned)s_sp[sp].Q;
-        const unsigned a = deposit_a(x[r], tw.wlo + key[r], P.inv_dx, Q);
-        if (P.dep_u32) {
-          // Q < 2^21 here: sum of a over a warp < 2^26, the count (<= 32) rides in bits 26..31
-          for (int s = 0; s < ns; ++s) {
-            const unsigned packed = __reduce_add_sync(m, sp == s ? (a + (1u << 26)) : 0u);
-            if (lane == leader && packed) {
-              const unsigned num = packed >> 26, sa = packed & ((1u << 26) - 1u);
-              atomicAdd(&s_dens[key[r] * ns + s], num * (unsigned)s_sp[s].Q - sa);
-              atomicAdd(&s_dens[(key[r] + 1) * ns + s], sa);
-            }
-          }
-        } else {
-          const int c = tw.wlo + key[r];
-          int j1 = c + 1;
-          if (!P.bc && j1 == P.nc) j1 = 0;
-          atomicAdd((unsigned long long*)&P.dens[(size_t)sp * P.ng + c], (unsigned long long)(Q - a));
-          atomicAdd((unsigned long long*)&P.dens[(size_t)sp * P.ng + j1], (unsigned long long)a);
+      const unsigned Q = (unsigned)s_sp[sp].Q;
+      const unsigned a = valid ? deposit_a(x[r], tw.wlo + key[r], P.inv_dx, Q) : 0u;
+      if (P.dep_u32) {
+        // Q < 2^21: the sum of a over a warp stays below 2^26
+        const unsigned m2 = __match_any_sync(0xffffffffu, valid ? (mk << 3) | (unsigned)sp : mk);
+        const unsigned sa = __reduce_add_sync(m2, a);
+        if (valid && lane == __ffs(m2) - 1) {
+          atomicAdd(&s_dens[key[r] * ns + sp], (unsigned)__popc(m2) * Q - sa);
+          atomicAdd(&s_dens[(key[r] + 1) * ns + sp], sa);
         }
+      } else if (valid) {
+        const int c = tw.wlo + key[r];
+        int j1 = c + 1;
+        if (!P.bc && j1 == P.nc) j1 = 0;
+        atomicAdd((unsigned long long*)&P.dens[(size_t)sp * P.ng + c], (unsigned long long)(Q - a));
+        atomicAdd((unsigned long long*)&P.dens[(size_t)sp * P.ng + j1], (unsigned long long)a);
+      }
+      if (valid) {
+        nxt.x[dst] = x[r]; nxt.vx[dst] = vx[r]; nxt.vy[dst] = vy[r]; nxt.vz[dst] = vz[r];
+        nxt.cell[dst] = tw.wlo + key[r]; nxt.pid[dst] = S->pid[off]; nxt.sp[dst] = (unsigned char)sp;
       }
       __syncwarp();
     }
-    if ((int)threadIdx.x < tw.W) s_tb[threadIdx.x] = mybase;
-    __syncthreads();  // barrier 1
-    // per cell, exclusive scan over the warps of the tile (groups of kWarps lanes) -> destination of each
-    // (cell, warp) run; the counts are zeroed for the next tile on the way
-    {
-      const int tot = tw.W * kWarps;
-      for (int b0 = warp * 32; b0 < tot; b0 += kThreads) {
-        const int idx = b0 + lane;
-        const unsigned v = idx < tot ? s_wcnt[idx] : 0u;
-        unsigned inc = v;
-#pragma unroll
-        for (int dd = 1; dd < (kWarps < 32 ? kWarps : 32); dd <<= 1) {
-          const unsigned t = __shfl_up_sync(0xffffffffu, inc, dd, kWarps < 32 ? kWarps : 32);
-          if ((lane & (kWarps - 1)) >= dd) inc += t;
-        }
-        if (idx < tot) {
-          s_wcnt[idx] = 0;
-          s_base[idx] = (unsigned)s_tb[idx / kWarps] + (inc - v);
-        }
-      }
-      // flush the tile's deposit
-      if (P.dep_u32) {
-        for (int k = threadIdx.x; k < ns * (tw.W + 1); k += kThreads) {
-          const unsigned v = s_dens[k];
-          if (v) {
-            s_dens[k] = 0;
-            const int kk = k / ns, s = k - kk * ns;
-            int j = tw.wlo + kk;
-            if (!P.bc && j == P.nc) j = 0;
-            atomicAdd((unsigned long long*)&P.dens[(size_t)s * P.ng + j], (unsigned long long)v);
-          }
-        }
-      }
-    }
-    __syncthreads();  // barrier 2
-
-    // phase 3: scatter (pid and species are read again from the stage)
-#pragma unroll
-    for (int r = 0; r < kItems; ++r) {
-      if (key[r] >= 0) {
-        const int off = warp * kWarpSpan + r * 32 + lane;
-        const unsigned dst = s_base[key[r] * kWarps + warp] + rank[r];
-        nxt.x[dst] = x[r]; nxt.vx[dst] = vx[r]; nxt.vy[dst] = vy[r]; nxt.vz[dst] = vz[r];
-        nxt.cell[dst] = tw.wlo + key[r]; nxt.pid[dst] = S->pid[off]; nxt.sp[dst] = S->sp[off];
-      }
-    }
     fence_proxy_async();
-    __syncthreads();  // barrier 3: the stage may be overwritten
+    __syncthreads();  // the stage may be overwritten; the tile's deposit is complete
     if (threadIdx.x == 0 && tnext < ntiles)
-      issue_tile(P, cur, S, &bar[it & 1], tnext, dn, VARIANT == 2, VARIANT == 2);
+      issue_tile(P, cur, S, &bar[it & 1], tnext, dn, VARIANT == 2, VARIANT == 2, true);
+    if (P.dep_u32) {
+      for (int k = threadIdx.x; k < ns * (tw.W + 1); k += kThreads) {
+        const unsigned v = s_dens[k];
+        if (v) {
+          s_dens[k] = 0;
+          const int kk = k / ns, s = k - kk * ns;
+          int j = tw.wlo + kk;
+          if (!P.bc && j == P.nc) j = 0;
+          atomicAdd((unsigned long long*)&P.dens[(size_t)s * P.ng + j], (unsigned long long)v);
+        }
+      }
+    }
   }
 
   // side list: far movers and births go to the slots k_mid computed for them
