@@ -83,7 +83,7 @@ CkptLayout ckpt_layout(int nc, size_t cap) {
 }
 
 struct Layout {
-  size_t st, tables, dens, rho, phi, E, cell_count, cell_start, cell_base, ovf_before, tile_hist, tile_base, tile_pre, evt,
+  size_t st, tables, dens, rho, phi, E, cell_count, cell_start, cell_start_old, scan_part, coop_scratch, cell_base, ovf_before, tile_hist, tile_base, tile_pre, evt,
       ovf_key, ovf_idx, ovf_dst, tmp_key, tmp_idx, ovf_rec, part[2], scratch, mom, total;
   unsigned ovf_cap, ovf_pow2;
   int max_tiles, ng;
@@ -109,6 +109,9 @@ Layout make_layout(int nc, int bc, int ns, size_t cap, int staging) {
   l.E = take((size_t)(nc + 4) * 8);  // the E window of a tile is copied in 16-byte units
   l.cell_count = take((size_t)nc * 4);
   l.cell_start = take((size_t)(nc + 1) * 4);
+  l.cell_start_old = take((size_t)(nc + 1) * 4);
+  l.scan_part = take(1024 * 4);
+  l.coop_scratch = take(4 * 1024 * 16);
   l.cell_base = take((size_t)nc * 4);
   l.ovf_before = take((size_t)nc * 4);
   const size_t rw = tile_row_words(nc, l.max_tiles, window_R());
@@ -300,6 +303,9 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   P.E = reinterpret_cast<double*>(ws + lay.E);
   P.cell_count = reinterpret_cast<int*>(ws + lay.cell_count);
   P.cell_start = reinterpret_cast<int*>(ws + lay.cell_start);
+  P.cell_start_old = reinterpret_cast<int*>(ws + lay.cell_start_old);
+  P.scan_part = reinterpret_cast<int*>(ws + lay.scan_part);
+  P.coop_scratch = ws + lay.coop_scratch;
   P.cell_base = reinterpret_cast<int*>(ws + lay.cell_base);
   P.ovf_before = reinterpret_cast<int*>(ws + lay.ovf_before);
   P.tile_base = reinterpret_cast<int*>(ws + lay.tile_base);
@@ -438,6 +444,8 @@ bit1_status bit1_step(bit1_ctx* c, uint64_t nsteps) {
       ev = &c->prof_ev[c->prof_steps * 5];
       c->prof_steps++;
     }
+    // the arrangement the last step (or load / restart) produced is this step's input
+    { int* t = c->P.cell_start; c->P.cell_start = c->P.cell_start_old; c->P.cell_start_old = t; }
     c->launches += launch_step(c->P, c->buf[c->cur], c->buf[c->cur ^ 1], c->variant, c->cs, ev);
     c->cur ^= 1;
   }

@@ -106,7 +106,10 @@ struct Params {
   long long *rho;   // ng
   double *phi, *E;  // nc + 1
   int *cell_count;  // nc
-  int *cell_start;  // nc + 1
+  int *cell_start;  // nc + 1: of the arrangement this step produces (k_mid)
+  int *cell_start_old;  // nc + 1: of the arrangement this step reads (swapped with cell_start every step)
+  int *scan_part;   // one partial sum per CTA of k_mid
+  void *coop_scratch;  // k_field: per-CTA partial sums (16-byte aligned)
   int *cell_base;   // nc: cell_start + far movers placed before the windowed particles
   int *ovf_before;  // nc
   // tiles

@@ -1,15 +1,19 @@
 // The kernels of one timestep:
 //   k_pass_a   mover: advance every particle, banded per-tile histogram of new cells, event bits, side list of
 //              far movers and births                               (PAPER.md:111 move0/moveb)
-//   k_mid      order the side list, counts -> cell_start           (row a4, scan part)
-//   k_colscan  banded column scan: destination base of every (tile, window cell)
+//   k_mid      order the side list, counts -> cell_start, banded column scan: destination base of every
+//              (tile, window cell)                                  (row a4, scan part)
 //   k_pass_b   arranger: stable ranks inside the tile, scatter to the sorted position with the charge
 //              deposition fused                                    (rows a4-a5; PAPER.md:111 arrj/narrj)
 //   k_field    exact integer-scan Poisson solve -> phi, E          (row a6; PAPER.md:33 step (iii))
 // Both particle passes are persistent (kMinBlocks CTAs per SM) and read their tiles through the two-stage
 // bulk-async pipeline of pipeline.cuh.
+#include <cooperative_groups.h>
+
 #include "advance.cuh"
 #include "step_kernels.h"
+
+namespace cg = cooperative_groups;
 
 namespace bit1 {
 
@@ -117,7 +121,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
     mbar_wait(&bar[it & 1], (unsigned)(it >> 1) & 1u);
 
     const int clo = S->d.x, chi = S->d.y;
-    if (threadIdx.x == 0) cur.desc[tile] = S->d;   // read by k_colscan and by pass B's issuing thread
+    if (threadIdx.x == 0) cur.desc[tile] = S->d;   // read by k_mid's column scan and by pass B's issuing thread
     const TileWin tw = make_window(clo, chi, P.R);
     int e0, ne;
     const double* Eptr = e_window(clo, chi, e0, ne) ? (S->E - e0) : P.E;
@@ -300,161 +304,209 @@ __device__ int block_exclusive_scan_int(int v, int* s_warp, int* total) {
   return res;
 }
 
-__global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Params P) {
+// block-wide sum of one int per thread (every thread gets it)
+__device__ int block_sum_int(int v, int* s_warp) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  if (lane == 0) s_warp[warp] = v;
+  __syncthreads();
+  int t = 0;
+  if (warp == 0) {
+    t = lane < (int)(blockDim.x >> 5) ? s_warp[lane] : 0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if (lane == 0) s_warp[32] = t;
+  }
+  __syncthreads();
+  t = s_warp[32];
+  __syncthreads();
+  return t;
+}
+
+// k_mid: cooperative launch, one CTA per SM at most.
+//   phase 0 (CTA 0)  side list: births get their pids, the list is ordered by (cell, class, order), every group
+//                    joins its cell's count
+//   phase 1          exclusive scan of the cell counts over all CTAs -> cell_start, cell_base; counts zeroed
+//   phase 2          destinations of the side-list entries; banded column scan (do_colscan): one thread per cell
+//                    walks, in tile order, the tiles whose window holds the cell and hands each its destination
+//                    base = cell_base[c] + what the earlier tiles send to c.  Those tiles are the ones that hold
+//                    old cells c-R .. c+R, found from the previous step's cell_start.
+__global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Params P, Particles cur, int do_colscan) {
   __shared__ unsigned long long s_key[kSortSmem];
   __shared__ unsigned s_val[kSortSmem];
   __shared__ int s_warp[33];
   __shared__ unsigned s_cnt;
+  cg::grid_group grid = cg::this_grid();
   DevState* st = P.st;
   const unsigned n = st->n;
+  const int G = gridDim.x, b = blockIdx.x;
   unsigned M = st->ovf_count;
   if (M > P.ovf_cap) M = P.ovf_cap;
-  const unsigned P2 = next_pow2(M > 1 ? M : 1);
-  unsigned Mv = 0;
 
-  if (M > 0) {
-    // (a) births: order by (parent index, kind), assign pid = next_pid + r, drop those beyond capacity
-    unsigned nb_local = 0;
-    for (unsigned i = threadIdx.x; i < P2; i += blockDim.x) {
-      unsigned long long bk = kInvalidKey;
-      if (i < M) {
-        const unsigned long long key = P.ovf_key[i];
-        if (((key >> kClsShift) & 3ull) == 2ull) { bk = key & ((1ull << kOrdBits) - 1ull); nb_local++; }
+  if (b == 0) {
+    const unsigned P2 = next_pow2(M > 1 ? M : 1);
+    unsigned Mv = 0;
+    if (M > 0) {
+      // (a) births: order by (parent index, kind), assign pid = next_pid + r, drop those beyond capacity
+      unsigned nb_local = 0;
+      for (unsigned i = threadIdx.x; i < P2; i += blockDim.x) {
+        unsigned long long bk = kInvalidKey;
+        if (i < M) {
+          const unsigned long long key = P.ovf_key[i];
+          if (((key >> kClsShift) & 3ull) == 2ull) { bk = key & ((1ull << kOrdBits) - 1ull); nb_local++; }
+        }
+        P.tmp_key[i] = bk;
+        P.tmp_idx[i] = i;
       }
-      P.tmp_key[i] = bk;
-      P.tmp_idx[i] = i;
-    }
-    if (threadIdx.x == 0) s_cnt = 0;
-    __syncthreads();
-    if (nb_local) atomicAdd(&s_cnt, nb_local);
-    __syncthreads();
-    const unsigned B = s_cnt;
-    __syncthreads();
-    if (B > 0) {
-      cta_sort(P.tmp_key, P.tmp_idx, P2, s_key, s_val);
-      const unsigned room = P.capacity > n ? P.capacity - n : 0u;
-      const unsigned next_pid = st->next_pid;
-      for (unsigned r = threadIdx.x; r < B; r += blockDim.x) {
-        const unsigned rec = P.tmp_idx[r];
-        if (r < room) P.ovf_rec[rec].pid = next_pid + r;
-        else P.ovf_key[rec] = kInvalidKey;
+      if (threadIdx.x == 0) s_cnt = 0;
+      __syncthreads();
+      if (nb_local) atomicAdd(&s_cnt, nb_local);
+      __syncthreads();
+      const unsigned B = s_cnt;
+      __syncthreads();
+      if (B > 0) {
+        cta_sort(P.tmp_key, P.tmp_idx, P2, s_key, s_val);
+        const unsigned room = P.capacity > n ? P.capacity - n : 0u;
+        const unsigned next_pid = st->next_pid;
+        for (unsigned r = threadIdx.x; r < B; r += blockDim.x) {
+          const unsigned rec = P.tmp_idx[r];
+          if (r < room) P.ovf_rec[rec].pid = next_pid + r;
+          else P.ovf_key[rec] = kInvalidKey;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+          const unsigned created = B < room ? B : room;
+          st->next_pid = next_pid + created;
+          st->births += created;
+          if (B > room) st->flags |= kFlagCapacity;
+        }
+      }
+      // (b) order the whole list by (cell, class, order)
+      for (unsigned i = threadIdx.x; i < P2; i += blockDim.x) {
+        if (i >= M) P.ovf_key[i] = kInvalidKey;
+        P.ovf_idx[i] = i;
       }
       __syncthreads();
-      if (threadIdx.x == 0) {
-        const unsigned created = B < room ? B : room;
-        st->next_pid = next_pid + created;
-        st->births += created;
-        if (B > room) st->flags |= kFlagCapacity;
+      cta_sort(P.ovf_key, P.ovf_idx, P2, s_key, s_val);
+      Mv = lower_bound_u64(P.ovf_key, P2, kInvalidKey);
+      // (c) groups per cell: rank inside the group, group size joins the cell count
+      for (unsigned p = threadIdx.x; p < Mv; p += blockDim.x) {
+        const unsigned long long key = P.ovf_key[p];
+        const unsigned long long c = key >> kCellShift;
+        const unsigned lb = lower_bound_u64(P.ovf_key, Mv, c << kCellShift);
+        const unsigned ub = lower_bound_u64(P.ovf_key, Mv, (c + 1ull) << kCellShift);
+        const unsigned cls = (unsigned)((key >> kClsShift) & 3ull);
+        if (p == lb) {
+          const unsigned ub0 = lower_bound_u64(P.ovf_key, Mv, (c << kCellShift) | (1ull << kClsShift));
+          P.cell_count[c] += (int)(ub - lb);
+          P.ovf_before[c] = (int)(ub0 - lb);
+        }
+        // class 0 counts from the cell's start, classes 1-2 from the cell's end
+        P.ovf_dst[p] = cls == 0 ? (int)(p - lb) : (int)(p - lb) - (int)(ub - lb);
       }
     }
-    // (b) order the whole list by (cell, class, order)
-    for (unsigned i = threadIdx.x; i < P2; i += blockDim.x) {
-      if (i >= M) P.ovf_key[i] = kInvalidKey;
-      P.ovf_idx[i] = i;
+    if (threadIdx.x == 0) {
+      st->ovf_valid = Mv;
+      st->far_movers += M;
+      if (M > st->max_far_movers) st->max_far_movers = M;
     }
-    __syncthreads();
-    cta_sort(P.ovf_key, P.ovf_idx, P2, s_key, s_val);
-    Mv = lower_bound_u64(P.ovf_key, P2, kInvalidKey);
-    // (d) groups per cell: rank inside the group, group size joins the cell count
-    for (unsigned p = threadIdx.x; p < Mv; p += blockDim.x) {
-      const unsigned long long key = P.ovf_key[p];
-      const unsigned long long c = key >> kCellShift;
-      const unsigned lb = lower_bound_u64(P.ovf_key, Mv, c << kCellShift);
-      const unsigned ub = lower_bound_u64(P.ovf_key, Mv, (c + 1ull) << kCellShift);
-      const unsigned cls = (unsigned)((key >> kClsShift) & 3ull);
-      if (p == lb) {
-        const unsigned ub0 = lower_bound_u64(P.ovf_key, Mv, (c << kCellShift) | (1ull << kClsShift));
-        P.cell_count[c] += (int)(ub - lb);
-        P.ovf_before[c] = (int)(ub0 - lb);
-      }
-      // class 0 counts from the cell's start, classes 1-2 from the cell's end
-      P.ovf_dst[p] = cls == 0 ? (int)(p - lb) : (int)(p - lb) - (int)(ub - lb);
-    }
-    __syncthreads();
   }
+  __threadfence();
+  grid.sync();
 
-  // (e) exclusive scan of the cell counts
-  int carry = 0;
+  // phase 1: scan of the cell counts.  CTA b owns cells [c_lo, c_hi).
   const int nc = P.nc;
-  for (int c0 = 0; c0 < nc; c0 += kMidThreads * 4) {
+  int per = (nc + G - 1) / G;
+  per = (per + 3) & ~3;
+  const int c_lo = min(b * per, nc), c_hi = min(c_lo + per, nc);
+  {
+    int sum = 0;
+    for (int c = c_lo + (int)threadIdx.x; c < c_hi; c += kMidThreads) sum += P.cell_count[c];
+    sum = block_sum_int(sum, s_warp);
+    if (threadIdx.x == 0) P.scan_part[b] = sum;
+  }
+  __threadfence();
+  grid.sync();
+  int carry, total;
+  {
+    int mine = 0, all = 0;
+    for (int i = threadIdx.x; i < G; i += kMidThreads) {
+      const int v = P.scan_part[i];
+      all += v;
+      if (i < b) mine += v;
+    }
+    carry = block_sum_int(mine, s_warp);
+    total = block_sum_int(all, s_warp);
+  }
+  for (int c0 = c_lo; c0 < c_hi; c0 += kMidThreads * 4) {
     const int c = c0 + (int)threadIdx.x * 4;
-    int v[4], b[4];
+    int v[4], bf[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-      const bool in = c + k < nc;
+      const bool in = c + k < c_hi;
       v[k] = in ? P.cell_count[c + k] : 0;
-      b[k] = in ? P.ovf_before[c + k] : 0;
+      bf[k] = in ? P.ovf_before[c + k] : 0;
     }
     const int tsum = (v[0] + v[1]) + (v[2] + v[3]);
-    int total;
-    int ex = carry + block_exclusive_scan_int(tsum, s_warp, &total);
+    int chunk;
+    int ex = carry + block_exclusive_scan_int(tsum, s_warp, &chunk);
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-      if (c + k < nc) {
+      if (c + k < c_hi) {
         P.cell_start[c + k] = ex;
-        P.cell_base[c + k] = ex + b[k];
+        P.cell_base[c + k] = ex + bf[k];
         P.cell_count[c + k] = 0;
         P.ovf_before[c + k] = 0;
       }
       ex += v[k];
     }
-    carry += total;
+    carry += chunk;
   }
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    P.cell_start[nc] = carry;
-    st->n_next = (unsigned)carry;
-    st->ovf_valid = Mv;
-    st->far_movers += M;
-    if (M > st->max_far_movers) st->max_far_movers = M;
+  if (b == 0 && threadIdx.x == 0) {
+    P.cell_start[nc] = total;
+    st->n_next = (unsigned)total;
   }
-  // (f) destinations of the side-list entries (reads cell_start written above by this CTA)
-  __threadfence_block();
-  __syncthreads();
-  for (unsigned p = threadIdx.x; p < Mv; p += blockDim.x) {
+  __threadfence();
+  grid.sync();
+
+  // phase 2
+  const unsigned Mv = st->ovf_valid;
+  const size_t gtid = (size_t)b * kMidThreads + threadIdx.x, gsz = (size_t)G * kMidThreads;
+  for (size_t p = gtid; p < Mv; p += gsz) {
     const unsigned long long key = P.ovf_key[p];
     const int c = (int)(key >> kCellShift);
     const unsigned cls = (unsigned)((key >> kClsShift) & 3ull);
     const int rel = P.ovf_dst[p];
     P.ovf_dst[p] = (cls == 0 ? P.cell_start[c] : P.cell_start[c + 1]) + rel;
   }
-}
-
-// ---------------------------------------------------------------------------------------------
-// k_colscan: for every tile t and every cell c of its window, the destination of the first particle that tile t
-// sends to c:  cell_base[c] + sum of tile_hist over the earlier tiles whose window holds c.  Windows' lower and
-// upper ends are monotone in t, so those tiles are the contiguous range just before t.  One warp per tile.
-constexpr int kColThreads = 256;
-
-__global__ void __launch_bounds__(kColThreads) k_colscan(const __grid_constant__ Params P, Particles cur) {
-  const unsigned n = P.st->n;
-  const int ntiles = (int)((n + kTile - 1) / kTile);
-  const int lane = threadIdx.x & 31;
-  const int wpb = kColThreads / 32;
-  for (int tile = blockIdx.x * wpb + (threadIdx.x >> 5); tile < ntiles; tile += gridDim.x * wpb) {
-    const int2 d = cur.desc[tile];
-    const TileWin tw = make_window(d.x, d.y, P.R);
-    int* out = P.tile_base + tile_row_offset(d.x, tile, P.R);
-    for (int k = lane; k < tw.W; k += 32) {
-      const int c = tw.wlo + k;
-      int pre = 0;
-      if (c >= 0 && c < P.nc) {
-        pre = P.cell_base[c];
-        for (int t = tile - 1; t >= 0; --t) {
-          const int2 dd = cur.desc[t];
-          const TileWin w2 = make_window(dd.x, dd.y, P.R);
-          if (c >= w2.wlo + w2.W) break;  // c >= w2.wlo always holds (wlo is monotone in t)
-          pre += (int)P.tile_hist[tile_row_offset(dd.x, t, P.R) + (size_t)(c - w2.wlo)];
+  if (do_colscan && n > 0) {
+    const int R = P.R;
+    const int* cso = P.cell_start_old;
+    for (size_t cc = gtid; cc < (size_t)nc; cc += gsz) {
+      const int c = (int)cc;
+      const int lo = cso[max(c - R, 0)];              // first old particle with cell >= c - R
+      const int hi = cso[min(c + R + 1, nc)] - 1;     // last old particle with cell <= c + R
+      if (lo >= (int)n || hi < 0) continue;
+      const int t0 = lo / kTile, t1 = hi / kTile;
+      int run = P.cell_base[c];
+      for (int t = t0; t <= t1; ++t) {
+        const int2 d = cur.desc[t];
+        const TileWin tw = make_window(d.x, d.y, R);
+        const int k = c - tw.wlo;
+        if (k >= 0 && k < tw.W) {
+          const size_t off = tile_row_offset(d.x, t, R) + (size_t)k;
+          P.tile_base[off] = run;
+          run += (int)P.tile_hist[off];
         }
       }
-      out[k] = pre;
     }
   }
 }
 
 // ---------------------------------------------------------------------------------------------
 // Pass B.  A tile arrives with its particles, its window of E, its row of tile_base (destination of the tile's
-// first particle of every window cell, from k_colscan) and its row of tile_pre (how many of those belong to
+// first particle of every window cell, from k_mid) and its row of tile_pre (how many of those belong to
 // earlier warps, from pass A).  So every warp knows where its own particles of each cell start and works alone:
 // phase 1 recomputes the push (V2) as straight-line arithmetic, phase 1b redoes the particles pass A flagged
 // through the full advance(), phase 2 ranks inside (warp, cell), deposits and scatters.  One CTA barrier per
@@ -652,8 +704,8 @@ __global__ void __launch_bounds__(kAuxThreads) k_deposit(const __grid_constant__
 
 // ---------------------------------------------------------------------------------------------
 // k_field: rho = sum_s sign_s dens_s; exact double prefix sum -> phi, E.  Single CTA.
-constexpr int kFieldThreads = 1024;
-constexpr int kFieldItems = 8;
+constexpr int kFieldThreads = 256;
+constexpr int kFieldItems = 4;
 typedef __int128 i128;
 
 __device__ __forceinline__ i128 shfl_up_128(i128 v, int d) {
@@ -717,63 +769,45 @@ __device__ i128 block_sum_128(i128 v, i128* s_warp) {
   return t;
 }
 
-__global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__ Params P, int commit_step) {
-  __shared__ i128 s_warp[33];
-  const int nc = P.nc, ng = P.ng, bc = P.bc;
-  DevState* st = P.st;
-  // phase A: rho, total charge, and T_nc = sum_{j=1}^{nc-1} (nc - j) R_j as plain reductions
-  i128 tot = 0, wsum = 0;
-  for (int j = threadIdx.x; j < ng; j += blockDim.x) {
-    long long r = 0;
-    for (int s = 0; s < P.ns; ++s) r += (long long)P.sp[s].sign * P.dens[(size_t)s * ng + j];
-    P.rho[j] = r;
-    tot += (i128)r;
-    if (j >= 1 && j <= nc - 1) wsum += (i128)(nc - j) * (i128)r;
-  }
-  tot = block_sum_128(tot, s_warp);
-  wsum = block_sum_128(wsum, s_warp);
-  if (threadIdx.x == 0) st->rho_total = (long long)tot;
-  const bool frozen = st->freeze_field != 0;
-  if (!frozen) {
-    // periodic: R'_j = nc R_j - tot  =>  T_nc' = nc * wsum - tot * nc (nc - 1) / 2
-    const i128 Tn = bc ? wsum : (i128)nc * wsum - tot * (((i128)nc * (i128)(nc - 1)) / 2);
-    // phase B: S_j = sum_{k=1..j} R_k (S_0 = 0), T_j = sum_{k<j} S_k, chunked over elements j = 1..jmax
-    const int jmax = bc ? nc : nc - 1;
-    i128 carryS = 0, carryT = 0;  // S_{j0-1}, T_{j0} at the chunk's first element j0
-    if (threadIdx.x == 0) {
-      // node 0
-      P.phi[0] = P.Kphi * dbl128((i128)0);
-      if (bc) P.E[0] = P.KE * dbl128(-2 * Tn - 2 * (i128)nc * (i128)P.rho[0]);
+// One pass of CTA b over its elements j in [j_lo, j_hi] (a sub-range of 1..jmax), in chunks of
+// kFieldThreads * kFieldItems.  carryS = S_{j_lo-1}, carryT = T_{j_lo} on entry.  APPLY = false: only the sums
+// (returns A = sum of R_j and C = sum of the local inclusive prefixes, so that T_{j_hi+1} = T_{j_lo} +
+// len * S_{j_lo-1} + C); APPLY = true: writes phi_j and E_j.
+template <bool APPLY>
+__device__ void field_range(const Params& P, int j_lo, int j_hi, i128 tot, i128 Tn, i128 carryS, i128 carryT,
+                            i128* s_warp, i128* outA, i128* outC) {
+  const int nc = P.nc, bc = P.bc;
+  const i128 S0 = carryS;
+  i128 accC = 0;
+  for (int j0 = j_lo; j0 <= j_hi; j0 += kFieldThreads * kFieldItems) {
+    const int jb = j0 + (int)threadIdx.x * kFieldItems;
+    i128 R[kFieldItems], Sl[kFieldItems];
+    i128 run = 0;
+#pragma unroll
+    for (int k = 0; k < kFieldItems; ++k) {
+      const int j = jb + k;
+      i128 r = 0;
+      if (j <= j_hi) r = bc ? (i128)P.rho[j] : (i128)nc * (i128)P.rho[j] - tot;
+      R[k] = r;
+      run += r;
+      Sl[k] = run;  // inclusive local
     }
-    for (int j0 = 1; j0 <= jmax; j0 += kFieldThreads * kFieldItems) {
-      const int jb = j0 + (int)threadIdx.x * kFieldItems;
-      i128 R[kFieldItems], Sl[kFieldItems];
-      i128 run = 0;
+    i128 chunkS;
+    const i128 exS = carryS + block_exclusive_scan_128(run, s_warp, &chunkS);
+    i128 tsumS = 0;
+#pragma unroll
+    for (int k = 0; k < kFieldItems; ++k) {
+      const int j = jb + k;
+      Sl[k] = exS + Sl[k];   // S_j
+      if (j <= j_hi) tsumS += Sl[k];
+    }
+    i128 chunkSS;
+    i128 T = carryT + block_exclusive_scan_128(tsumS, s_warp, &chunkSS);  // T at this thread's first element
+    if (APPLY) {
 #pragma unroll
       for (int k = 0; k < kFieldItems; ++k) {
         const int j = jb + k;
-        i128 r = 0;
-        if (j <= jmax) r = bc ? (i128)P.rho[j] : (i128)nc * (i128)P.rho[j] - tot;
-        R[k] = r;
-        run += r;
-        Sl[k] = run;  // inclusive local
-      }
-      i128 chunkS;
-      const i128 exS = carryS + block_exclusive_scan_128(run, s_warp, &chunkS);
-      // S_j = exS + Sl[k]; thread sum of S over its elements
-      i128 tsumS = 0;
-#pragma unroll
-      for (int k = 0; k < kFieldItems; ++k) {
-        const int j = jb + k;
-        Sl[k] = exS + Sl[k];
-        if (j <= jmax) tsumS += Sl[k];
-      }
-      i128 chunkSS;
-      i128 T = carryT + block_exclusive_scan_128(tsumS, s_warp, &chunkSS);  // T at this thread's first element
-#pragma unroll
-      for (int k = 0; k < kFieldItems; ++k) {
-        const int j = jb + k;
-        if (j <= jmax) {
+        if (j <= j_hi) {
           const i128 Sj = Sl[k], Sm = Sl[k] - R[k];
           P.phi[j] = P.Kphi * dbl128((i128)j * Tn - (i128)nc * T);
           if (bc) {
@@ -785,18 +819,94 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
           T += Sj;
         }
       }
-      carryS += chunkS;
-      carryT += chunkSS;
     }
-    if (!bc && threadIdx.x == 0) {
-      // node 0 of the periodic grid: S_{-1} = S_{nc-1} (= carryS after the loop), S_0 = 0; ghosts at nc
-      P.E[0] = P.KE * dbl128((i128)nc * (carryS + (i128)0) - 2 * Tn);
-      P.E[nc] = P.E[0];
-      P.phi[nc] = P.phi[0];
-    }
+    carryS += chunkS;
+    carryT += chunkSS;
+    accC += chunkSS;
   }
-  __syncthreads();
-  if (threadIdx.x == 0) {
+  if (!APPLY) {
+    // chunkSS sums S_j = S0 + local prefix: take the S0 part out again
+    const int len = j_hi >= j_lo ? j_hi - j_lo + 1 : 0;
+    *outA = carryS - S0;
+    *outC = accC - (i128)len * S0;
+  }
+}
+
+// k_field: cooperative launch.  rho = sum_s sign_s dens_s; exact integer double prefix sum -> phi, E
+// (SURVEY 8(c) "P").  Phase A: rho and the two plain reductions (total charge, T_nc); phase B: every CTA sums its
+// range of elements; phase C: carries from the CTAs before it, then phi and E.
+__global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__ Params P, int commit_step) {
+  __shared__ i128 s_warp[33];
+  cg::grid_group grid = cg::this_grid();
+  const int nc = P.nc, ng = P.ng, bc = P.bc;
+  const int G = gridDim.x, b = blockIdx.x;
+  DevState* st = P.st;
+  i128* part = reinterpret_cast<i128*>(P.coop_scratch);  // [4][G]: tot, wsum, A, C
+  // phase A
+  i128 tot = 0, wsum = 0;
+  for (int j = b * kFieldThreads + (int)threadIdx.x; j < ng; j += G * kFieldThreads) {
+    long long r = 0;
+    for (int s = 0; s < P.ns; ++s) r += (long long)P.sp[s].sign * P.dens[(size_t)s * ng + j];
+    P.rho[j] = r;
+    tot += (i128)r;
+    if (j >= 1 && j <= nc - 1) wsum += (i128)(nc - j) * (i128)r;
+  }
+  tot = block_sum_128(tot, s_warp);
+  wsum = block_sum_128(wsum, s_warp);
+  if (threadIdx.x == 0) { part[b] = tot; part[G + b] = wsum; }
+  __threadfence();
+  grid.sync();
+  tot = 0; wsum = 0;
+  for (int i = threadIdx.x; i < G; i += kFieldThreads) { tot += part[i]; wsum += part[G + i]; }
+  tot = block_sum_128(tot, s_warp);
+  wsum = block_sum_128(wsum, s_warp);
+  if (b == 0 && threadIdx.x == 0) st->rho_total = (long long)tot;
+  const bool frozen = st->freeze_field != 0;
+  if (!frozen) {
+    // periodic: R'_j = nc R_j - tot  =>  T_nc' = nc * wsum - tot * nc (nc - 1) / 2
+    const i128 Tn = bc ? wsum : (i128)nc * wsum - tot * (((i128)nc * (i128)(nc - 1)) / 2);
+    // elements j = 1..jmax, CTA b owns [j_lo, j_hi]
+    const int jmax = bc ? nc : nc - 1;
+    const int unit = kFieldThreads * kFieldItems;
+    int per = (jmax + G - 1) / G;
+    per = ((per + unit - 1) / unit) * unit;
+    const int j_lo = min(1 + b * per, jmax + 1), j_hi = min(j_lo + per - 1, jmax);
+    // phase B
+    i128 A = 0, C = 0;
+    field_range<false>(P, j_lo, j_hi, tot, Tn, (i128)0, (i128)0, s_warp, &A, &C);
+    if (threadIdx.x == 0) { part[2 * G + b] = A; part[3 * G + b] = C; }
+    __threadfence();
+    grid.sync();
+    // phase C: S_{j_lo-1} = sum of A over earlier CTAs; T_{j_lo} = sum over earlier CTAs of (len * S_before + C)
+    i128 myA = 0, myLen = 0, myC = 0;
+    if ((int)threadIdx.x < G) {
+      const int i = threadIdx.x;
+      myA = part[2 * G + i];
+      myC = part[3 * G + i];
+      const int lo = min(1 + i * per, jmax + 1), hi = min(lo + per - 1, jmax);
+      myLen = hi >= lo ? hi - lo + 1 : 0;
+    }
+    i128 dummy;
+    const i128 Sbefore = block_exclusive_scan_128(myA, s_warp, &dummy);            // S at the start of CTA i
+    const i128 term = ((int)threadIdx.x < b) ? myLen * Sbefore + myC : (i128)0;
+    const i128 carryT = block_sum_128(term, s_warp);
+    const i128 carryS = block_sum_128(((int)threadIdx.x < b) ? myA : (i128)0, s_warp);
+    const i128 Send = block_sum_128(myA, s_warp);                                    // S_jmax
+    if (b == 0 && threadIdx.x == 0) {
+      // node 0
+      P.phi[0] = P.Kphi * dbl128((i128)0);
+      if (bc) {
+        P.E[0] = P.KE * dbl128(-2 * Tn - 2 * (i128)nc * (i128)P.rho[0]);
+      } else {
+        // periodic: S_{-1} = S_{nc-1}, S_0 = 0; ghosts at nc
+        P.E[0] = P.KE * dbl128((i128)nc * (Send + (i128)0) - 2 * Tn);
+        P.E[nc] = P.E[0];
+        P.phi[nc] = P.phi[0];
+      }
+    }
+    field_range<true>(P, j_lo, j_hi, tot, Tn, carryS, carryT, s_warp, nullptr, nullptr);
+  }
+  if (b == 0 && threadIdx.x == 0) {
     st->n = st->n_next;
     if (commit_step) st->step += 1ull;
     st->ovf_count = 0;
@@ -835,24 +945,45 @@ cudaError_t configure_kernels() {
   return cudaFuncSetAttribute(k_pass_b<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::b_total);
 }
 
+static int coop_grid(int work_items, int per_cta) {
+  int g = (work_items + per_cta - 1) / per_cta;
+  if (g < 1) g = 1;
+  const int cap = sm_count() < kFieldThreads ? sm_count() : kFieldThreads;   // co-resident, and G <= threads
+  return g < cap ? g : cap;
+}
+
+static void launch_mid(const Params& P, const Particles& cur, int do_colscan, cudaStream_t s) {
+  Params Pc = P;
+  Particles pc = cur;
+  int dc = do_colscan;
+  void* args[] = {&Pc, &pc, &dc};
+  cudaLaunchCooperativeKernel((const void*)k_mid, dim3(coop_grid(P.nc, kMidThreads)), dim3(kMidThreads), args, 0, s);
+}
+
+static void launch_field(const Params& P, int commit_step, cudaStream_t s) {
+  Params Pc = P;
+  int cs = commit_step;
+  void* args[] = {&Pc, &cs};
+  cudaLaunchCooperativeKernel((const void*)k_field, dim3(coop_grid(P.ng, kFieldThreads * kFieldItems)),
+                              dim3(kFieldThreads), args, 0, s);
+}
+
 int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int variant, cudaStream_t s,
                 cudaEvent_t* ev) {
   typedef PassSmem SM;
   const int g = particle_grid(P);
-  const int gc = (P.max_tiles + (kColThreads / 32) - 1) / (kColThreads / 32);
   if (ev) cudaEventRecord(ev[0], s);
   if (variant == 2) k_pass_a<2><<<g, kThreads, SM::a_total, s>>>(P, cur);
   else k_pass_a<1><<<g, kThreads, SM::a_total, s>>>(P, cur);
   if (ev) cudaEventRecord(ev[1], s);
-  k_mid<<<1, kMidThreads, 0, s>>>(P);
-  k_colscan<<<gc < 1 ? 1 : (gc > 16384 ? 16384 : gc), kColThreads, 0, s>>>(P, cur);
+  launch_mid(P, cur, 1, s);
   if (ev) cudaEventRecord(ev[2], s);
   if (variant == 2) k_pass_b<2><<<g, kThreads, SM::b_total, s>>>(P, cur, nxt);
   else k_pass_b<1><<<g, kThreads, SM::b_total, s>>>(P, cur, nxt);
   if (ev) cudaEventRecord(ev[3], s);
-  k_field<<<1, kFieldThreads, 0, s>>>(P, 1);
+  launch_field(P, 1, s);
   if (ev) cudaEventRecord(ev[4], s);
-  return 5;
+  return 4;
 }
 
 // load / restart: counts -> cell_start, deposit, field (no push).  cur must be sorted by cell.  (The tile
@@ -876,9 +1007,9 @@ int launch_rebuild(const Params& P, const Particles& cur, cudaStream_t s) {
   const int g = sm_count() * 4;
   k_clear_grids<<<g, 256, 0, s>>>(P);
   k_count_cells<<<g, kAuxThreads, 0, s>>>(P, cur);
-  k_mid<<<1, kMidThreads, 0, s>>>(P);   // ovf_count == 0: plain scan; n_next = n
+  launch_mid(P, cur, 0, s);   // ovf_count == 0: plain scan; n_next = n; no column scan (no tile rows yet)
   k_deposit<<<g, kAuxThreads, 0, s>>>(P, cur);
-  k_field<<<1, kFieldThreads, 0, s>>>(P, 0);  // commits n = n_next, leaves the step counter alone
+  launch_field(P, 0, s);  // commits n = n_next, leaves the step counter alone
   return 5;
 }
 
