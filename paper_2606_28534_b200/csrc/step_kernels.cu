@@ -598,45 +598,62 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
         }
       }
     }
-    // phase 2: stable rank inside (warp, cell) -> destination; deposit; scatter
+    // phase 2: stable rank inside (warp, cell) -> destination; deposit; scatter.  Written as batches of the
+    // same operation over the kItems particles so that the shared-memory and warp-wide operations of different
+    // particles overlap instead of forming one long dependent chain.
+    int sp[kItems];
+    unsigned m[kItems], a[kItems], old[kItems];
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
       const int off = warp * kWarpSpan + r * 32 + lane;
       const bool valid = key[r] >= 0;
-      const int sp = valid ? (int)S->sp[off] : 0;
-      const unsigned mk = valid ? (unsigned)key[r] : (0x80000000u | (unsigned)lane);
-      const unsigned m = __match_any_sync(0xffffffffu, mk);
-      const int leader = __ffs(m) - 1;
-      unsigned old = 0;
-      if (valid && lane == leader) {
-        old = wc[key[r]];
-        wc[key[r]] = old + (unsigned)__popc(m);
-      }
-      old = __shfl_sync(0xffffffffu, old, leader);
-      const unsigned dst = old + (unsigned)__popc(m & lt);
-      // deposit (SURVEY 8(c) "D"): one shared-memory atomic pair per (cell, species) run of the warp
-      const unsigned Q = (unsigned)s_sp[sp].Q;
-      const unsigned a = valid ? deposit_a(x[r], tw.wlo + key[r], P.inv_dx, Q) : 0u;
-      if (P.dep_u32) {
-        // Q < 2^21: the sum of a over a warp stays below 2^26
-        const unsigned m2 = __match_any_sync(0xffffffffu, valid ? (mk << 3) | (unsigned)sp : mk);
-        const unsigned sa = __reduce_add_sync(m2, a);
-        if (valid && lane == __ffs(m2) - 1) {
-          atomicAdd(&s_dens[key[r] * ns + sp], (unsigned)__popc(m2) * Q - sa);
-          atomicAdd(&s_dens[(key[r] + 1) * ns + sp], sa);
-        }
-      } else if (valid) {
-        const int c = tw.wlo + key[r];
-        int j1 = c + 1;
-        if (!P.bc && j1 == P.nc) j1 = 0;
-        atomicAdd((unsigned long long*)&P.dens[(size_t)sp * P.ng + c], (unsigned long long)(Q - a));
-        atomicAdd((unsigned long long*)&P.dens[(size_t)sp * P.ng + j1], (unsigned long long)a);
-      }
-      if (valid) {
-        nxt.x[dst] = x[r]; nxt.vx[dst] = vx[r]; nxt.vy[dst] = vy[r]; nxt.vz[dst] = vz[r];
-        nxt.cell[dst] = tw.wlo + key[r]; nxt.pid[dst] = S->pid[off]; nxt.sp[dst] = (unsigned char)sp;
-      }
+      sp[r] = valid ? (int)S->sp[off] : 0;
+      m[r] = __match_any_sync(0xffffffffu, valid ? (unsigned)key[r] : (0x80000000u | (unsigned)lane));
+      a[r] = valid ? deposit_a(x[r], tw.wlo + key[r], P.inv_dx, (unsigned)s_sp[sp[r]].Q) : 0u;
+    }
+    // the leader of every (item, cell) group reserves the group's destinations; items in order (stability)
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) {
+      old[r] = 0;
+      if (key[r] >= 0 && lane == __ffs(m[r]) - 1) old[r] = atomicAdd(&wc[key[r]], (unsigned)__popc(m[r]));
       __syncwarp();
+    }
+    // deposit (SURVEY 8(c) "D"): one shared-memory atomic pair per (cell, species) run of the warp
+    if (P.dep_u32) {
+      // Q < 2^21: the sum of a over a warp stays below 2^26
+#pragma unroll
+      for (int r = 0; r < kItems; ++r) {
+        const bool valid = key[r] >= 0;
+        const unsigned mk2 = valid ? ((unsigned)key[r] << 3) | (unsigned)sp[r] : (0x80000000u | (unsigned)lane);
+        const unsigned m2 = __match_any_sync(0xffffffffu, mk2);
+        const unsigned sa = __reduce_add_sync(m2, a[r]);
+        if (valid && lane == __ffs(m2) - 1) {
+          atomicAdd(&s_dens[key[r] * ns + sp[r]], (unsigned)__popc(m2) * (unsigned)s_sp[sp[r]].Q - sa);
+          atomicAdd(&s_dens[(key[r] + 1) * ns + sp[r]], sa);
+        }
+      }
+    } else {
+#pragma unroll
+      for (int r = 0; r < kItems; ++r) {
+        if (key[r] >= 0) {
+          const int c = tw.wlo + key[r];
+          int j1 = c + 1;
+          if (!P.bc && j1 == P.nc) j1 = 0;
+          const unsigned Q = (unsigned)s_sp[sp[r]].Q;
+          atomicAdd((unsigned long long*)&P.dens[(size_t)sp[r] * P.ng + c], (unsigned long long)(Q - a[r]));
+          atomicAdd((unsigned long long*)&P.dens[(size_t)sp[r] * P.ng + j1], (unsigned long long)a[r]);
+        }
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < kItems; ++r) {
+      const unsigned o = __shfl_sync(0xffffffffu, old[r], __ffs(m[r]) - 1);
+      if (key[r] >= 0) {
+        const int off = warp * kWarpSpan + r * 32 + lane;
+        const unsigned dst = o + (unsigned)__popc(m[r] & lt);
+        nxt.x[dst] = x[r]; nxt.vx[dst] = vx[r]; nxt.vy[dst] = vy[r]; nxt.vz[dst] = vz[r];
+        nxt.cell[dst] = tw.wlo + key[r]; nxt.pid[dst] = S->pid[off]; nxt.sp[dst] = (unsigned char)sp[r];
+      }
     }
     fence_proxy_async();
     __syncthreads();  // the stage may be overwritten; the tile's deposit is complete
