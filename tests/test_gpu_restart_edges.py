@@ -1,0 +1,235 @@
+"""GPU tests beyond the plain parity cases: checkpoint/restart, determinism,
+edge cases (empty input, capacity hit, window radius, degenerate tiles) and the error behaviour of the C ABI.
+Everything goes through the C ABI (paper_2606_28534_b200.binding) and is compared with the CPU oracle."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2606_28534_b200 import workloads as W
+from parity import run_pair, assert_state_equal
+
+pytestmark = pytest.mark.gpu
+
+
+def _state(g):
+    p = g.get_particles()
+    p["rho"] = g.get_rho()
+    p["dens"] = g.get_dens()
+    p["E"] = g.get_E()
+    p["phi"] = g.get_phi()
+    m = g.get_moments()
+    p["wall_count"], p["wall_charge"] = m["wall_count"], m["wall_charge"]
+    p["scalars"] = np.array([m["step"], m["next_pid"], m["births"], m["reinject"], m["flags"], m["rho_total"]],
+                            dtype=np.int64)
+    p["events"], p["candidates"] = m["events"], m["candidates"]
+    return p
+
+
+def _assert_identical(a, b, where):
+    assert a.keys() == b.keys()
+    for k in a:
+        assert np.array_equal(a[k], b[k]), f"{where}: {k} differs"
+
+
+@pytest.mark.parametrize("staging", [False, True])
+@pytest.mark.parametrize("cfg,scale,kw", [
+    (2, 1 / 32, dict(pair_source=True)),
+    (3, 1 / 128, dict(n0_scale=200.0)),
+    (5, 1 / 8192, dict(n0_scale=200.0)),
+])
+def test_checkpoint_restart_is_bit_identical(cfg, scale, kw, staging):
+    """run 0 -> m  ==  run 0 -> k, checkpoint, (keep stepping), restart from the blob, k -> m; also == oracle."""
+    import torch
+    from oracle.oracle import Oracle
+    from paper_2606_28534_b200.binding import Bit1
+
+    k, m = 7, 19
+    w = W.make_config(cfg, scale=scale, **kw)
+    ref = Bit1(w)
+    ref.load()
+    ref.step(m)
+    ref.sync(check_flags=False)
+    want = _state(ref)
+    ref.close()
+
+    g = Bit1(w, checkpoint_staging=staging)
+    g.load()
+    g.step(k)
+    blob = torch.empty(g.checkpoint_size(), dtype=torch.uint8).pin_memory()
+    written = g.checkpoint(blob)
+    assert written == g.checkpoint_size()
+    g.step(5)  # the snapshot must not see these steps (they overlap the D2H copy when staging is on)
+    g.checkpoint_wait()
+    g.sync(check_flags=False)
+    g.close()
+
+    h = Bit1(w, checkpoint_staging=staging)  # a fresh context, as after a crash
+    h.restart(blob)
+    assert h.get_moments()["step"] == k
+    h.step(m - k)
+    h.sync(check_flags=False)
+    _assert_identical(_state(h), want, f"c{cfg} restart staging={staging}")
+
+    o = Oracle(w)
+    o.step(m)
+    assert assert_state_equal(h, o, where=f"c{cfg} restarted run vs oracle")
+    h.close()
+
+
+def test_restart_rejects_a_blob_of_another_configuration():
+    import torch
+    from paper_2606_28534_b200.binding import Bit1, Bit1Error, ERR_CHECKPOINT
+
+    w = W.make_config(2, scale=1 / 64)
+    g = Bit1(w)
+    g.load()
+    blob = torch.empty(g.checkpoint_size(), dtype=torch.uint8).pin_memory()
+    g.checkpoint(blob)
+    g.checkpoint_wait()
+    g.close()
+    w2 = W.make_config(2, scale=1 / 64, lib_seed=99)  # same sizes, other seed -> other config hash
+    h = Bit1(w2)
+    with pytest.raises(Bit1Error) as e:
+        h.restart(blob)
+    assert e.value.status == ERR_CHECKPOINT
+    bad = blob.clone()
+    bad[0] = 0  # magic
+    with pytest.raises(Bit1Error):
+        Bit1(w).restart(bad)
+    h.close()
+
+
+def test_two_runs_give_identical_bits():
+    w = W.make_config(3, scale=1 / 64, n0_scale=100.0)
+    a, _ = None, None
+    from paper_2606_28534_b200.binding import Bit1
+
+    states = []
+    for _ in range(2):
+        g = Bit1(w)
+        g.load()
+        g.step(25)
+        g.sync(check_flags=False)
+        states.append(_state(g))
+        g.close()
+    _assert_identical(states[0], states[1], "determinism")
+
+
+def test_empty_input_steps_and_reports_zero():
+    from paper_2606_28534_b200.binding import Bit1
+
+    w = W.make_config(2, scale=1 / 64)
+    g = Bit1(w)
+    e = np.zeros(0)
+    g.load_particles(e, e, e, e, np.zeros(0, np.uint8))
+    g.step(3)
+    g.sync()
+    assert g.n_live() == 0
+    assert not g.get_rho().any() and not g.get_E().any() and not g.get_phi().any()
+    m = g.get_moments()
+    assert m["step"] == 3 and m["n_live"] == 0 and m["flags"] == 0
+    g.close()
+
+
+@pytest.mark.parametrize("n", [1, 31, 1023, 1024, 1025, 2049])
+def test_ragged_and_single_tile_sizes(n):
+    """Particle counts around the tile size (1024): one particle, one warp minus one, exactly one tile, one
+    tile plus a one-particle tail."""
+    w0 = W.make_config(3, scale=1 / 256, n0_scale=300.0)
+    idx = np.random.default_rng(5).choice(w0.n, size=n, replace=False)
+    idx.sort()
+    for k in ("x", "vx", "vy", "vz", "sp"):
+        setattr(w0, k, np.ascontiguousarray(getattr(w0, k)[idx]))
+    g, o = run_pair(w0, 5)
+    assert assert_state_equal(g, o, where=f"n={n}")
+    g.close()
+
+
+def test_all_particles_in_one_cell_and_sparse_cells():
+    """Degenerate tiles: every particle in one cell (a cell spanning many tiles), and a plasma so thin that a
+    tile spans more cells than the shared-memory window holds (the rest goes through the side list)."""
+    w = W.make_config(2, scale=1 / 64)
+    n = 6000
+    rng = np.random.default_rng(11)
+    L = w.nc * w.dx
+    for k in ("vx", "vy", "vz", "sp"):
+        setattr(w, k, np.ascontiguousarray(getattr(w, k)[:n]))
+    w.x = np.ascontiguousarray((17 + rng.random(n)) * w.dx)  # all in cell 17
+    g, o = run_pair(w, 4)
+    assert assert_state_equal(g, o, where="one cell")
+    g.close()
+    w = W.make_config(2, scale=1 / 4)  # 1024 cells
+    n = 1500  # ~1.5 particles per cell: a 1024-particle tile spans ~700 cells > window capacity
+    sel = np.sort(rng.choice(w.n, size=n, replace=False))
+    for k in ("x", "vx", "vy", "vz", "sp"):
+        setattr(w, k, np.ascontiguousarray(getattr(w, k)[sel]))
+    g, o = run_pair(w, 3)
+    assert assert_state_equal(g, o, where="sparse cells")
+    assert g.get_moments()["far_movers"] > 0
+    g.close()
+
+
+def test_capacity_hit_matches_oracle_and_raises_the_sticky_flag():
+    """Ionisation births beyond capacity are dropped in (parent, kind) order and flag CAPACITY (reading R-W)."""
+    from paper_2606_28534_b200.binding import Bit1Error, ERR_DEVICE_FLAG, FLAG_CAPACITY
+
+    w = W.make_config(3, scale=1 / 256, n0_scale=3000.0, capacity_factor=1.0)
+    w.capacity = w.n + 40
+    g, o = run_pair(w, 12)
+    assert o.flagword & FLAG_CAPACITY, "the workload was meant to run out of capacity"
+    assert assert_state_equal(g, o, where="capacity")
+    with pytest.raises(Bit1Error) as e:
+        g.sync()
+    assert e.value.status == ERR_DEVICE_FLAG
+    g.close()
+
+
+@pytest.mark.parametrize("R", [0, 2, 4])
+def test_sort_window_radius_does_not_change_the_result(R):
+    """Reading R-win: R only moves particles between the windowed path and the side list."""
+    os.environ["BIT1_WINDOW_R"] = str(R)
+    try:
+        w = W.make_config(3, scale=1 / 128, n0_scale=200.0)
+        g, o = run_pair(w, 10)
+        assert assert_state_equal(g, o, where=f"R={R}")
+        g.close()
+        w = W.make_config(1, scale=1 / 8)
+        g, o = run_pair(w, 10)
+        assert assert_state_equal(g, o, where=f"R={R} periodic")
+        g.close()
+    finally:
+        del os.environ["BIT1_WINDOW_R"]
+
+
+def test_error_behaviour_of_the_c_abi():
+    from paper_2606_28534_b200.binding import (Bit1, Bit1Error, ERR_CAPACITY, ERR_INVALID_ARG, ERR_RANGE,
+                                               ERR_STATE)
+
+    w = W.make_config(2, scale=1 / 64)
+    g = Bit1(w)
+    with pytest.raises(Bit1Error) as e:
+        g.step(1)  # nothing loaded yet
+    assert e.value.status == ERR_STATE
+    big = np.zeros(w.capacity + 1)
+    with pytest.raises(Bit1Error) as e:
+        g.load_particles(big, big, big, big, np.zeros(big.shape[0], np.uint8))
+    assert e.value.status == ERR_CAPACITY
+    x = w.x.copy()
+    x[5] = w.nc * w.dx * 1.5  # outside [0, L)
+    with pytest.raises(Bit1Error) as e:
+        g.load_particles(x, w.vx, w.vy, w.vz, w.sp)
+    assert e.value.status == ERR_INVALID_ARG
+    sp = w.sp.copy()
+    sp[3] = 7  # no such species
+    with pytest.raises(Bit1Error) as e:
+        g.load_particles(w.x, w.vx, w.vy, w.vz, sp)
+    assert e.value.status == ERR_INVALID_ARG
+    g.load()  # the context is still usable
+    g.step(2)
+    g.sync()
+    g.close()
+    w.species[0].weight *= 1e9  # Q >= 2^31
+    with pytest.raises(Bit1Error) as e:
+        Bit1(w)
+    assert e.value.status == ERR_RANGE
