@@ -28,6 +28,7 @@ sys.path.insert(0, ROOT)
 
 STATE_BYTES = 41  # x, vx, vy, vz fp64 + cell int32 + pid uint32 + species uint8
 METRIC = "particle-steps/sec"
+UNIT = "particle-steps/s"
 
 
 def _peaks():
@@ -38,9 +39,12 @@ def _peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def _traffic(kernel: str):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, if any."""
+def _traffic(kernel: str, args=None):
+    """DRAM bytes per launch of the kernel from the committed ncu --set full capture (profiles/traffic.json);
+    the capture is of the default workload, so any other workload reports null."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
+    if args is not None and (args.config != 4 or args.scale != 1.0):
+        return None
     if os.path.exists(p):
         with open(p) as f:
             return json.load(f).get(kernel)
@@ -142,7 +146,7 @@ def cpu_baseline(args, seconds_hint: float = 12.0):
         if time.perf_counter() - t0 > seconds_hint or steps >= 400:
             break
     dt = time.perf_counter() - t0
-    return {"value": w.n * steps / dt, "unit": METRIC, "cores": 1, "kind": "oracle",
+    return {"value": w.n * steps / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
             "sample": f"configs[{args.config - 1}] cut down to {w.n} particles / {w.nc} cells (same particles per "
                       f"cell and profile), {steps} steps in {dt:.1f} s, single thread, gcc -O2 -ffp-contract=off"}
 
@@ -279,10 +283,10 @@ def run_cuda(args):
         "roofline": {"bound": "hbm", "kernel": f"k_pass_b<{variant}> (arranger: stable scatter + fused deposit)",
                      "achieved": b_bytes / (b_ms * 1e-3) / 1e9 if b_ms > 0 else None, "peak": peak, "unit": "GB/s",
                      "frac": (b_bytes / (b_ms * 1e-3) / 1e9 / peak) if b_ms > 0 else None,
-                     "traffic": _traffic("k_pass_b"), "peak_source": peak_src,
+                     "traffic": _traffic("k_pass_b", args), "peak_source": peak_src,
                      "bytes_per_particle": 2 * STATE_BYTES,
                      "pass_a": {"achieved": a_bytes / (a_ms * 1e-3) / 1e9 if a_ms > 0 else None,
-                                "bytes_per_particle": a_bytes / n_mean, "traffic": _traffic("k_pass_a")},
+                                "bytes_per_particle": a_bytes / n_mean, "traffic": _traffic("k_pass_a", args)},
                      "step": {"bytes_per_particle_step": step_bytes / n_mean,
                               "achieved": step_bytes / (ms_max / args.steps * 1e-3) / 1e9,
                               "frac_of_measured_peak": step_bytes / (ms_max / args.steps * 1e-3) / 1e9 / peak,
