@@ -260,10 +260,13 @@ def run_cuda(args):
     peak, peak_src = _peaks()
     n_mean = 0.5 * (n_start + n_end)
     variant = 1 if args.variant == 1 else 2
-    # dominant kernel: the arranger (pass B): reads the 41 B state and writes it to its sorted slot
-    b_bytes = 2 * STATE_BYTES * n_mean
+    # dominant kernel: the arranger (pass B).  Algorithmic bytes per particle: V2 reads the 41 B
+    # state minus the 4 B cell index (recomputed from x) in both passes and writes 41 B in pass B: 37 + 78 = 115 B;
+    # V1 writes x, v, cell in place in pass A (37 + 36) and reads everything in pass B (41 + 41).
+    a_bpp, b_bpp = (37, 78) if variant == 2 else (73, 82)
+    b_bytes = b_bpp * n_mean
     b_ms = prof["pass_b"] / max(psteps, 1)
-    a_bytes = STATE_BYTES * n_mean * (1 if variant == 2 else 2) - (0 if variant == 2 else 5 * n_mean)
+    a_bytes = a_bpp * n_mean
     a_ms = prof["pass_a"] / max(psteps, 1)
     step_bytes = a_bytes + b_bytes
     kernels = {k: round(v / max(psteps, 1), 4) for k, v in prof.items()}
@@ -284,7 +287,7 @@ def run_cuda(args):
                      "achieved": b_bytes / (b_ms * 1e-3) / 1e9 if b_ms > 0 else None, "peak": peak, "unit": "GB/s",
                      "frac": (b_bytes / (b_ms * 1e-3) / 1e9 / peak) if b_ms > 0 else None,
                      "traffic": _traffic("k_pass_b", args), "peak_source": peak_src,
-                     "bytes_per_particle": 2 * STATE_BYTES,
+                     "bytes_per_particle": b_bpp,
                      "pass_a": {"achieved": a_bytes / (a_ms * 1e-3) / 1e9 if a_ms > 0 else None,
                                 "bytes_per_particle": a_bytes / n_mean, "traffic": _traffic("k_pass_a", args)},
                      "step": {"bytes_per_particle_step": step_bytes / n_mean,

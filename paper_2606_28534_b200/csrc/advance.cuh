@@ -225,7 +225,7 @@ template <bool EMIT>
 static __device__ __noinline__ int slow_advance(const Params& P, const SpeciesP* S, unsigned long long step,
                                                 const double* Eptr, Stage* st, int off, unsigned gidx) {
   double x = st->x[off], vx = st->vx[off], vy = st->vy[off], vz = st->vz[off];
-  int c = st->cell[off];
+  int c = cell_of(P, x);   // the particle's current cell (the staged tile may not carry the cell array)
   advance<EMIT>(P, S, step, Eptr, (int)st->sp[off], st->pid[off], gidx, x, vx, vy, vz, c);
   st->x[off] = x; st->vx[off] = vx; st->vy[off] = vy; st->vz[off] = vz;
   return c;

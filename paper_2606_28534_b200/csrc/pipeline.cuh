@@ -61,11 +61,14 @@ __device__ __forceinline__ bool e_window(int clo, int chi, int& e0, int& ne) {
 // One elected thread: arm the stage's barrier and issue the copies of tile `tile` (always whole tiles: the
 // arrays are padded to a multiple of kTile, the tail of the last tile is never used).
 __device__ __forceinline__ void issue_tile(const Params& P, const Particles& cur, Stage* st, unsigned long long* bar,
-                                           int tile, int2 d, bool with_evt, bool with_E, bool with_rank) {
+                                           int tile, int2 d, bool with_evt, bool with_E, bool with_rank,
+                                           bool with_cell) {
   const size_t base = (size_t)tile * kTile;
   int e0 = 0, ne = 0;
   const bool stage_E = with_E && e_window(d.x, d.y, e0, ne);
-  unsigned bytes = 4u * kTile * 8u + 2u * kTile * 4u + kTile;
+  // the cell array is not fetched on the V2 path: cell == cell_of(x) by construction (load, pass B, side list)
+  unsigned bytes = 4u * kTile * 8u + kTile * 4u + kTile;
+  if (with_cell) bytes += kTile * 4u;
   if (with_evt) bytes += kTile / 8;
   if (stage_E) bytes += (unsigned)ne * 8u;
   // window of the tile, rounded up to whole 16-byte units (the rows are padded, see tile_row_offset)
@@ -79,7 +82,7 @@ __device__ __forceinline__ void issue_tile(const Params& P, const Particles& cur
   bulk_g2s(st->vx, cur.vx + base, kTile * 8, bar);
   bulk_g2s(st->vy, cur.vy + base, kTile * 8, bar);
   bulk_g2s(st->vz, cur.vz + base, kTile * 8, bar);
-  bulk_g2s(st->cell, cur.cell + base, kTile * 4, bar);
+  if (with_cell) bulk_g2s(st->cell, cur.cell + base, kTile * 4, bar);
   bulk_g2s(st->pid, cur.pid + base, kTile * 4, bar);
   bulk_g2s(st->sp, cur.sp + base, kTile, bar);
   if (with_evt) bulk_g2s(st->evt, P.evt + base / 32, kTile / 8, bar);

@@ -96,7 +96,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
     fence_proxy_async();
     for (int k = 0; k < 2; ++k) {
       const int t = blockIdx.x + k * G;
-      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, tile_cells(cur, t, n), false, true, false);
+      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, tile_cells(cur, t, n), false, true, false, false);
     }
   }
   load_species(P, s_sp);
@@ -137,8 +137,8 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
       const bool have = (unsigned)off < cnt;
       const int sp = have ? (int)S->sp[off] : 0;
       const SpeciesP& s = s_sp[sp];
-      const int c = have ? S->cell[off] : clo;
       x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off];
+      const int c = have ? cell_of(P, x[r]) : clo;
       const bool inside = push_fast(P, s, Eptr, c, x[r], vx[r], vy[r], vz[r]);
       cn[r] = cell_of(P, x[r]);
       const int k = cn[r] - tw.wlo;
@@ -218,7 +218,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
       const int c = tw.wlo + k;
       if (run && c >= 0 && c < P.nc) atomicAdd(&P.cell_count[c], (int)run);
     }
-    if (threadIdx.x == 0 && tnext < ntiles) issue_tile(P, cur, S, &bar[it & 1], tnext, dn, false, true, false);
+    if (threadIdx.x == 0 && tnext < ntiles) issue_tile(P, cur, S, &bar[it & 1], tnext, dn, false, true, false, false);
   }
 }
 
@@ -539,7 +539,7 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     fence_proxy_async();
     for (int k = 0; k < 2; ++k) {
       const int t = blockIdx.x + k * G;
-      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, cur.desc[t], VARIANT == 2, VARIANT == 2, true);
+      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, cur.desc[t], VARIANT == 2, VARIANT == 2, true, VARIANT == 1);
     }
   }
   load_species(P, s_sp);
@@ -574,8 +574,9 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     for (int r = 0; r < kItems; ++r) {
       const int off = warp * kWarpSpan + r * 32 + lane;
       const bool have = (unsigned)off < cnt;
-      int c = have ? S->cell[off] : d.x;
       x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off];
+      int c = d.x;
+      if (have) c = VARIANT == 2 ? cell_of(P, x[r]) : S->cell[off];
       if (VARIANT == 2) {
         const int sp = have ? (int)S->sp[off] : 0;
         if (have && ((S->evt[warp * kItems + r] >> lane) & 1u)) evm |= 1u << r;
@@ -658,7 +659,7 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     fence_proxy_async();
     __syncthreads();  // the stage may be overwritten; the tile's deposit is complete
     if (threadIdx.x == 0 && tnext < ntiles)
-      issue_tile(P, cur, S, &bar[it & 1], tnext, dn, VARIANT == 2, VARIANT == 2, true);
+      issue_tile(P, cur, S, &bar[it & 1], tnext, dn, VARIANT == 2, VARIANT == 2, true, VARIANT == 1);
     if (P.dep_u32) {
       for (int k = threadIdx.x; k < ns * (tw.W + 1); k += kThreads) {
         const unsigned v = s_dens[k];
