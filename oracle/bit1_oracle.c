@@ -113,6 +113,13 @@ typedef struct {
   uint64_t diag_nu_overflow, diag_dir_fallback, diag_escape, diag_births, diag_reinject;
   uint64_t diag_candidates[ORC_MAX_SPECIES];
   uint64_t diag_events[ORC_MAX_SPECIES][3]; /* elastic, ionise, cx */
+  /* NEXT-1: density smoothing and time-averaged diagnostics */
+  int32_t smooth_passes; /* 0 = off */
+  int64_t *rho_s;        /* ng: 4^passes * smoothed rho, what the field solve used */
+  int32_t avg_window, avg_interval; /* mvflag, mvStep; 0 = off */
+  int64_t *acc_dens, *avg_dens;     /* ns*ng running / latched sums over the window */
+  double *acc_phi, *avg_phi;        /* nc+1 */
+  uint64_t acc_count, avg_count, avg_step;
 } orc;
 
 /* ------------------------------------------------------------------ */
@@ -278,6 +285,11 @@ orc *orc_create(int32_t nc, double dx, int32_t bc, double area, const double B[3
   o->rho = xcalloc((size_t)o->ng, 8);
   o->phi = xcalloc((size_t)nc + 1, 8);
   o->E = xcalloc((size_t)nc + 1, 8);
+  o->rho_s = xcalloc((size_t)o->ng, 8);
+  o->acc_dens = xcalloc((size_t)ns * (size_t)o->ng, 8);
+  o->avg_dens = xcalloc((size_t)ns * (size_t)o->ng, 8);
+  o->acc_phi = xcalloc((size_t)nc + 1, 8);
+  o->avg_phi = xcalloc((size_t)nc + 1, 8);
   return o;
 }
 
@@ -287,6 +299,7 @@ void orc_destroy(orc *o) {
   free(o->x); free(o->vx); free(o->vy); free(o->vz); free(o->cell); free(o->pid); free(o->sp);
   free(o->x2); free(o->vx2); free(o->vy2); free(o->vz2); free(o->cell2); free(o->pid2); free(o->sp2);
   free(o->cell_start); free(o->dens); free(o->rho); free(o->phi); free(o->E);
+  free(o->rho_s); free(o->acc_dens); free(o->avg_dens); free(o->acc_phi); free(o->avg_phi);
   free(o);
 }
 
@@ -417,7 +430,93 @@ void orc_poisson(int32_t nc, int32_t bc, double Kphi, double KE, const int64_t *
   free(S); free(T);
 }
 
-void orc_phase_field(orc *o) { orc_poisson(o->nc, o->bc, o->Kphi, o->KE, o->rho, o->phi, o->E); }
+/* Density smoothing ("density smoothing ... improve[s] numerical stability", PAPER.md:37
+ * "smoothing operators"; reading N1-a).  One pass of the 1-2-1 binomial
+ * filter in exact integers: out_j = in_{j-1} + 2 in_j + in_{j+1} = 4 x the smoothed value (the 1/4 is
+ * folded into the field constants).  Every node hands 1/4, 1/2, 1/4 of its charge to j-1, j, j+1;
+ * periodic: indices wrap; bounded: the quarter that would leave through a wall stays on the wall node
+ * (out_0 = 3 in_0 + in_1, out_nc = in_{nc-1} + 3 in_nc), so the total charge is conserved exactly:
+ * sum(out) = 4 sum(in), and global Gauss's law keeps holding in the integers. */
+void orc_smooth121(int32_t nc, int32_t bc, const int64_t *in, int64_t *out) {
+  if (bc) {
+    out[0] = 3 * in[0] + in[1];
+    for (int32_t j = 1; j < nc; ++j) out[j] = in[j - 1] + 2 * in[j] + in[j + 1];
+    out[nc] = in[nc - 1] + 3 * in[nc];
+  } else {
+    for (int32_t j = 0; j < nc; ++j) {
+      int32_t jm = j == 0 ? nc - 1 : j - 1, jp = j == nc - 1 ? 0 : j + 1;
+      out[j] = in[jm] + 2 * in[j] + in[jp];
+    }
+  }
+}
+
+/* Field phase: `smooth_passes` passes over rho (the per-species densities stay as deposited), then the
+ * Poisson solve with both constants scaled by 4^-passes (an exact power of two). */
+void orc_phase_field(orc *o) {
+  int32_t p = o->smooth_passes;
+  if (p <= 0) {
+    orc_poisson(o->nc, o->bc, o->Kphi, o->KE, o->rho, o->phi, o->E);
+    return;
+  }
+  int64_t *tmp = (int64_t *)xcalloc((size_t)o->ng, 8);
+  memcpy(o->rho_s, o->rho, (size_t)o->ng * 8);
+  for (int32_t k = 0; k < p; ++k) {
+    orc_smooth121(o->nc, o->bc, o->rho_s, tmp);
+    memcpy(o->rho_s, tmp, (size_t)o->ng * 8);
+  }
+  free(tmp);
+  double scale = 1.0 / (double)((int64_t)1 << (2 * p));
+  orc_poisson(o->nc, o->bc, o->Kphi * scale, o->KE * scale, o->rho_s, o->phi, o->E);
+}
+
+/* Time-averaged diagnostics (Table 2: `datfile` "time-averaged diagnostics", `mvflag`
+ * "snapshot averaged over mvflag time steps", `mvStep` "interval between successive diagnostic outputs";
+ * SURVEY 8(f) NEXT-1; reading N1-b).  With window W = mvflag and interval I = mvStep (W <= I):
+ * after the step that makes the step counter k, r = k mod I (0 read as I); the grid state of that step
+ * (per-species deposited charge, phi) joins the running sums when r > I - W, i.e. over the last W steps
+ * of every interval; at r == I the sums are latched as the latest output and cleared.  Densities are
+ * summed in int64 (exact), phi in fp64 in step order (one addition per node and step). */
+static void phase_average(orc *o) {
+  int32_t W = o->avg_window, I = o->avg_interval;
+  if (W <= 0) return;
+  uint64_t r = o->step % (uint64_t)I;
+  if (r == 0) r = (uint64_t)I;
+  size_t nd = (size_t)o->ns * (size_t)o->ng;
+  if (r > (uint64_t)(I - W)) {
+    for (size_t i = 0; i < nd; ++i) o->acc_dens[i] += o->dens[i];
+    for (int32_t j = 0; j <= o->nc; ++j) o->acc_phi[j] = o->acc_phi[j] + o->phi[j];
+    o->acc_count += 1;
+  }
+  if (r == (uint64_t)I) {
+    memcpy(o->avg_dens, o->acc_dens, nd * 8);
+    memcpy(o->avg_phi, o->acc_phi, ((size_t)o->nc + 1) * 8);
+    o->avg_count = o->acc_count;
+    o->avg_step = o->step;
+    memset(o->acc_dens, 0, nd * 8);
+    memset(o->acc_phi, 0, ((size_t)o->nc + 1) * 8);
+    o->acc_count = 0;
+  }
+}
+
+void orc_set_smoothing(orc *o, int32_t passes) { o->smooth_passes = passes < 0 ? 0 : (passes > 8 ? 8 : passes); }
+/* (re)arms the averaging: running and latched sums are cleared */
+int orc_set_averaging(orc *o, int32_t window, int32_t interval) {
+  if (window < 0 || (window > 0 && interval < window)) return 1;
+  o->avg_window = window; o->avg_interval = window > 0 ? interval : 0;
+  size_t nd = (size_t)o->ns * (size_t)o->ng;
+  memset(o->acc_dens, 0, nd * 8); memset(o->avg_dens, 0, nd * 8);
+  memset(o->acc_phi, 0, ((size_t)o->nc + 1) * 8); memset(o->avg_phi, 0, ((size_t)o->nc + 1) * 8);
+  o->acc_count = 0; o->avg_count = 0; o->avg_step = 0;
+  return 0;
+}
+void orc_get_average(const orc *o, int64_t *dens_sum, double *phi_sum, uint64_t *count, uint64_t *step) {
+  memcpy(dens_sum, o->avg_dens, (size_t)o->ns * (size_t)o->ng * 8);
+  memcpy(phi_sum, o->avg_phi, ((size_t)o->nc + 1) * 8);
+  *count = o->avg_count; *step = o->avg_step;
+}
+void orc_get_rho_smoothed(const orc *o, int64_t *out) {
+  memcpy(out, o->smooth_passes > 0 ? o->rho_s : o->rho, (size_t)o->ng * 8);
+}
 
 /* ------------------------------------------------------------------ */
 /* Append one birth.  SURVEY 8(c) "A": parent-index order, pid = next_pid + r;
@@ -607,6 +706,7 @@ void orc_step(orc *o, uint64_t nsteps, int freeze_field) {
     orc_phase_deposit(o);
     if (!freeze_field) orc_phase_field(o);
     o->step += 1;
+    phase_average(o);
   }
 }
 

@@ -78,6 +78,12 @@ def lib():
         L.orc_get_density.argtypes = [C.c_void_p, C.c_int, c_f64p]
         L.orc_get_moments.argtypes = [C.c_void_p, c_u64p, c_f64p, c_f64p, c_f64p]
         L.orc_poisson.argtypes = [C.c_int32, C.c_int32, C.c_double, C.c_double, c_i64p, c_f64p, c_f64p]
+        L.orc_smooth121.argtypes = [C.c_int32, C.c_int32, c_i64p, c_i64p]
+        L.orc_set_smoothing.argtypes = [C.c_void_p, C.c_int32]
+        L.orc_set_averaging.restype = C.c_int
+        L.orc_set_averaging.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
+        L.orc_get_average.argtypes = [C.c_void_p, c_i64p, c_f64p, c_u64p, c_u64p]
+        L.orc_get_rho_smoothed.argtypes = [C.c_void_p, c_i64p]
         L.orc_philox4x32_10.argtypes = [c_u32p, c_u32p, c_u32p]
         L.orc_u53.restype = C.c_double
         L.orc_u53.argtypes = [C.c_uint32, C.c_uint32]
@@ -122,6 +128,14 @@ def poisson(nc, bc, Kphi, KE, rho):
     E = np.zeros(nc + 1)
     lib().orc_poisson(nc, bc, Kphi, KE, _p(rho, c_i64p), _p(phi, c_f64p), _p(E, c_f64p))
     return phi, E
+
+
+def smooth121(nc, bc, rho):
+    """One 1-2-1 pass in exact integers: returns 4 x the smoothed array (reading N1-a)."""
+    rho = np.ascontiguousarray(np.asarray(rho, dtype=np.int64))
+    out = np.zeros_like(rho)
+    lib().orc_smooth121(nc, bc, _p(rho, c_i64p), _p(out, c_i64p))
+    return out
 
 
 class Oracle:
@@ -249,6 +263,26 @@ class Oracle:
     def rho(self):
         r = np.zeros(self.ng, np.int64)
         lib().orc_get_rho(self.h, _p(r, c_i64p))
+        return r
+
+    def set_smoothing(self, passes: int):
+        lib().orc_set_smoothing(self.h, int(passes))
+
+    def set_averaging(self, window: int, interval: int):
+        assert lib().orc_set_averaging(self.h, int(window), int(interval)) == 0
+
+    def average(self):
+        """Latest latched window: (dens_sum[ns, ng] int64, phi_sum[nc+1], count, step)."""
+        d = np.zeros((self.ns, self.ng), np.int64)
+        f = np.zeros(self.nc + 1)
+        cnt = np.zeros(1, np.uint64)
+        st = np.zeros(1, np.uint64)
+        lib().orc_get_average(self.h, _p(d, c_i64p), _p(f, c_f64p), _p(cnt, c_u64p), _p(st, c_u64p))
+        return d, f, int(cnt[0]), int(st[0])
+
+    def rho_smoothed(self):
+        r = np.zeros(self.ng, np.int64)
+        lib().orc_get_rho_smoothed(self.h, _p(r, c_i64p))
         return r
 
     def dens(self):

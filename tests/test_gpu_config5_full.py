@@ -1,0 +1,108 @@
+"""BASELINE.json configs[4] at FULL size (1e9 particles, 1 048 576 cells, 100 steps, pinned-host checkpoint every
+50 steps, restart leg compared bit for bit).
+
+Opt-in (BIT1_FULL_C5=1): it needs ~130 GB of HBM, ~130 GB of host memory and about ten minutes, which does not
+belong in the default `pytest -m gpu` run.  The result of the run made for this round is recorded in
+profiles/r1d_config5_full.md.  State digests are taken array by array (8 GB at a time) through the C ABI."""
+import ctypes as C
+import hashlib
+import json
+import os
+import time
+
+import numpy as np
+import pytest
+
+from paper_2606_28534_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+FULL = os.environ.get("BIT1_FULL_C5") == "1"
+
+
+def _digest(g):
+    """blake2b of every live array, fetched one at a time with bit1_get_particles (other pointers null)."""
+    n = g.n_live()
+    out = {"n": n}
+    order = ["x", "vx", "vy", "vz", "cell", "pid", "sp"]
+    dt = dict(x=np.float64, vx=np.float64, vy=np.float64, vz=np.float64, cell=np.int32, pid=np.uint32, sp=np.uint8)
+    for i, k in enumerate(order):
+        a = np.empty(n, dt[k])
+        args = [None] * 8
+        args[i] = a.ctypes.data
+        s = g.lib.bit1_get_particles(g.h, *args)
+        assert s == 0, f"bit1_get_particles({k}) -> {s}"
+        out[k] = hashlib.blake2b(a.data, digest_size=16).hexdigest()
+        del a
+    for k, a in (("rho", g.get_rho()), ("dens", g.get_dens()), ("E", g.get_E()), ("phi", g.get_phi())):
+        out[k] = hashlib.blake2b(np.ascontiguousarray(a).data, digest_size=16).hexdigest()
+    m = g.get_moments()
+    out["scalars"] = [m["step"], m["next_pid"], m["births"], m["reinject"], m["flags"], m["rho_total"],
+                      m["wall_charge"].tolist(), m["wall_count"].tolist(), m["events"].tolist()]
+    return out, m
+
+
+@pytest.mark.skipif(not FULL, reason="set BIT1_FULL_C5=1 (about 130 GB HBM, 130 GB host RAM, ten minutes)")
+def test_config5_full_size_checkpoint_every_50_steps_and_bit_identical_restart():
+    import torch
+    from paper_2606_28534_b200.binding import Bit1
+
+    t0 = time.time()
+    w = W.make_config(5)
+    t_gen = time.time() - t0
+    g = Bit1(w, checkpoint_staging=True)
+    t0 = time.time()
+    g.load()
+    g.sync()
+    t_load = time.time() - t0
+    n0 = w.n
+    w.x = w.vx = w.vy = w.vz = w.sp = None   # the library copied them
+
+    blob = torch.empty(g.checkpoint_size(), dtype=torch.uint8).pin_memory()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    cs = g.compute_stream
+    g.step(3)   # warm-up (part of the 100)
+    ev[0].record(cs)
+    g.step(47)
+    ev[1].record(cs)
+    t0 = time.time()
+    g.checkpoint(blob)          # step 50: D2D snapshot on the compute stream, D2H on the side stream
+    ev[2].record(cs)
+    g.step(50)                  # overlaps the 42 GB copy to pinned host memory
+    ev[3].record(cs)
+    g.sync()
+    t_steps_with_ckpt = time.time() - t0
+    g.checkpoint_wait()
+    t_ckpt_done = time.time() - t0
+    ms_a = ev[0].elapsed_time(ev[1]) / 47
+    ms_snap = ev[1].elapsed_time(ev[2])
+    ms_b = ev[2].elapsed_time(ev[3]) / 50
+    want, m = _digest(g)
+    assert m["step"] == 100 and m["flags"] == 0
+    assert want["n"] == n0 + m["births"]
+    far = m["far_movers"] / 100
+    g.close()
+    del g
+    torch.cuda.empty_cache()
+
+    h = Bit1(w, checkpoint_staging=True)   # fresh context, as after a crash
+    t0 = time.time()
+    h.restart(blob)
+    t_restart = time.time() - t0
+    assert h.get_moments()["step"] == 50
+    h.step(50)
+    h.sync()
+    got, m2 = _digest(h)
+    h.close()
+    report = {"particles": n0, "cells": w.nc, "gen_s": t_gen, "load_s": t_load,
+              "ms_per_step_plain": ms_a, "ms_per_step_during_checkpoint_d2h": ms_b, "snapshot_d2d_ms": ms_snap,
+              "particle_steps_per_s_plain": n0 / (ms_a * 1e-3),
+              "particle_steps_per_s_during_d2h": n0 / (ms_b * 1e-3),
+              "checkpoint_bytes": int(blob.numel()), "steps_50_wall_s": t_steps_with_ckpt,
+              "checkpoint_complete_wall_s": t_ckpt_done, "restart_s": t_restart, "births": m["births"],
+              "far_movers_per_step": far, "n_final": want["n"], "bit_identical": got == want}
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open("gpurun_out/config5_full.json", "w") as f:
+        json.dump(report, f, indent=1)
+    print(json.dumps(report))
+    assert got == want, "restarted run differs from the uninterrupted one"
