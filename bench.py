@@ -7,7 +7,7 @@ One "step" is one whole timestep (mover, side-list ordering + cell scan, arrange
 solve) over every particle of the workload.  Default workload: BASELINE.json configs[3] (2e8 particles, 65536
 cells, exponential sheath profile, 3 species, config-3 collisions) -- the first configuration at the
 "1e8+ particles" size that the metric's HBM target is quoted on; configs[4] (1e9) also fits one GPU but its
-41 GB host-side generation does not fit a default run of a few minutes (use --config 5 --device-gen).
+host-side generation and load take several minutes (python bench.py --config 5 --steps 10 runs it).
 Inputs are larger than L2 (8.2 GB state vs 126 MB), so no L2 flush is needed between steps.
 
 The path does not shard (BASELINE.json north_star: no multi-GPU sharding or collectives): --gpus N runs N
@@ -307,7 +307,7 @@ def run_cuda(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--scale", type=float, default=1.0)

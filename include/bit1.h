@@ -104,7 +104,8 @@ typedef struct {
   void *compute_stream;    /* cudaStream_t, borrowed; NULL = default stream */
   void *side_stream;       /* cudaStream_t for checkpoint device->host copies; NULL = compute stream */
   int32_t checkpoint_staging; /* 1: reserve a device snapshot area so bit1_checkpoint overlaps later steps */
-  int32_t variant;         /* 0 default; 1 = in-place push then scatter ("V1"); 2 = recompute in the scatter pass ("V2") */
+  int32_t variant;         /* 0 default; 1 = in-place push then scatter ("V1"); 2 = recompute in the scatter pass ("V2");
+                              3 = V2 without CTA barriers in the particle passes ("V3") */
 } bit1_options;
 
 typedef struct {
@@ -156,6 +157,25 @@ bit1_status bit1_get_moments(bit1_ctx *ctx, bit1_moments *out);
 /* Any pointer may be NULL.  n_live entries each (bit1_get_count), cell_start nc+1 entries. */
 bit1_status bit1_get_particles(bit1_ctx *ctx, double *x, double *vx, double *vy, double *vz,
                                int32_t *cell, uint32_t *pid, uint8_t *species, int64_t *cell_start_or_null);
+
+/* Density smoothing ("density smoothing", "smoothing operators"; SURVEY 8(f) NEXT-1;
+ * DESIGN.md reading N1-a): `passes` (0..8, 0 = off) passes of the 1-2-1 binomial filter over rho before every
+ * field solve, in exact integers (each pass yields 4 x the smoothed array; the 1/4 is folded into the field
+ * constants).  Periodic: indices wrap; bounded: the quarter that would cross a wall stays on the wall node, so
+ * total charge is conserved.  bit1_get_rho / bit1_get_dens keep returning the raw deposit; bit1_get_rho_smoothed
+ * returns 4^passes x the smoothed array the last solve used (HOST, ng entries).  Takes effect at the next step. */
+bit1_status bit1_set_smoothing(bit1_ctx *ctx, int passes);
+bit1_status bit1_get_rho_smoothed(bit1_ctx *ctx, int64_t *rho_s_fixed);
+/* Time-averaged diagnostics (Table 2: datfile, mvflag = window, mvStep = interval; DESIGN.md
+ * reading N1-b): over the last `window` steps of every `interval` steps (step counter k, r = k mod interval read
+ * as interval when 0, accumulate when r > interval - window) the per-species deposited charge (int64, exact) and
+ * phi (fp64, summed in step order) are accumulated on the device; at r == interval the sums are latched and
+ * cleared.  window = 0 switches it off; (re)arming clears all sums.  BIT1_ERR_INVALID_ARG unless
+ * 0 <= window <= interval (interval ignored when window == 0).  bit1_get_average returns the latest latched
+ * sums (HOST: nspecies*ng int64, nc+1 doubles), how many steps they hold and the step counter at the latch
+ * (all zero before the first latch).  The sums are part of the checkpoint. */
+bit1_status bit1_set_averaging(bit1_ctx *ctx, int window, int interval);
+bit1_status bit1_get_average(bit1_ctx *ctx, int64_t *dens_sum, double *phi_sum, uint64_t *count, uint64_t *step);
 
 /* Test hook: overwrite E (HOST, nc+1 entries) and optionally freeze the field solve (E stays as set
  * while rho keeps being deposited) -- used by closed-form push tests. */

@@ -640,7 +640,12 @@ void orc_phase_push(orc *o) {
           if (chosen < 0 && r < cum) chosen = 0;
         }
         if (fl & F_IONISE) {
-          cum = cum + (o->n0 * sigma_lookup(o, o->sig_ion, EeV)) * g;
+          /* DESIGN.md reading R-thr: the ionisation cross-section is the table value above the threshold and
+           * zero at or below it.  A table that is linear between nodes is positive on the whole interval that
+           * holds the threshold (13.5..14.0 eV for SURVEY's 0.5 eV table), and an ionisation picked there would
+           * share out a negative energy E - E_ion (sqrt of a negative number: NaN velocities). */
+          double sig_i = EeV > o->E_ion ? sigma_lookup(o, o->sig_ion, EeV) : 0.0;
+          cum = cum + (o->n0 * sig_i) * g;
           if (chosen < 0 && r < cum) chosen = 1;
         }
         if (fl & F_CX) {

@@ -89,6 +89,14 @@ def load_library(path: Optional[str] = None):
     L.bit1_get_moments.argtypes = [vp, C.POINTER(bit1_moments)]
     L.bit1_get_particles.restype = C.c_int
     L.bit1_get_particles.argtypes = [vp] + [vp] * 8
+    L.bit1_set_smoothing.restype = C.c_int
+    L.bit1_set_smoothing.argtypes = [vp, C.c_int]
+    L.bit1_get_rho_smoothed.restype = C.c_int
+    L.bit1_get_rho_smoothed.argtypes = [vp, vp]
+    L.bit1_set_averaging.restype = C.c_int
+    L.bit1_set_averaging.argtypes = [vp, C.c_int, C.c_int]
+    L.bit1_get_average.restype = C.c_int
+    L.bit1_get_average.argtypes = [vp, vp, vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     L.bit1_set_E.restype = C.c_int
     L.bit1_set_E.argtypes = [vp, vp, C.c_int]
     L.bit1_set_step.restype = C.c_int
@@ -300,6 +308,27 @@ class Bit1:
         if cell_start:
             d["cell_start"] = cs
         return d
+
+    # -- NEXT-1: density smoothing, time-averaged diagnostics ----------------------------------
+    def set_smoothing(self, passes: int):
+        _check(self.lib.bit1_set_smoothing(self.h, int(passes)), "bit1_set_smoothing")
+
+    def get_rho_smoothed(self):
+        r = np.zeros(self.ng, np.int64)
+        _check(self.lib.bit1_get_rho_smoothed(self.h, r.ctypes.data), "bit1_get_rho_smoothed")
+        return r
+
+    def set_averaging(self, window: int, interval: int):
+        _check(self.lib.bit1_set_averaging(self.h, int(window), int(interval)), "bit1_set_averaging")
+
+    def get_average(self):
+        """Latest latched window: (dens_sum[ns, ng] int64, phi_sum[nc+1], count, step)."""
+        d = np.zeros((self.ns, self.ng), np.int64)
+        f = np.zeros(self.nc + 1)
+        cnt, st = C.c_uint64(), C.c_uint64()
+        _check(self.lib.bit1_get_average(self.h, d.ctypes.data, f.ctypes.data, C.byref(cnt), C.byref(st)),
+               "bit1_get_average")
+        return d, f, int(cnt.value), int(st.value)
 
     def set_E(self, E, freeze_field: bool = True):
         E = _f8(E)

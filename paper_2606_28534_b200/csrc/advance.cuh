@@ -93,7 +93,9 @@ __device__ __noinline__ void collide(const Params& P, const SpeciesP* S, unsigne
     if (chosen < 0 && r < cum) chosen = 0;
   }
   if (fl & kIonise) {
-    cum = cum + (P.n0 * sigma_lookup(P, P.sig_ion, EeV)) * g;
+    // reading R-thr: zero at or below the threshold, whatever the table interpolates to there
+    const double sig_i = EeV > P.E_ion ? sigma_lookup(P, P.sig_ion, EeV) : 0.0;
+    cum = cum + (P.n0 * sig_i) * g;
     if (chosen < 0 && r < cum) chosen = 1;
   }
   if (fl & kCx) {

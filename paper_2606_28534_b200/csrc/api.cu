@@ -24,7 +24,7 @@ constexpr int kMaxSig = 16384;
 constexpr int kMaxNorm = 1 << 20;
 constexpr int kMaxR = 4;
 constexpr size_t kAlign = 256;
-constexpr uint32_t kCkptVersion = 1;
+constexpr uint32_t kCkptVersion = 2;   // 2: + averaging sums (NEXT-1)
 
 // sort window radius in cells (reading R-win); BIT1_WINDOW_R overrides it for the tests
 inline int window_R() {
@@ -69,21 +69,26 @@ Particles part_at(void* base, const PartLayout& l) {
   return p;
 }
 
+// running + latched sums of the time-averaged diagnostics, one contiguous block:
+// acc_dens[ns*ng] | avg_dens[ns*ng] (int64) | acc_phi[nc+1] | avg_phi[nc+1] (fp64)
+size_t avg_bytes(int nc, int ng, int ns) { return 2 * ((size_t)ns * ng + (size_t)(nc + 1)) * 8; }
+
 struct CkptLayout {
-  size_t header, state, cell_start, part, bytes;
+  size_t header, state, cell_start, avg, part, bytes;
 };
-CkptLayout ckpt_layout(int nc, size_t cap) {
+CkptLayout ckpt_layout(int nc, int ng, int ns, size_t cap) {
   CkptLayout c;
   c.header = 0;
   c.state = 256;
   c.cell_start = c.state + align_up(sizeof(DevState));
-  c.part = c.cell_start + align_up((size_t)(nc + 1) * 4);
+  c.avg = c.cell_start + align_up((size_t)(nc + 1) * 4);
+  c.part = c.avg + align_up(avg_bytes(nc, ng, ns));
   c.bytes = c.part + part_layout(cap).bytes;
   return c;
 }
 
 struct Layout {
-  size_t st, tables, dens, rho, phi, E, cell_count, cell_start, cell_start_old, scan_part, coop_scratch, cell_base, ovf_before, tile_hist, tile_base, tile_pre, evt,
+  size_t st, tables, dens, rho, rho_s, rho_t, avg, phi, E, cell_count, cell_start, cell_start_old, scan_part, coop_scratch, cell_base, ovf_before, tile_hist, tile_base, tile_pre, evt,
       ovf_key, ovf_idx, ovf_dst, tmp_key, tmp_idx, ovf_rec, part[2], scratch, mom, total;
   unsigned ovf_cap, ovf_pow2;
   int max_tiles, ng;
@@ -105,6 +110,9 @@ Layout make_layout(int nc, int bc, int ns, size_t cap, int staging) {
   l.tables = take(((size_t)3 * kMaxSig + kMaxNorm + 1) * 8);
   l.dens = take((size_t)ns * l.ng * 8);
   l.rho = take((size_t)l.ng * 8);
+  l.rho_s = take((size_t)l.ng * 8);
+  l.rho_t = take((size_t)l.ng * 8);
+  l.avg = take(avg_bytes(nc, l.ng, ns));
   l.phi = take((size_t)(nc + 1) * 8);
   l.E = take((size_t)(nc + 4) * 8);  // the E window of a tile is copied in 16-byte units
   l.cell_count = take((size_t)nc * 4);
@@ -130,7 +138,7 @@ Layout make_layout(int nc, int bc, int ns, size_t cap, int staging) {
   l.part[1] = take(pl.bytes);
   l.scratch_bytes = load_scratch_bytes((unsigned)cap);
   if (staging) {
-    const size_t cb = ckpt_layout(nc, cap).bytes;
+    const size_t cb = ckpt_layout(nc, l.ng, ns, cap).bytes;
     if (cb > l.scratch_bytes) l.scratch_bytes = cb;
   }
   l.scratch = take(l.scratch_bytes);
@@ -299,6 +307,12 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   P.sig_el = tab; P.sig_ion = tab + kMaxSig; P.sig_cx = tab + 2 * kMaxSig; P.inv_norm = tab + 3 * kMaxSig;
   P.dens = reinterpret_cast<long long*>(ws + lay.dens);
   P.rho = reinterpret_cast<long long*>(ws + lay.rho);
+  P.rho_s = reinterpret_cast<long long*>(ws + lay.rho_s);
+  P.rho_t = reinterpret_cast<long long*>(ws + lay.rho_t);
+  P.acc_dens = reinterpret_cast<long long*>(ws + lay.avg);
+  P.avg_dens = P.acc_dens + (size_t)ns * lay.ng;
+  P.acc_phi = reinterpret_cast<double*>(P.avg_dens + (size_t)ns * lay.ng);
+  P.avg_phi = P.acc_phi + (g->nc + 1);
   P.phi = reinterpret_cast<double*>(ws + lay.phi);
   P.E = reinterpret_cast<double*>(ws + lay.E);
   P.cell_count = reinterpret_cast<int*>(ws + lay.cell_count);
@@ -400,6 +414,53 @@ static bit1_status read_state(bit1_ctx* c, DevState* h) {
   return BIT1_OK;
 }
 
+// The NEXT-1 settings live in the host-side Params (the launches read them) and ride along in DevState so that a
+// checkpoint carries them; clear_sums also zeroes the running and latched averaging sums.
+static bit1_status push_settings(bit1_ctx* c, bool clear_sums) {
+  const int v[4] = {c->P.smooth, c->P.avg_window, c->P.avg_interval, 0};
+  CUDA_OK(cudaMemcpyAsync(&c->P.st->smooth_passes, v, sizeof(v), cudaMemcpyHostToDevice, c->cs));
+  if (clear_sums) {
+    CUDA_OK(cudaMemsetAsync(c->P.acc_dens, 0, avg_bytes(c->P.nc, c->P.ng, c->P.ns), c->cs));
+    CUDA_OK(cudaMemsetAsync(&c->P.st->acc_count, 0, 3 * sizeof(unsigned long long), c->cs));
+  }
+  CUDA_OK(cudaStreamSynchronize(c->cs));   // v is a stack object
+  return BIT1_OK;
+}
+
+bit1_status bit1_set_smoothing(bit1_ctx* c, int passes) {
+  if (!c || passes < 0 || passes > 8) return BIT1_ERR_INVALID_ARG;
+  c->P.smooth = passes;
+  return push_settings(c, false);
+}
+
+bit1_status bit1_set_averaging(bit1_ctx* c, int window, int interval) {
+  if (!c || window < 0 || (window > 0 && interval < window)) return BIT1_ERR_INVALID_ARG;
+  c->P.avg_window = window;
+  c->P.avg_interval = window > 0 ? interval : 0;
+  return push_settings(c, true);
+}
+
+bit1_status bit1_get_rho_smoothed(bit1_ctx* c, int64_t* out) {
+  if (!c || !out) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  CUDA_OK(cudaMemcpyAsync(out, c->P.smooth > 0 ? c->P.rho_s : c->P.rho, (size_t)c->P.ng * 8, cudaMemcpyDeviceToHost, c->cs));
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  return BIT1_OK;
+}
+
+bit1_status bit1_get_average(bit1_ctx* c, int64_t* dens_sum, double* phi_sum, uint64_t* count, uint64_t* step) {
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  if (dens_sum) CUDA_OK(cudaMemcpyAsync(dens_sum, c->P.avg_dens, (size_t)c->P.ns * c->P.ng * 8, cudaMemcpyDeviceToHost, c->cs));
+  if (phi_sum) CUDA_OK(cudaMemcpyAsync(phi_sum, c->P.avg_phi, (size_t)(c->P.nc + 1) * 8, cudaMemcpyDeviceToHost, c->cs));
+  DevState h;
+  CUDA_OK(cudaMemcpyAsync(&h, c->P.st, sizeof(DevState), cudaMemcpyDeviceToHost, c->cs));
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  if (count) *count = h.avg_count;
+  if (step) *step = h.avg_step;
+  return BIT1_OK;
+}
+
 bit1_status bit1_load_particles(bit1_ctx* c, uint64_t n, const double* x, const double* vx, const double* vy,
                                 const double* vz, const uint8_t* sp, const uint32_t* pid, int on_device) {
   if (!c || (n && (!x || !vx || !vy || !vz || !sp))) return BIT1_ERR_INVALID_ARG;
@@ -408,6 +469,7 @@ bit1_status bit1_load_particles(bit1_ctx* c, uint64_t n, const double* x, const 
   const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   Particles in = c->buf[1], outp = c->buf[0];
   CUDA_OK(cudaMemsetAsync(c->P.st, 0, sizeof(DevState), c->cs));
+  { bit1_status ps = push_settings(c, true); if (ps != BIT1_OK) return ps; }
   if (n) {
     CUDA_OK(cudaMemcpyAsync(in.x, x, n * 8, kind, c->cs));
     CUDA_OK(cudaMemcpyAsync(in.vx, vx, n * 8, kind, c->cs));
@@ -648,13 +710,13 @@ bit1_status bit1_set_step(bit1_ctx* c, uint64_t step) {
 
 size_t bit1_checkpoint_size(bit1_ctx* c) {
   if (!c) return 0;
-  return ckpt_layout(c->P.nc, c->P.capacity).bytes;
+  return ckpt_layout(c->P.nc, c->P.ng, c->P.ns, c->P.capacity).bytes;
 }
 
 bit1_status bit1_checkpoint(bit1_ctx* c, void* host, size_t cap, size_t* written) {
   if (!c || !host) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
-  const CkptLayout cl = ckpt_layout(c->P.nc, c->P.capacity);
+  const CkptLayout cl = ckpt_layout(c->P.nc, c->P.ng, c->P.ns, c->P.capacity);
   if (cap < cl.bytes) return BIT1_ERR_CAPACITY;
   const PartLayout pl = part_layout(c->P.capacity);
   CkptHeader hd;
@@ -672,6 +734,7 @@ bit1_status bit1_checkpoint(bit1_ctx* c, void* host, size_t cap, size_t* written
     char* sg = c->ws + c->lay.scratch;
     CUDA_OK(cudaMemcpyAsync(sg + cl.state, c->P.st, sizeof(DevState), cudaMemcpyDeviceToDevice, c->cs));
     CUDA_OK(cudaMemcpyAsync(sg + cl.cell_start, c->P.cell_start, (size_t)(c->P.nc + 1) * 4, cudaMemcpyDeviceToDevice, c->cs));
+    CUDA_OK(cudaMemcpyAsync(sg + cl.avg, c->P.acc_dens, avg_bytes(c->P.nc, c->P.ng, c->P.ns), cudaMemcpyDeviceToDevice, c->cs));
     CUDA_OK(cudaMemcpyAsync(sg + cl.part, live, pl.bytes, cudaMemcpyDeviceToDevice, c->cs));
     CUDA_OK(cudaEventRecord(c->ev_snap, c->cs));
     CUDA_OK(cudaStreamWaitEvent(c->ss, c->ev_snap, 0));
@@ -680,6 +743,7 @@ bit1_status bit1_checkpoint(bit1_ctx* c, void* host, size_t cap, size_t* written
   } else {
     CUDA_OK(cudaMemcpyAsync(hb + cl.state, c->P.st, sizeof(DevState), cudaMemcpyDeviceToHost, c->cs));
     CUDA_OK(cudaMemcpyAsync(hb + cl.cell_start, c->P.cell_start, (size_t)(c->P.nc + 1) * 4, cudaMemcpyDeviceToHost, c->cs));
+    CUDA_OK(cudaMemcpyAsync(hb + cl.avg, c->P.acc_dens, avg_bytes(c->P.nc, c->P.ng, c->P.ns), cudaMemcpyDeviceToHost, c->cs));
     CUDA_OK(cudaMemcpyAsync(hb + cl.part, live, pl.bytes, cudaMemcpyDeviceToHost, c->cs));
     CUDA_OK(cudaEventRecord(c->ev_done, c->cs));
   }
@@ -699,7 +763,7 @@ bit1_status bit1_checkpoint_wait(bit1_ctx* c) {
 
 bit1_status bit1_restart(bit1_ctx* c, const void* blob, size_t bytes) {
   if (!c || !blob) return BIT1_ERR_INVALID_ARG;
-  const CkptLayout cl = ckpt_layout(c->P.nc, c->P.capacity);
+  const CkptLayout cl = ckpt_layout(c->P.nc, c->P.ng, c->P.ns, c->P.capacity);
   if (bytes < cl.bytes) return BIT1_ERR_CHECKPOINT;
   CkptHeader hd;
   memcpy(&hd, blob, sizeof(hd));
@@ -714,8 +778,12 @@ bit1_status bit1_restart(bit1_ctx* c, const void* blob, size_t bytes) {
   if (h.n > c->P.capacity) return BIT1_ERR_CHECKPOINT;
   h.ovf_count = 0; h.ovf_valid = 0; h.freeze_field = 0; h.load_error = 0; h.n_next = h.n;
   CUDA_OK(cudaStreamSynchronize(c->cs));
+  if (h.smooth_passes < 0 || h.smooth_passes > 8 || h.avg_window < 0 || h.avg_interval < h.avg_window)
+    return BIT1_ERR_CHECKPOINT;
   CUDA_OK(cudaMemcpyAsync(c->P.st, &h, sizeof(DevState), cudaMemcpyHostToDevice, c->cs));
   CUDA_OK(cudaStreamSynchronize(c->cs));  // h is a stack object
+  c->P.smooth = h.smooth_passes; c->P.avg_window = h.avg_window; c->P.avg_interval = h.avg_interval;
+  CUDA_OK(cudaMemcpyAsync(c->P.acc_dens, hb + cl.avg, avg_bytes(c->P.nc, c->P.ng, c->P.ns), cudaMemcpyHostToDevice, c->cs));
   c->cur = 0;
   CUDA_OK(cudaMemcpyAsync(c->ws + c->lay.part[0], hb + cl.part, pl.bytes, cudaMemcpyHostToDevice, c->cs));
   c->launches += launch_rebuild(c->P, c->buf[0], c->cs);

@@ -83,6 +83,9 @@ struct DevState {
   unsigned long long events[kMaxSpecies][3];
   unsigned long long far_movers, max_far_movers;
   long long rho_total;
+  // NEXT-1: settings ride along so that a checkpoint carries them; the running/latched window counters
+  int smooth_passes, avg_window, avg_interval, pad_;
+  unsigned long long acc_count, avg_count, avg_step;
 };
 
 struct Params {
@@ -105,6 +108,12 @@ struct Params {
   long long *dens;  // ns * ng
   long long *rho;   // ng
   double *phi, *E;  // nc + 1
+  // NEXT-1 (density smoothing, time-averaged diagnostics; readings N1-a, N1-b)
+  int smooth;                    // passes of the 1-2-1 filter over rho before the field solve (0 = off)
+  int avg_window, avg_interval;  // mvflag, mvStep (0 = off)
+  long long *rho_s, *rho_t;      // ng each: 4^smooth x smoothed rho (what the solve used), ping-pong scratch
+  long long *acc_dens, *avg_dens;  // ns * ng: running / latched sums of dens over the averaging window
+  double *acc_phi, *avg_phi;       // nc + 1
   int *cell_count;  // nc
   int *cell_start;  // nc + 1: of the arrangement this step produces (k_mid)
   int *cell_start_old;  // nc + 1: of the arrangement this step reads (swapped with cell_start every step)

@@ -598,12 +598,13 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     unsigned* s_dens = s_dens2 + (it & 1) * kDensWords;
     const unsigned base = (unsigned)tile * kTile;
     const unsigned cnt = min((unsigned)kTile, n - base);
-    const int2 d = S->d;
-    const TileWin tw = make_window(d.x, d.y, P.R);
     int2 dn = make_int2(0, 0);
     const int tnext = tile + 2 * G;
     if (threadIdx.x == 0 && tnext < ntiles) dn = cur.desc[tnext];
     mbar_wait(&bar[it & 1], (unsigned)(it >> 1) & 1u);
+    // the stage's descriptor is only valid once its barrier has completed (variant 3 has no CTA barrier in between)
+    const int2 d = S->d;
+    const TileWin tw = make_window(d.x, d.y, P.R);
 
     // destination of this warp's first particle of every window cell
     if (VARIANT == 3) {
@@ -884,8 +885,9 @@ __device__ i128 block_sum_128(i128 v, i128* s_warp) {
 // (returns A = sum of R_j and C = sum of the local inclusive prefixes, so that T_{j_hi+1} = T_{j_lo} +
 // len * S_{j_lo-1} + C); APPLY = true: writes phi_j and E_j.
 template <bool APPLY>
-__device__ void field_range(const Params& P, int j_lo, int j_hi, i128 tot, i128 Tn, i128 carryS, i128 carryT,
-                            i128* s_warp, i128* outA, i128* outC) {
+__device__ void field_range(const Params& P, const long long* __restrict__ R_in, double Kphi, double KE, int j_lo,
+                            int j_hi, i128 tot, i128 Tn, i128 carryS, i128 carryT, i128* s_warp, i128* outA,
+                            i128* outC) {
   const int nc = P.nc, bc = P.bc;
   const i128 S0 = carryS;
   i128 accC = 0;
@@ -897,7 +899,7 @@ __device__ void field_range(const Params& P, int j_lo, int j_hi, i128 tot, i128 
     for (int k = 0; k < kFieldItems; ++k) {
       const int j = jb + k;
       i128 r = 0;
-      if (j <= j_hi) r = bc ? (i128)P.rho[j] : (i128)nc * (i128)P.rho[j] - tot;
+      if (j <= j_hi) r = bc ? (i128)R_in[j] : (i128)nc * (i128)R_in[j] - tot;
       R[k] = r;
       run += r;
       Sl[k] = run;  // inclusive local
@@ -919,12 +921,12 @@ __device__ void field_range(const Params& P, int j_lo, int j_hi, i128 tot, i128 
         const int j = jb + k;
         if (j <= j_hi) {
           const i128 Sj = Sl[k], Sm = Sl[k] - R[k];
-          P.phi[j] = P.Kphi * dbl128((i128)j * Tn - (i128)nc * T);
+          P.phi[j] = Kphi * dbl128((i128)j * Tn - (i128)nc * T);
           if (bc) {
-            if (j < nc) P.E[j] = P.KE * dbl128((i128)nc * (Sm + Sj) - 2 * Tn);
-            else P.E[nc] = P.KE * dbl128(2 * (i128)nc * Sm - 2 * Tn + 2 * (i128)nc * (i128)P.rho[nc]);
+            if (j < nc) P.E[j] = KE * dbl128((i128)nc * (Sm + Sj) - 2 * Tn);
+            else P.E[nc] = KE * dbl128(2 * (i128)nc * Sm - 2 * Tn + 2 * (i128)nc * (i128)R_in[nc]);
           } else {
-            P.E[j] = P.KE * dbl128((i128)nc * (Sm + Sj) - 2 * Tn);
+            P.E[j] = KE * dbl128((i128)nc * (Sm + Sj) - 2 * Tn);
           }
           T += Sj;
         }
@@ -952,14 +954,56 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
   const int G = gridDim.x, b = blockIdx.x;
   DevState* st = P.st;
   i128* part = reinterpret_cast<i128*>(P.coop_scratch);  // [4][G]: tot, wsum, A, C
-  // phase A
+  // phase A: rho, then (NEXT-1, reading N1-a) `smooth` passes of the exact-integer 1-2-1 filter, then the two
+  // plain reductions over the array the solve uses
+  const int smooth = P.smooth;
+  const long long* R = P.rho;
+  double Kphi = P.Kphi, KE = P.KE;
   i128 tot = 0, wsum = 0;
-  for (int j = b * kFieldThreads + (int)threadIdx.x; j < ng; j += G * kFieldThreads) {
-    long long r = 0;
-    for (int s = 0; s < P.ns; ++s) r += (long long)P.sp[s].sign * P.dens[(size_t)s * ng + j];
-    P.rho[j] = r;
-    tot += (i128)r;
-    if (j >= 1 && j <= nc - 1) wsum += (i128)(nc - j) * (i128)r;
+  if (smooth > 0) {
+    for (int j = b * kFieldThreads + (int)threadIdx.x; j < ng; j += G * kFieldThreads) {
+      long long r = 0;
+      for (int s = 0; s < P.ns; ++s) r += (long long)P.sp[s].sign * P.dens[(size_t)s * ng + j];
+      P.rho[j] = r;
+    }
+    const long long* in = P.rho;
+    for (int k = 0; k < smooth; ++k) {
+      long long* out = ((smooth - 1 - k) & 1) ? P.rho_t : P.rho_s;   // the last pass lands in rho_s
+      __threadfence();
+      grid.sync();
+      for (int j = b * kFieldThreads + (int)threadIdx.x; j < ng; j += G * kFieldThreads) {
+        long long v;
+        if (bc) {
+          if (j == 0) v = 3 * in[0] + in[1];
+          else if (j == nc) v = in[nc - 1] + 3 * in[nc];
+          else v = in[j - 1] + 2 * in[j] + in[j + 1];
+        } else {
+          const int jm = j == 0 ? nc - 1 : j - 1, jp = j == nc - 1 ? 0 : j + 1;
+          v = in[jm] + 2 * in[j] + in[jp];
+        }
+        out[j] = v;
+      }
+      in = out;
+    }
+    __threadfence();
+    grid.sync();
+    R = P.rho_s;
+    const double scale = 1.0 / (double)(1ll << (2 * smooth));   // exact power of two
+    Kphi = Kphi * scale;
+    KE = KE * scale;
+    for (int j = b * kFieldThreads + (int)threadIdx.x; j < ng; j += G * kFieldThreads) {
+      const long long r = R[j];
+      tot += (i128)r;
+      if (j >= 1 && j <= nc - 1) wsum += (i128)(nc - j) * (i128)r;
+    }
+  } else {
+    for (int j = b * kFieldThreads + (int)threadIdx.x; j < ng; j += G * kFieldThreads) {
+      long long r = 0;
+      for (int s = 0; s < P.ns; ++s) r += (long long)P.sp[s].sign * P.dens[(size_t)s * ng + j];
+      P.rho[j] = r;
+      tot += (i128)r;
+      if (j >= 1 && j <= nc - 1) wsum += (i128)(nc - j) * (i128)r;
+    }
   }
   tot = block_sum_128(tot, s_warp);
   wsum = block_sum_128(wsum, s_warp);
@@ -970,7 +1014,7 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
   for (int i = threadIdx.x; i < G; i += kFieldThreads) { tot += part[i]; wsum += part[G + i]; }
   tot = block_sum_128(tot, s_warp);
   wsum = block_sum_128(wsum, s_warp);
-  if (b == 0 && threadIdx.x == 0) st->rho_total = (long long)tot;
+  if (b == 0 && threadIdx.x == 0) st->rho_total = (long long)(tot >> (2 * smooth));   // the filter conserves charge
   const bool frozen = st->freeze_field != 0;
   if (!frozen) {
     // periodic: R'_j = nc R_j - tot  =>  T_nc' = nc * wsum - tot * nc (nc - 1) / 2
@@ -983,7 +1027,7 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
     const int j_lo = min(1 + b * per, jmax + 1), j_hi = min(j_lo + per - 1, jmax);
     // phase B
     i128 A = 0, C = 0;
-    field_range<false>(P, j_lo, j_hi, tot, Tn, (i128)0, (i128)0, s_warp, &A, &C);
+    field_range<false>(P, R, Kphi, KE, j_lo, j_hi, tot, Tn, (i128)0, (i128)0, s_warp, &A, &C);
     if (threadIdx.x == 0) { part[2 * G + b] = A; part[3 * G + b] = C; }
     __threadfence();
     grid.sync();
@@ -1004,23 +1048,55 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
     const i128 Send = block_sum_128(myA, s_warp);                                    // S_jmax
     if (b == 0 && threadIdx.x == 0) {
       // node 0
-      P.phi[0] = P.Kphi * dbl128((i128)0);
+      P.phi[0] = Kphi * dbl128((i128)0);
       if (bc) {
-        P.E[0] = P.KE * dbl128(-2 * Tn - 2 * (i128)nc * (i128)P.rho[0]);
+        P.E[0] = KE * dbl128(-2 * Tn - 2 * (i128)nc * (i128)R[0]);
       } else {
         // periodic: S_{-1} = S_{nc-1}, S_0 = 0; ghosts at nc
-        P.E[0] = P.KE * dbl128((i128)nc * (Send + (i128)0) - 2 * Tn);
+        P.E[0] = KE * dbl128((i128)nc * (Send + (i128)0) - 2 * Tn);
         P.E[nc] = P.E[0];
         P.phi[nc] = P.phi[0];
       }
     }
-    field_range<true>(P, j_lo, j_hi, tot, Tn, carryS, carryT, s_warp, nullptr, nullptr);
+    field_range<true>(P, R, Kphi, KE, j_lo, j_hi, tot, Tn, carryS, carryT, s_warp, nullptr, nullptr);
   }
   if (b == 0 && threadIdx.x == 0) {
     st->n = st->n_next;
     if (commit_step) st->step += 1ull;
     st->ovf_count = 0;
     st->ovf_valid = 0;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// k_average (NEXT-1, reading N1-b; PAPER.md:79-83 mvflag / mvStep): runs after k_field when averaging is armed.
+// Step counter k (already advanced): r = k mod interval (0 read as interval); the step's dens and phi join the
+// running sums when r > interval - window; at r == interval the sums are latched and cleared.
+__global__ void __launch_bounds__(kAuxThreads) k_average(const __grid_constant__ Params P) {
+  DevState* st = P.st;
+  const unsigned long long I = (unsigned long long)P.avg_interval, W = (unsigned long long)P.avg_window;
+  unsigned long long r = st->step % I;
+  if (r == 0) r = I;
+  const bool in_window = r > I - W, latch = r == I;
+  if (!in_window && !latch) return;
+  const size_t nd = (size_t)P.ns * (size_t)P.ng, gsz = (size_t)gridDim.x * blockDim.x;
+  const size_t g0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  for (size_t i = g0; i < nd; i += gsz) {
+    long long a = P.acc_dens[i];
+    if (in_window) a += P.dens[i];
+    if (latch) { P.avg_dens[i] = a; a = 0; }
+    P.acc_dens[i] = a;
+  }
+  for (size_t j = g0; j <= (size_t)P.nc; j += gsz) {
+    double a = P.acc_phi[j];
+    if (in_window) a = a + P.phi[j];
+    if (latch) { P.avg_phi[j] = a; a = 0.0; }
+    P.acc_phi[j] = a;
+  }
+  if (g0 == 0) {
+    unsigned long long c = st->acc_count + (in_window ? 1ull : 0ull);
+    if (latch) { st->avg_count = c; st->avg_step = st->step; c = 0; }
+    st->acc_count = c;
   }
 }
 
@@ -1099,6 +1175,10 @@ int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int
   if (ev) cudaEventRecord(ev[3], s);
   launch_field(P, 1, s);
   if (ev) cudaEventRecord(ev[4], s);
+  if (P.avg_window > 0) {
+    k_average<<<sm_count(), kAuxThreads, 0, s>>>(P);
+    return 5;
+  }
   return 4;
 }
 

@@ -248,8 +248,12 @@ def make_config(cfg: int, scale: float = 1.0, *, n0_scale: float = 1.0, pair_sou
     for k, s in enumerate(sp):
         Tk = T0 if s.name == "D" else T
         x, vx, vy, vz = _species_arrays(gseed, k, n_per, L, c["profile"], _vth(Tk, s.m))
-        if cfg == 1 and k == 1:
-            x = x_e.copy()  # ions on top of electrons: rho == 0 at step 0
+        if k == 1:
+            # quiet, quasi-neutral start: every ion is loaded on its electron, rho == 0 at step 0 (SURVEY 8(d) for
+            # config 1; extended to every config -- DESIGN.md "Input recipe": independent random loads leave a
+            # sqrt(N) charge imbalance over 1e4..5e5 Debye lengths, i.e. Langmuir oscillations of many thermal
+            # speeds that no sheath deck starts from)
+            x = x_e.copy()
         if k == 0:
             x_e = x
         xs.append(x); vxs.append(vx); vys.append(vy); vzs.append(vz)

@@ -173,6 +173,23 @@ def test_no_collision_below_threshold_and_for_flagless_species():
     assert o.diag()["candidates"].sum() == 0
 
 
+def test_no_ionisation_inside_the_table_interval_that_holds_the_threshold():
+    """Reading R-thr: the 0.5 eV table interpolates to a positive cross-section on (13.5, 13.6] eV; an ionisation
+    there would hand out E - 13.6 < 0 (NaN speeds).  The rule 'zero at or below the threshold' forbids it."""
+    ion = W.Species("i", +E_CH, M_DP, 1e9, flags=W.ION_PRODUCT)
+    for E_eV, expect_events in ((13.58, False), (13.6 - 1e-9, False), (13.7, True)):
+        o, w, v = beam(200_000, E_eV, M_E, -E_CH, W.IONISE | W.ELECTRON_PRODUCT, n0=3e24, extra_species=(ion,))
+        assert O.lib().orc_sigma(o.h, 1, E_eV) > 0.0          # the table alone would allow it
+        o.step(1, freeze_field=True)
+        d = o.diag()
+        p = o.particles()
+        assert d["candidates"][0] > 1000
+        assert (d["events"][0][1] > 0) == expect_events and (d["births"] > 0) == expect_events
+        for k in ("x", "vx", "vy", "vz"):
+            assert np.all(np.isfinite(p[k]))
+        assert o.flagword == 0
+
+
 def test_capacity_flag():
     n, n0 = 20_000, 4e23
     ion = W.Species("i", +E_CH, M_DP, 1e9, flags=W.ION_PRODUCT)
