@@ -203,6 +203,9 @@ __device__ __forceinline__ void advance(const Params& P, const SpeciesP* S, unsi
 // Returns true when the moved particle is inside [0, L) -- no wall hit, no periodic wrap.
 __device__ __forceinline__ bool push_fast(const Params& P, const SpeciesP& s, const double* Eptr, int c, double& x,
                                           double& vx, double& vy, double& vz) {
+#ifdef BIT1_EXPERIMENT_NOPUSH   // measurement builds only (never the shipped library): identity step
+  return true;
+#endif
   const double f = x * P.inv_dx - (double)c;
   const double e0 = Eptr[c], e1 = Eptr[c + 1];
   const double Ex = e0 + f * (e1 - e0);

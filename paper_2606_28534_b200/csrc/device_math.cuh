@@ -82,12 +82,11 @@ __device__ __forceinline__ double sigma_lookup(const Params& P, const double* ta
 }
 
 // cell of a position: (int)(x*inv_dx) clamped to [0, nc-1]
+// The clamps are taken on the integer: cvt.rzi.s32.f64 truncates toward zero, saturates and maps NaN to 0, and
+// truncation is monotone, so max(0, min((int)t, nc-1)) equals the cast of the clamped double for every t.
 __device__ __forceinline__ int cell_of(const Params& P, double x) {
-  double t = x * P.inv_dx;
-  if (!(t >= 0.0)) t = 0.0;
-  const double top = (double)(P.nc - 1);
-  if (t > top) t = top;
-  return (int)t;
+  const int c = __double2int_rz(x * P.inv_dx);
+  return max(0, min(c, P.nc - 1));
 }
 
 // CIC split of the fixed-point charge Q (SURVEY 8(c) "D"): a goes to node c+1, Q-a to node c

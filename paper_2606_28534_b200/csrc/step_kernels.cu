@@ -146,7 +146,11 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
       const bool inside = push_fast(P, s, Eptr, c, x[r], vx[r], vy[r], vz[r]);
       cn[r] = cell_of(P, x[r]);
       const int k = cn[r] - tw.wlo;
+#ifdef BIT1_EXPERIMENT_NOPUSH
+      thr[r] = 0ull;
+#else
       thr[r] = have ? s.pthr : 0ull;
+#endif
       if (have && !(inside && k >= 0 && k < tw.W)) evm |= 1u << r;
     }
     unsigned long long any = 0;
