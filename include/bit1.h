@@ -104,8 +104,7 @@ typedef struct {
   void *compute_stream;    /* cudaStream_t, borrowed; NULL = default stream */
   void *side_stream;       /* cudaStream_t for checkpoint device->host copies; NULL = compute stream */
   int32_t checkpoint_staging; /* 1: reserve a device snapshot area so bit1_checkpoint overlaps later steps */
-  int32_t variant;         /* 0 default; 1 = in-place push then scatter ("V1"); 2 = recompute in the scatter pass ("V2");
-                              3 = V2 without CTA barriers in the particle passes ("V3") */
+  int32_t variant;         /* 0 default; 1 = in-place push then scatter ("V1"); 2 = recompute in the scatter pass ("V2") */
 } bit1_options;
 
 typedef struct {

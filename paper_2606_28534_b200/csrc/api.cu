@@ -249,8 +249,8 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   c->cs = static_cast<cudaStream_t>(o->compute_stream);
   c->ss = o->side_stream ? static_cast<cudaStream_t>(o->side_stream) : c->cs;
   c->staging = staging != 0;
-  c->variant = (o->variant >= 1 && o->variant <= 3) ? o->variant : 2;
-  if (const char* ev = getenv("BIT1_VARIANT")) { const int v = atoi(ev); if (v >= 1 && v <= 3) c->variant = v; }
+  c->variant = o->variant == 1 ? 1 : 2;
+  if (const char* ev = getenv("BIT1_VARIANT")) { const int v = atoi(ev); if (v == 1 || v == 2) c->variant = v; }
   c->cur = 0; c->loaded = false; c->ckpt_pending = false; c->launches = 0; c->dt = dt;
   c->profiling = false; c->prof_steps = 0;
 

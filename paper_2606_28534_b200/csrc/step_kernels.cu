@@ -46,12 +46,12 @@ struct PassSmem {
   static constexpr size_t a_hist = stages;                                  // unsigned[2][kWCap][kWarps]
   static constexpr size_t a_sp = a_hist + 2 * (size_t)kWCap * kWarps * 4;   // SpeciesP[kMaxSpecies]
   static constexpr size_t a_bar = (a_sp + kMaxSpecies * sizeof(SpeciesP) + 15) & ~(size_t)15;  // 2 x u64
-  static constexpr size_t a_total = a_bar + 48;   // + arrival counters[2], next-tile cells[2] (variant 3)
+  static constexpr size_t a_total = a_bar + 16;
   static constexpr size_t b_wc = stages;                                    // unsigned[kWarps][kWCap]
   static constexpr size_t b_dens = b_wc + (size_t)kWCap * kWarps * 4;       // unsigned[2][kWCap + 1][kMaxSpecies]
   static constexpr size_t b_sp = b_dens + 2 * (size_t)kDensWords * 4;
   static constexpr size_t b_bar = (b_sp + kMaxSpecies * sizeof(SpeciesP) + 15) & ~(size_t)15;
-  static constexpr size_t b_total = b_bar + 48;
+  static constexpr size_t b_total = b_bar + 16;
 };
 
 // (cell of the first particle, cell of the last particle) of tile t, read from the sorted cell array itself
@@ -82,8 +82,6 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
   unsigned* s_hist2 = reinterpret_cast<unsigned*>(smem + SM::a_hist);
   SpeciesP* s_sp = reinterpret_cast<SpeciesP*>(smem + SM::a_sp);
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem + SM::a_bar);
-  unsigned* s_done = reinterpret_cast<unsigned*>(smem + SM::a_bar + 16);   // [2] warps that finished the stage
-  int2* s_dn = reinterpret_cast<int2*>(smem + SM::a_bar + 32);             // [2] cells of the tile to load next
 
   const unsigned n = P.st->n;
   const unsigned long long step = P.st->step;
@@ -103,7 +101,6 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
   }
   load_species(P, s_sp);
   for (int k = threadIdx.x; k < 2 * kWCap * kWarps; k += kThreads) s_hist2[k] = 0;
-  if (threadIdx.x < 2) s_done[threadIdx.x] = 0;
   // the deposition of this step accumulates into dens: clear it here (nobody reads it during pass A)
   {
     const size_t tot = (size_t)P.ns * (size_t)P.ng;
@@ -114,8 +111,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
   int it = 0;
   for (int tile = blockIdx.x; tile < ntiles; tile += G, ++it) {
     Stage* S = &stg[it & 1];
-    // V1/V2: [window cell][warp], double-buffered over tiles; V3: this warp's own row [window cell]
-    unsigned* s_hist = VARIANT == 3 ? s_hist2 + warp * kWCap : s_hist2 + (it & 1) * (kWCap * kWarps);
+    unsigned* s_hist = s_hist2 + (it & 1) * (kWCap * kWarps);   // [window cell][warp]
     const unsigned base = (unsigned)tile * kTile;
     const unsigned cnt = min((unsigned)kTile, n - base);
     // cells of the tile after next (its load is issued at the end of this iteration)
@@ -199,41 +195,13 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
         }
         if (cn[r] >= 0) key = (unsigned)(cn[r] - tw.wlo);
       }
-      if (VARIANT >= 2) {
+      if (VARIANT == 2) {
         const unsigned eb = __ballot_sync(0xffffffffu, (evm >> r) & 1u);
         if (lane == 0) P.evt[(base >> 5) + (unsigned)(warp * kItems + r)] = eb;
       }
       const unsigned m = __match_any_sync(0xffffffffu, key);
-      if (!(key & 0x80000000u) && lane == __ffs(m) - 1)
-        s_hist[VARIANT == 3 ? key : key * kWarps + warp] += (unsigned)__popc(m);
+      if (!(key & 0x80000000u) && lane == __ffs(m) - 1) s_hist[key * kWarps + warp] += (unsigned)__popc(m);
       __syncwarp();
-    }
-    if (VARIANT == 3) {
-      // No CTA barrier: every warp publishes its own counts per window cell (pass B turns them into prefixes
-      // over the warps, k_mid sums them), then signs the stage off; the last warp to do so reloads it.
-      const size_t rowo = tile_row_offset(clo, tile, P.R);
-      for (int k = lane; k < tw.W; k += 32) {
-        const unsigned t = s_hist[k];
-        s_hist[k] = 0;
-        P.tile_pre[(rowo + (size_t)k) * kWarps + warp] = t;
-        const int c = tw.wlo + k;
-        if (t && c >= 0 && c < P.nc) atomicAdd(&P.cell_count[c], (int)t);
-      }
-      fence_proxy_async();
-      __syncwarp();
-      unsigned old = 0;
-      if (lane == 0) {
-        if (warp == 0) s_dn[it & 1] = dn;
-        __threadfence_block();
-        old = atomicAdd(&s_done[it & 1], 1u);
-        if (old == (unsigned)kWarps - 1u) {
-          __threadfence_block();
-          s_done[it & 1] = 0;
-          if (tnext < ntiles) issue_tile(P, cur, S, &bar[it & 1], tnext, s_dn[it & 1], false, true, false, false);
-        }
-      }
-      __syncwarp();
-      continue;
     }
     fence_proxy_async();
     __syncthreads();
@@ -368,8 +336,7 @@ __device__ int block_sum_int(int v, int* s_warp) {
 //                    walks, in tile order, the tiles whose window holds the cell and hands each its destination
 //                    base = cell_base[c] + what the earlier tiles send to c.  Those tiles are the ones that hold
 //                    old cells c-R .. c+R, found from the previous step's cell_start.
-__global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Params P, Particles cur, int do_colscan,
-                                                     int warp_counts) {
+__global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Params P, Particles cur, int do_colscan) {
   __shared__ unsigned long long s_key[kSortSmem];
   __shared__ unsigned s_val[kSortSmem];
   __shared__ int s_warp[33];
@@ -534,16 +501,7 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
         if (k >= 0 && k < tw.W) {
           const size_t off = tile_row_offset(d.x, t, R) + (size_t)k;
           P.tile_base[off] = run;
-          if (warp_counts) {   // variant 3: pass A left one count per warp in tile_pre
-            const uint4* q = reinterpret_cast<const uint4*>(P.tile_pre + off * kWarps);
-#pragma unroll
-            for (int w4 = 0; w4 < kWarps / 4; ++w4) {
-              const uint4 v = q[w4];
-              run += (int)((v.x + v.y) + (v.z + v.w));
-            }
-          } else {
-            run += (int)P.tile_hist[off];
-          }
+          run += (int)P.tile_hist[off];
         }
       }
     }
@@ -568,9 +526,7 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
   unsigned* s_dens2 = reinterpret_cast<unsigned*>(smem + SM::b_dens);   // [2][kWCap + 1][ns]
   SpeciesP* s_sp = reinterpret_cast<SpeciesP*>(smem + SM::b_sp);
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem + SM::b_bar);
-  unsigned* s_done = reinterpret_cast<unsigned*>(smem + SM::b_bar + 16);
-  int2* s_dn = reinterpret_cast<int2*>(smem + SM::b_bar + 32);
-  constexpr bool kRecompute = VARIANT >= 2;   // V2, V3: the tile carries the old state and the event bits
+  constexpr bool kRecompute = VARIANT == 2;   // V2: the tile carries the old state and the event bits
 
   const unsigned n = P.st->n;
   const unsigned long long step = P.st->step;
@@ -593,7 +549,6 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
   }
   load_species(P, s_sp);
   for (int k = threadIdx.x; k < 2 * kDensWords; k += kThreads) s_dens2[k] = 0;
-  if (threadIdx.x < 2) s_done[threadIdx.x] = 0;
   __syncthreads();
 
   int it = 0;
@@ -606,22 +561,12 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     const int tnext = tile + 2 * G;
     if (threadIdx.x == 0 && tnext < ntiles) dn = cur.desc[tnext];
     mbar_wait(&bar[it & 1], (unsigned)(it >> 1) & 1u);
-    // the stage's descriptor is only valid once its barrier has completed (variant 3 has no CTA barrier in between)
+    // the stage's descriptor is only valid once its barrier has completed
     const int2 d = S->d;
     const TileWin tw = make_window(d.x, d.y, P.R);
 
     // destination of this warp's first particle of every window cell
-    if (VARIANT == 3) {
-      // pre holds the warps' counts: this warp starts after the earlier warps' particles of the cell
-      for (int k = lane; k < tw.W; k += 32) {
-        unsigned run = (unsigned)S->tb[k];
-#pragma unroll
-        for (int w2 = 0; w2 < kWarps; ++w2) run += w2 < warp ? S->pre[k * kWarps + w2] : 0u;
-        wc[k] = run;
-      }
-    } else {
-      for (int k = lane; k < tw.W; k += 32) wc[k] = (unsigned)S->tb[k] + S->pre[k * kWarps + warp];
-    }
+    for (int k = lane; k < tw.W; k += 32) wc[k] = (unsigned)S->tb[k] + S->pre[k * kWarps + warp];
     __syncwarp();
 
     int e0, ne;
@@ -716,42 +661,6 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
         nxt.x[dst] = x[r]; nxt.vx[dst] = vx[r]; nxt.vy[dst] = vy[r]; nxt.vz[dst] = vz[r];
         nxt.cell[dst] = tw.wlo + key[r]; nxt.pid[dst] = S->pid[off]; nxt.sp[dst] = (unsigned char)sp[r];
       }
-    }
-    if (VARIANT == 3) {
-      // No CTA barrier: the last warp to sign the stage off flushes the tile's deposit and reloads the stage.
-      // (The other buffer of s_dens belongs to the next tile, whose flush precedes the load of the tile after
-      // it, so nobody deposits into a buffer that is being flushed.)
-      fence_proxy_async();
-      __syncwarp();
-      unsigned old = 0;
-      if (lane == 0) {
-        if (warp == 0) s_dn[it & 1] = dn;
-        __threadfence_block();
-        old = atomicAdd(&s_done[it & 1], 1u);
-      }
-      old = __shfl_sync(0xffffffffu, old, 0);
-      if (old == (unsigned)kWarps - 1u) {
-        __threadfence_block();
-        if (P.dep_u32) {
-          for (int k = lane; k < ns * (tw.W + 1); k += 32) {
-            const unsigned v = s_dens[k];
-            if (v) {
-              s_dens[k] = 0;
-              const int kk = k / ns, s = k - kk * ns;
-              int j = tw.wlo + kk;
-              if (!P.bc && j == P.nc) j = 0;
-              atomicAdd((unsigned long long*)&P.dens[(size_t)s * P.ng + j], (unsigned long long)v);
-            }
-          }
-        }
-        __syncwarp();
-        if (lane == 0) {
-          s_done[it & 1] = 0;
-          __threadfence_block();
-          if (tnext < ntiles) issue_tile(P, cur, S, &bar[it & 1], tnext, s_dn[it & 1], true, true, true, false);
-        }
-      }
-      continue;
     }
     fence_proxy_async();
     __syncthreads();  // the stage may be overwritten; the tile's deposit is complete
@@ -1132,10 +1041,6 @@ cudaError_t configure_kernels() {
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(k_pass_b<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::b_total);
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_pass_a<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::a_total);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_pass_b<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::b_total);
-  if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(k_pass_b<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::b_total);
 }
 
@@ -1146,11 +1051,11 @@ static int coop_grid(int work_items, int per_cta) {
   return g < cap ? g : cap;
 }
 
-static void launch_mid(const Params& P, const Particles& cur, int do_colscan, int warp_counts, cudaStream_t s) {
+static void launch_mid(const Params& P, const Particles& cur, int do_colscan, cudaStream_t s) {
   Params Pc = P;
   Particles pc = cur;
-  int dc = do_colscan, wcn = warp_counts;
-  void* args[] = {&Pc, &pc, &dc, &wcn};
+  int dc = do_colscan;
+  void* args[] = {&Pc, &pc, &dc};
   cudaLaunchCooperativeKernel((const void*)k_mid, dim3(coop_grid(P.nc, kMidThreads)), dim3(kMidThreads), args, 0, s);
 }
 
@@ -1167,14 +1072,12 @@ int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int
   typedef PassSmem SM;
   const int g = particle_grid(P);
   if (ev) cudaEventRecord(ev[0], s);
-  if (variant == 3) k_pass_a<3><<<g, kThreads, SM::a_total, s>>>(P, cur);
-  else if (variant == 2) k_pass_a<2><<<g, kThreads, SM::a_total, s>>>(P, cur);
+  if (variant == 2) k_pass_a<2><<<g, kThreads, SM::a_total, s>>>(P, cur);
   else k_pass_a<1><<<g, kThreads, SM::a_total, s>>>(P, cur);
   if (ev) cudaEventRecord(ev[1], s);
-  launch_mid(P, cur, 1, variant == 3, s);
+  launch_mid(P, cur, 1, s);
   if (ev) cudaEventRecord(ev[2], s);
-  if (variant == 3) k_pass_b<3><<<g, kThreads, SM::b_total, s>>>(P, cur, nxt);
-  else if (variant == 2) k_pass_b<2><<<g, kThreads, SM::b_total, s>>>(P, cur, nxt);
+  if (variant == 2) k_pass_b<2><<<g, kThreads, SM::b_total, s>>>(P, cur, nxt);
   else k_pass_b<1><<<g, kThreads, SM::b_total, s>>>(P, cur, nxt);
   if (ev) cudaEventRecord(ev[3], s);
   launch_field(P, 1, s);
@@ -1207,7 +1110,7 @@ int launch_rebuild(const Params& P, const Particles& cur, cudaStream_t s) {
   const int g = sm_count() * 4;
   k_clear_grids<<<g, 256, 0, s>>>(P);
   k_count_cells<<<g, kAuxThreads, 0, s>>>(P, cur);
-  launch_mid(P, cur, 0, 0, s);   // ovf_count == 0: plain scan; n_next = n; no column scan (no tile rows yet)
+  launch_mid(P, cur, 0, s);   // ovf_count == 0: plain scan; n_next = n; no column scan (no tile rows yet)
   k_deposit<<<g, kAuxThreads, 0, s>>>(P, cur);
   launch_field(P, 0, s);  // commits n = n_next, leaves the step counter alone
   return 5;
