@@ -531,7 +531,7 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
   const unsigned n = P.st->n;
   const unsigned long long step = P.st->step;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const unsigned lt = lanemask_lt();
+  const unsigned lt = (1u << lane) - 1u;   // lanes below this one (cheaper to rematerialise than S2R SR_LTMASK)
   const int ntiles = (int)((n + kTile - 1) / kTile);
   const int G = gridDim.x;
   const int ns = P.ns;
