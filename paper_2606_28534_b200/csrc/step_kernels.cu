@@ -280,6 +280,67 @@ __device__ void cta_sort(unsigned long long* gkey, unsigned* gval, unsigned P2, 
   }
 }
 
+// Side lists too long for one CTA's shared memory (a degenerate input: most particles leave their tile's window):
+// bitonic sort over the whole cooperative grid.  Chunks of kSortSmem elements are sorted in shared memory; the
+// exchanges at distance >= kSortSmem run in global memory with one grid barrier each.  The direction of a compare
+// is taken from the global index, so the network is the same as cta_bitonic's.
+__device__ void chunk_steps(unsigned long long* gkey, unsigned* gval, unsigned base, unsigned k_lo, unsigned k_hi,
+                            unsigned long long* s_key, unsigned* s_val) {
+  for (unsigned i = threadIdx.x; i < (unsigned)kSortSmem; i += blockDim.x) { s_key[i] = gkey[base + i]; s_val[i] = gval[base + i]; }
+  __syncthreads();
+  for (unsigned k = k_lo; k <= k_hi; k <<= 1) {
+    unsigned j = k >> 1;
+    if (j > (unsigned)kSortSmem / 2) j = (unsigned)kSortSmem / 2;
+    for (; j > 0; j >>= 1) {
+      for (unsigned i = threadIdx.x; i < (unsigned)kSortSmem; i += blockDim.x) {
+        const unsigned ixj = i ^ j;
+        if (ixj > i) {
+          const unsigned long long a = s_key[i], b = s_key[ixj];
+          const bool asc = ((base + i) & k) == 0;
+          if ((a > b) == asc) {
+            s_key[i] = b; s_key[ixj] = a;
+            const unsigned t = s_val[i]; s_val[i] = s_val[ixj]; s_val[ixj] = t;
+          }
+        }
+      }
+      __syncthreads();
+    }
+  }
+  for (unsigned i = threadIdx.x; i < (unsigned)kSortSmem; i += blockDim.x) { gkey[base + i] = s_key[i]; gval[base + i] = s_val[i]; }
+  __syncthreads();
+}
+
+__device__ void grid_bitonic(cg::grid_group& grid, unsigned long long* gkey, unsigned* gval, unsigned P2,
+                             unsigned long long* s_key, unsigned* s_val) {
+  const unsigned nchunk = P2 / (unsigned)kSortSmem;   // P2 > kSortSmem, both powers of two
+  for (unsigned c = blockIdx.x; c < nchunk; c += gridDim.x)
+    chunk_steps(gkey, gval, c * (unsigned)kSortSmem, 2u, (unsigned)kSortSmem, s_key, s_val);
+  __threadfence();
+  grid.sync();
+  const size_t gtid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, gsz = (size_t)gridDim.x * blockDim.x;
+  for (unsigned k = 2u * (unsigned)kSortSmem; k <= P2 && k != 0; k <<= 1) {
+    for (unsigned j = k >> 1; j >= (unsigned)kSortSmem; j >>= 1) {
+      for (size_t i = gtid; i < (size_t)P2; i += gsz) {
+        const size_t ixj = i ^ (size_t)j;
+        if (ixj > i) {
+          const unsigned long long a = gkey[i], b = gkey[ixj];
+          const bool asc = (i & (size_t)k) == 0;
+          if ((a > b) == asc) {
+            gkey[i] = b; gkey[ixj] = a;
+            const unsigned t = gval[i]; gval[i] = gval[ixj]; gval[ixj] = t;
+          }
+        }
+      }
+      __threadfence();
+      grid.sync();
+    }
+    for (unsigned c = blockIdx.x; c < nchunk; c += gridDim.x)
+      chunk_steps(gkey, gval, c * (unsigned)kSortSmem, k, k, s_key, s_val);
+    __threadfence();
+    grid.sync();
+  }
+}
+
 __device__ int block_exclusive_scan_int(int v, int* s_warp, int* total) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   int inc = v;
@@ -348,8 +409,73 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
   unsigned M = st->ovf_count;
   if (M > P.ovf_cap) M = P.ovf_cap;
 
-  if (b == 0) {
-    const unsigned P2 = next_pow2(M > 1 ? M : 1);
+  const unsigned P2 = next_pow2(M > 1 ? M : 1);
+  const bool big = P2 > (unsigned)kSortSmem;   // uniform over the grid
+  if (big) {
+    // the same three steps as below, spread over the grid (grid_bitonic); births are counted in scan_part[0]
+    const size_t gt = (size_t)b * kMidThreads + threadIdx.x, gs = (size_t)G * kMidThreads;
+    if (gt == 0) P.scan_part[0] = 0;
+    __threadfence();
+    grid.sync();
+    unsigned nb_local = 0;
+    for (size_t i = gt; i < (size_t)P2; i += gs) {
+      unsigned long long bk = kInvalidKey;
+      if (i < M) {
+        const unsigned long long key = P.ovf_key[i];
+        if (((key >> kClsShift) & 3ull) == 2ull) { bk = key & ((1ull << kOrdBits) - 1ull); nb_local++; }
+      }
+      P.tmp_key[i] = bk;
+      P.tmp_idx[i] = (unsigned)i;
+    }
+    if (nb_local) atomicAdd(&P.scan_part[0], (int)nb_local);
+    __threadfence();
+    grid.sync();
+    const unsigned B = (unsigned)P.scan_part[0];
+    if (B > 0) {
+      grid_bitonic(grid, P.tmp_key, P.tmp_idx, P2, s_key, s_val);
+      const unsigned room = P.capacity > n ? P.capacity - n : 0u;
+      const unsigned next_pid = st->next_pid;
+      for (size_t r = gt; r < (size_t)B; r += gs) {
+        const unsigned rec = P.tmp_idx[r];
+        if (r < room) P.ovf_rec[rec].pid = next_pid + (unsigned)r;
+        else P.ovf_key[rec] = kInvalidKey;
+      }
+      __threadfence();
+      grid.sync();
+      if (gt == 0) {
+        const unsigned created = B < room ? B : room;
+        st->next_pid = next_pid + created;
+        st->births += created;
+        if (B > room) st->flags |= kFlagCapacity;
+      }
+    }
+    for (size_t i = gt; i < (size_t)P2; i += gs) {
+      if (i >= M) P.ovf_key[i] = kInvalidKey;
+      P.ovf_idx[i] = (unsigned)i;
+    }
+    __threadfence();
+    grid.sync();
+    grid_bitonic(grid, P.ovf_key, P.ovf_idx, P2, s_key, s_val);
+    const unsigned Mv = lower_bound_u64(P.ovf_key, P2, kInvalidKey);
+    for (size_t p = gt; p < (size_t)Mv; p += gs) {
+      const unsigned long long key = P.ovf_key[p];
+      const unsigned long long c = key >> kCellShift;
+      const unsigned lb = lower_bound_u64(P.ovf_key, Mv, c << kCellShift);
+      const unsigned ub = lower_bound_u64(P.ovf_key, Mv, (c + 1ull) << kCellShift);
+      const unsigned cls = (unsigned)((key >> kClsShift) & 3ull);
+      if (p == lb) {
+        const unsigned ub0 = lower_bound_u64(P.ovf_key, Mv, (c << kCellShift) | (1ull << kClsShift));
+        P.cell_count[c] += (int)(ub - lb);
+        P.ovf_before[c] = (int)(ub0 - lb);
+      }
+      P.ovf_dst[p] = cls == 0 ? (int)(p - lb) : (int)(p - lb) - (int)(ub - lb);
+    }
+    if (gt == 0) {
+      st->ovf_valid = Mv;
+      st->far_movers += M;
+      if (M > st->max_far_movers) st->max_far_movers = M;
+    }
+  } else if (b == 0) {
     unsigned Mv = 0;
     if (M > 0) {
       // (a) births: order by (parent index, kind), assign pid = next_pid + r, drop those beyond capacity

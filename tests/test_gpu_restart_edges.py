@@ -170,6 +170,21 @@ def test_all_particles_in_one_cell_and_sparse_cells():
     g.close()
 
 
+@pytest.mark.parametrize("cfg,scale,kw", [(1, 1 / 4, {}), (3, 1 / 256, dict(n0_scale=300.0, pair_source=True))])
+def test_side_list_longer_than_one_cta_sorts_over_the_grid(cfg, scale, kw):
+    """A plasma 40 times hotter than the grid was sized for: nearly every particle leaves its tile's window, so the
+    side list (far movers and births) holds tens of thousands of entries and k_mid orders it with the grid-wide
+    bitonic sort instead of one CTA's shared memory.  Same bits as the oracle, which has no such notion."""
+    w = W.make_config(cfg, scale=scale, **kw)
+    for k in ("vx", "vy", "vz"):
+        setattr(w, k, np.ascontiguousarray(getattr(w, k) * 40.0))
+    g, o = run_pair(w, 3)
+    m = g.get_moments()
+    assert m["max_far_movers_per_step"] > 4096, "the workload was meant to overflow one CTA's sort"
+    assert assert_state_equal(g, o, where=f"c{cfg} hot plasma, long side list")
+    g.close()
+
+
 def test_capacity_hit_matches_oracle_and_raises_the_sticky_flag():
     """Ionisation births beyond capacity are dropped in (parent, kind) order and flag CAPACITY (reading R-W)."""
     from paper_2606_28534_b200.binding import Bit1Error, ERR_DEVICE_FLAG, FLAG_CAPACITY
