@@ -113,6 +113,10 @@ typedef struct {
   uint64_t diag_nu_overflow, diag_dir_fallback, diag_escape, diag_births, diag_reinject;
   uint64_t diag_candidates[ORC_MAX_SPECIES];
   uint64_t diag_events[ORC_MAX_SPECIES][3]; /* elastic, ionise, cx */
+  /* NEXT-2: wall recycling, per species: index of the species born at the wall (-1 = none) */
+  int32_t recycle_to[ORC_MAX_SPECIES];
+  double recycle_vth[ORC_MAX_SPECIES];
+  uint64_t diag_recycled;
   /* NEXT-1: density smoothing and time-averaged diagnostics */
   int32_t smooth_passes; /* 0 = off */
   int64_t *rho_s;        /* ng: 4^passes * smoothed rho, what the field solve used */
@@ -259,6 +263,7 @@ orc *orc_create(int32_t nc, double dx, int32_t bc, double area, const double B[3
     o->kin_eV[s] = (0.5 * m[s]) / E_CHARGE;
     o->two_e_over_m[s] = (2.0 * E_CHARGE) / m[s];
     o->el_loss[s] = (2.0 * m[s]) / m_n;
+    o->recycle_to[s] = -1;
     o->Q[s] = (int64_t)llrint((E_CHARGE * weight[s]) * 1099511627776.0);
     o->sign[s] = q[s] > 0.0 ? 1 : (q[s] < 0.0 ? -1 : 0);
     if (o->Q[s] < 1 || o->Q[s] >= ((int64_t)1 << 31)) { free(o); return NULL; }
@@ -498,6 +503,15 @@ static void phase_average(orc *o) {
   }
 }
 
+/* NEXT-2: species s recycles into species `to` (-1 switches it off) at wall temperature sqrt(e T_w / m_to) = vth */
+int orc_set_recycling(orc *o, int32_t s, int32_t to, double vth) {
+  if (s < 0 || s >= o->ns || to >= o->ns || (to >= 0 && !(vth >= 0.0))) return 1;
+  o->recycle_to[s] = to < 0 ? -1 : to;
+  o->recycle_vth[s] = vth;
+  return 0;
+}
+uint64_t orc_recycled(const orc *o) { return o->diag_recycled; }
+
 void orc_set_smoothing(orc *o, int32_t passes) { o->smooth_passes = passes < 0 ? 0 : (passes > 8 ? 8 : passes); }
 /* (re)arms the averaging: running and latched sums are cleared */
 int orc_set_averaging(orc *o, int32_t window, int32_t interval) {
@@ -566,6 +580,9 @@ void orc_phase_push(orc *o) {
     int alive = 1;
     int pair_birth = 0;
     double bvx = 0, bvy = 0, bvz = 0;
+    int recycled = 0;
+    double rx = 0, rvx = 0, rvy = 0, rvz = 0;
+    int32_t rc = 0;
     if (!o->bc) {
       if (x < 0.0) x = x + L;
       if (x >= L) x = x - L;
@@ -583,6 +600,25 @@ void orc_phase_push(orc *o) {
       if (side >= 0) {
         o->wall_count[side][s] += 1;
         o->wall_charge[side] += (int64_t)o->sign[s] * o->Q[s];
+        if (o->recycle_to[s] >= 0) {
+          /* Wall recycling ("Plasma is absorbed at the walls ..., recycling D+ ions into D neutrals";
+           * SURVEY 8(f) NEXT-2; reading N2-a): the absorbed particle leaves one particle of species
+           * recycle_to at the wall it hit -- x = 0 at the left wall, x = L - dx*2^-20 at the right one -- with a
+           * half-Maxwellian velocity at the wall temperature pointing into the plasma: slot 14 (RC) of the
+           * parent's stream, vx = +-vth*|z0| (away from the wall), vy = vth*z1, vz = vth*z2.  What happens to the
+           * absorbed particle itself (death, re-injection, pair source) is unchanged. */
+          uint32_t wr[4];
+          draw(o, pid, step, 14u, wr); /* slot RC */
+          double z0 = normal_from_word(o, wr[0]);
+          if (z0 < 0.0) z0 = -z0;
+          double vth_r = o->recycle_vth[s];
+          rvx = side == 0 ? vth_r * z0 : -(vth_r * z0);
+          rvy = vth_r * normal_from_word(o, wr[1]);
+          rvz = vth_r * normal_from_word(o, wr[2]);
+          rx = side == 0 ? 0.0 : L - o->dx * 9.5367431640625e-07;
+          rc = side == 0 ? 0 : o->nc - 1;
+          recycled = 1;
+        }
         if (o->src_mode[s] == SRC_NONE) {
           alive = 0;
         } else {
@@ -698,6 +734,11 @@ void orc_phase_push(orc *o) {
     if (ionised) {
       append_birth(o, &births, o->sp_electron_product, x, cn, e2vx, e2vy, e2vz);
       append_birth(o, &births, o->sp_ion_product, x, cn, ivx, ivy, ivz);
+    }
+    if (recycled) {   /* a parent's fourth and last birth */
+      uint32_t before = births;
+      append_birth(o, &births, o->recycle_to[s], rx, rc, rvx, rvy, rvz);
+      o->diag_recycled += births - before;
     }
   }
   o->next_pid += births;

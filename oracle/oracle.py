@@ -80,6 +80,10 @@ def lib():
         L.orc_poisson.argtypes = [C.c_int32, C.c_int32, C.c_double, C.c_double, c_i64p, c_f64p, c_f64p]
         L.orc_smooth121.argtypes = [C.c_int32, C.c_int32, c_i64p, c_i64p]
         L.orc_set_smoothing.argtypes = [C.c_void_p, C.c_int32]
+        L.orc_set_recycling.restype = C.c_int
+        L.orc_set_recycling.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double]
+        L.orc_recycled.restype = C.c_uint64
+        L.orc_recycled.argtypes = [C.c_void_p]
         L.orc_set_averaging.restype = C.c_int
         L.orc_set_averaging.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
         L.orc_get_average.argtypes = [C.c_void_p, c_i64p, c_f64p, c_u64p, c_u64p]
@@ -163,6 +167,9 @@ class Oracle:
                               int(inv_norm.shape[0] - 1))
         if not self.h:
             raise ValueError("orc_create rejected the configuration")
+        for k, spc in enumerate(sp):
+            if getattr(spc, "recycle_to", -1) >= 0:
+                self.set_recycling(k, spc.recycle_to, spc.recycle_vth)
         if load and w.x is not None:
             self.load(w.x, w.vx, w.vy, w.vz, w.sp)
 
@@ -264,6 +271,13 @@ class Oracle:
         r = np.zeros(self.ng, np.int64)
         lib().orc_get_rho(self.h, _p(r, c_i64p))
         return r
+
+    def set_recycling(self, s: int, to: int, vth: float):
+        assert lib().orc_set_recycling(self.h, int(s), int(to), float(vth)) == 0
+
+    @property
+    def recycled(self):
+        return int(lib().orc_recycled(self.h))
 
     def set_smoothing(self, passes: int):
         lib().orc_set_smoothing(self.h, int(passes))

@@ -50,6 +50,8 @@ class Species:
     src_vth: float = 0.0
     pnull: float = 0.0
     numax: float = 0.0
+    recycle_to: int = -1      # NEXT-2: species born at the wall when this one is absorbed (-1 = none)
+    recycle_vth: float = 0.0  # sqrt(e T_wall / m_recycle_to), m/s
 
 
 @dataclass
@@ -184,7 +186,7 @@ _CFG = {
 }
 
 
-def make_config(cfg: int, scale: float = 1.0, *, n0_scale: float = 1.0, pair_source: bool = False,
+def make_config(cfg: int, scale: float = 1.0, *, n0_scale: float = 1.0, pair_source: bool = False, recycle: bool = False,
                 gen_seed: Optional[int] = None, lib_seed: Optional[int] = None,
                 capacity_factor: float = 1.02, particles: bool = True) -> Workload:
     """Build configuration `cfg` (1..5) of BASELINE.json.
@@ -193,6 +195,8 @@ def make_config(cfg: int, scale: float = 1.0, *, n0_scale: float = 1.0, pair_sou
     n0_scale    multiplies the neutral density (tests use it to make collisions frequent).
     pair_source config 2 validation variant "2P" (reading A9): electrons SRC_NONE,
                 D+ SRC_PAIR(e).
+    recycle     NEXT-2: absorbed D+ ions leave a D neutral at the wall; configs without a neutral
+                species get an (initially empty) one.
     particles   False skips the particle arrays (only parameters and tables).
     """
     c = _CFG[cfg]
@@ -221,6 +225,11 @@ def make_config(cfg: int, scale: float = 1.0, *, n0_scale: float = 1.0, pair_sou
     ]
     if ns == 3:
         sp.append(Species("D", 0.0, M_D, weight, 0, src, -1, _vth(T0, M_D)))
+    if recycle and c["bc"]:
+        if len(sp) == 2:
+            sp.append(Species("D", 0.0, M_D, weight, 0, src, -1, _vth(T0, M_D)))
+        sp[1].recycle_to = 2
+        sp[1].recycle_vth = _vth(T0, M_D)
     if pair_source:
         sp[0].src_mode = SRC_NONE
         sp[1].src_mode = SRC_PAIR
@@ -245,7 +254,7 @@ def make_config(cfg: int, scale: float = 1.0, *, n0_scale: float = 1.0, pair_sou
     gseed = gen_seed if gen_seed is not None else 2606285340 + cfg
     xs, vxs, vys, vzs, tags = [], [], [], [], []
     x_e = None
-    for k, s in enumerate(sp):
+    for k, s in enumerate(sp[:ns]):   # a neutral species added for recycling starts empty
         Tk = T0 if s.name == "D" else T
         x, vx, vy, vz = _species_arrays(gseed, k, n_per, L, c["profile"], _vth(Tk, s.m))
         if k == 1:
