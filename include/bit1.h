@@ -122,6 +122,7 @@ typedef struct {
   uint64_t candidates[BIT1_MAX_SPECIES];
   uint64_t events[BIT1_MAX_SPECIES][3]; /* elastic, ionise, cx */
   uint64_t far_movers, max_far_movers_per_step; /* entries that took the sorted side list */
+  uint64_t recycled;                  /* wall-recycling events (NEXT-2) */
   double *density[BIT1_MAX_SPECIES];  /* HOST, optional (NULL to skip), ng entries each, m^-3 */
 } bit1_moments;
 
@@ -156,6 +157,15 @@ bit1_status bit1_get_moments(bit1_ctx *ctx, bit1_moments *out);
 /* Any pointer may be NULL.  n_live entries each (bit1_get_count), cell_start nc+1 entries. */
 bit1_status bit1_get_particles(bit1_ctx *ctx, double *x, double *vx, double *vy, double *vz,
                                int32_t *cell, uint32_t *pid, uint8_t *species, int64_t *cell_start_or_null);
+
+/* Wall recycling ("Plasma is absorbed at the walls (depositing charge), recycling D+ ions into D neutrals";
+ * SURVEY 8(f) NEXT-2; reading N2-a): every particle of `species` absorbed at a wall leaves one particle of
+ * species `to_species` at that wall (x = 0 at the left, x = nc*dx - dx*2^-20 at the right), velocity half-Maxwellian into
+ * the plasma with per-component thermal speed `vth` = sqrt(e*T_wall/m_to) (slot 14 of the parent's Philox stream).  The
+ * absorbed particle's own fate (death / re-injection / pair source) is unchanged.  to_species = -1 switches it off.
+ * Part of the configuration: call it after bit1_create and before bit1_load_particles / bit1_restart (it enters the
+ * configuration hash a checkpoint is validated against).  BIT1_ERR_INVALID_ARG for bad indices or vth < 0. */
+bit1_status bit1_set_recycling(bit1_ctx *ctx, int species, int to_species, double vth);
 
 /* Density smoothing ("density smoothing", "smoothing operators"; SURVEY 8(f) NEXT-1;
  * DESIGN.md reading N1-a): `passes` (0..8, 0 = off) passes of the 1-2-1 binomial filter over rho before every

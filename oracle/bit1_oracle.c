@@ -736,9 +736,8 @@ void orc_phase_push(orc *o) {
       append_birth(o, &births, o->sp_ion_product, x, cn, ivx, ivy, ivz);
     }
     if (recycled) {   /* a parent's fourth and last birth */
-      uint32_t before = births;
       append_birth(o, &births, o->recycle_to[s], rx, rc, rvx, rvy, rvz);
-      o->diag_recycled += births - before;
+      o->diag_recycled += 1;   /* recycling events (the birth itself may be dropped at capacity, reading R-W) */
     }
   }
   o->next_pid += births;

@@ -50,7 +50,7 @@ class bit1_moments(C.Structure):
                 ("nu_overflow", C.c_uint64), ("dir_fallback", C.c_uint64), ("escape", C.c_uint64),
                 ("births", C.c_uint64), ("reinject", C.c_uint64), ("candidates", C.c_uint64 * MAX_SPECIES),
                 ("events", (C.c_uint64 * 3) * MAX_SPECIES), ("far_movers", C.c_uint64),
-                ("max_far_movers_per_step", C.c_uint64), ("density", c_f64p * MAX_SPECIES)]
+                ("max_far_movers_per_step", C.c_uint64), ("recycled", C.c_uint64), ("density", c_f64p * MAX_SPECIES)]
 
 
 _lib = None
@@ -89,6 +89,8 @@ def load_library(path: Optional[str] = None):
     L.bit1_get_moments.argtypes = [vp, C.POINTER(bit1_moments)]
     L.bit1_get_particles.restype = C.c_int
     L.bit1_get_particles.argtypes = [vp] + [vp] * 8
+    L.bit1_set_recycling.restype = C.c_int
+    L.bit1_set_recycling.argtypes = [vp, C.c_int, C.c_int, C.c_double]
     L.bit1_set_smoothing.restype = C.c_int
     L.bit1_set_smoothing.argtypes = [vp, C.c_int]
     L.bit1_get_rho_smoothed.restype = C.c_int
@@ -199,6 +201,9 @@ class Bit1:
         h = C.c_void_p()
         _check(self.lib.bit1_create(C.byref(g), sp, self.ns, w.dt, C.byref(o), C.byref(h)), "bit1_create")
         self.h = h
+        for k, s in enumerate(w.species):   # NEXT-2: part of the configuration, set before any load or restart
+            if getattr(s, "recycle_to", -1) >= 0:
+                self.set_recycling(k, s.recycle_to, s.recycle_vth)
 
     def close(self):
         if getattr(self, "h", None):
@@ -291,7 +296,8 @@ class Bit1:
                    dir_fallback=int(m.dir_fallback), escape=int(m.escape), births=int(m.births),
                    reinject=int(m.reinject), candidates=np.array(m.candidates[:ns], np.uint64),
                    events=np.array([list(m.events[k][:]) for k in range(ns)], np.uint64),
-                   far_movers=int(m.far_movers), max_far_movers_per_step=int(m.max_far_movers_per_step))
+                   far_movers=int(m.far_movers), max_far_movers_per_step=int(m.max_far_movers_per_step),
+                   recycled=int(m.recycled))
         if density:
             out["density"] = dens
         return out
@@ -308,6 +314,9 @@ class Bit1:
         if cell_start:
             d["cell_start"] = cs
         return d
+
+    def set_recycling(self, species: int, to_species: int, vth: float):
+        _check(self.lib.bit1_set_recycling(self.h, int(species), int(to_species), float(vth)), "bit1_set_recycling")
 
     # -- NEXT-1: density smoothing, time-averaged diagnostics ----------------------------------
     def set_smoothing(self, passes: int):

@@ -36,8 +36,8 @@ struct PairBirth {
 // W: wall hit on an absorbing boundary.  Returns alive.
 template <bool EMIT>
 __device__ __noinline__ bool wall_event(const Params& P, const SpeciesP* S, unsigned long long step, int sp,
-                                        unsigned pid, int side, bool escaped, double& x, double& vx, double& vy,
-                                        double& vz, PairBirth& pb) {
+                                        unsigned pid, unsigned gidx, int side, bool escaped, double& x, double& vx,
+                                        double& vy, double& vz, PairBirth& pb) {
   const SpeciesP& s = S[sp];
   if (EMIT) {
     if (escaped) {
@@ -46,6 +46,21 @@ __device__ __noinline__ bool wall_event(const Params& P, const SpeciesP* S, unsi
     }
     atomicAdd(&P.st->wall_count[side][sp], 1ull);
     atomicAdd((unsigned long long*)&P.st->wall_charge[side], (unsigned long long)((long long)s.sign * s.Q));
+    if (s.recycle_to >= 0) {
+      // NEXT-2 wall recycling (reading N2-a): one particle of species recycle_to is born at
+      // the wall, half-Maxwellian into the plasma, from slot 14 of the parent's stream; the parent's fourth birth
+      const uint4 wr = draw(P, pid, step, 14u);
+      double z0 = normal_from_word(P, wr.x);
+      if (z0 < 0.0) z0 = -z0;
+      const double vz0 = s.recycle_vth * z0;
+      const double rvx = side == 0 ? vz0 : -vz0;
+      const double rvy = s.recycle_vth * normal_from_word(P, wr.y);
+      const double rvz = s.recycle_vth * normal_from_word(P, wr.z);
+      const double rx = side == 0 ? 0.0 : P.L - P.dx * 9.5367431640625e-07;
+      const int rc = side == 0 ? 0 : P.nc - 1;
+      emit_record(P, make_key(rc, 2u, (unsigned long long)gidx * 4ull + 3ull), rx, rvx, rvy, rvz, 0u, s.recycle_to);
+      atomicAdd(&P.st->recycled, 1ull);
+    }
   }
   if (s.src_mode == kSrcNone) return false;
   const uint4 w = draw(P, pid, step, 2u);  // slot RJ
@@ -183,7 +198,7 @@ __device__ __forceinline__ void advance(const Params& P, const SpeciesP* S, unsi
   } else if (!(x >= 0.0 && x < P.L)) {
     const int side = (x >= P.L) ? 1 : 0;
     const bool escaped = !(x < 0.0) && !(x >= P.L);  // NaN
-    alive = wall_event<EMIT>(P, S, step, sp, pid, side, escaped, x, vx, vy, vz, pb);
+    alive = wall_event<EMIT>(P, S, step, sp, pid, gidx, side, escaped, x, vx, vy, vz, pb);
   }
   const int cn = alive ? cell_of(P, x) : -1;
   // C

@@ -24,7 +24,7 @@ constexpr int kMaxSig = 16384;
 constexpr int kMaxNorm = 1 << 20;
 constexpr int kMaxR = 4;
 constexpr size_t kAlign = 256;
-constexpr uint32_t kCkptVersion = 2;   // 2: + averaging sums (NEXT-1)
+constexpr uint32_t kCkptVersion = 3;   // 2: + averaging sums (NEXT-1); 3: + recycling counter (NEXT-2)
 
 // sort window radius in cells (reading R-win); BIT1_WINDOW_R overrides it for the tests
 inline int window_R() {
@@ -172,7 +172,7 @@ struct bit1_ctx {
   cudaEvent_t ev_snap, ev_done;
   bool ckpt_pending, staging, loaded;
   int variant;
-  uint64_t launches, cfg_hash;
+  uint64_t launches, cfg_hash, cfg_hash_base;
   double m[BIT1_MAX_SPECIES], weight[BIT1_MAX_SPECIES];
   double dt;
   bool profiling;
@@ -297,6 +297,7 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
     q.Q = llrint((kECharge * sp[s].weight) * 1099511627776.0);
     q.sign = sp[s].q > 0.0 ? 1 : (sp[s].q < 0.0 ? -1 : 0);
     q.flags = sp[s].flags; q.src_mode = sp[s].src_mode; q.src_partner = sp[s].src_partner;
+    q.recycle_to = -1; q.recycle_vth = 0.0;
     if (q.Q < 1 || q.Q >= (1ll << 31)) { delete c; return BIT1_ERR_RANGE; }
     if ((unsigned long long)q.Q * (unsigned long long)kTile >= (1ull << 32) || q.Q >= (1ll << 21)) P.dep_u32 = 0;
     c->m[s] = sp[s].m; c->weight[s] = sp[s].weight;
@@ -354,6 +355,11 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
     h = fnv1a(h, o->sig_cx, (size_t)o->n_sig * 8);
   }
   h = fnv1a(h, o->inv_norm, (size_t)(o->n_norm + 1) * 8);
+  c->cfg_hash_base = h;
+  for (int s = 0; s < ns; ++s) {   // the recycling settings (bit1_set_recycling) are hashed on top of the base
+    h = fnv1a(h, &P.sp[s].recycle_to, 4);
+    h = fnv1a(h, &P.sp[s].recycle_vth, 8);
+  }
   c->cfg_hash = h;
 
   bool ok = true;
@@ -424,6 +430,20 @@ static bit1_status push_settings(bit1_ctx* c, bool clear_sums) {
     CUDA_OK(cudaMemsetAsync(&c->P.st->acc_count, 0, 3 * sizeof(unsigned long long), c->cs));
   }
   CUDA_OK(cudaStreamSynchronize(c->cs));   // v is a stack object
+  return BIT1_OK;
+}
+
+bit1_status bit1_set_recycling(bit1_ctx* c, int species, int to, double vth) {
+  if (!c || species < 0 || species >= c->P.ns || to >= c->P.ns || (to >= 0 && !(vth >= 0.0))) return BIT1_ERR_INVALID_ARG;
+  c->P.sp[species].recycle_to = to < 0 ? -1 : to;
+  c->P.sp[species].recycle_vth = to < 0 ? 0.0 : vth;
+  // configuration hash: recomputed from the base hash and every species' setting, so the order of calls is irrelevant
+  uint64_t h = c->cfg_hash_base;
+  for (int s = 0; s < c->P.ns; ++s) {
+    h = fnv1a(h, &c->P.sp[s].recycle_to, 4);
+    h = fnv1a(h, &c->P.sp[s].recycle_vth, 8);
+  }
+  c->cfg_hash = h;
   return BIT1_OK;
 }
 
@@ -631,7 +651,7 @@ bit1_status bit1_get_moments(bit1_ctx* c, bit1_moments* out) {
   out->rho_total_fixed = h.rho_total;
   out->flags = h.flags; out->next_pid = h.next_pid;
   out->nu_overflow = h.nu_overflow; out->dir_fallback = h.dir_fallback; out->escape = h.escape;
-  out->births = h.births; out->reinject = h.reinject;
+  out->births = h.births; out->reinject = h.reinject; out->recycled = h.recycled;
   out->far_movers = h.far_movers; out->max_far_movers_per_step = h.max_far_movers;
   bool any = false;
   for (int k = 0; k < P.ns; ++k) any = any || dens_out[k];

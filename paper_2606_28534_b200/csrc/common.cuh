@@ -48,6 +48,8 @@ struct __align__(16) SpeciesP {
   int sign;
   unsigned flags;
   int src_mode, src_partner;
+  int recycle_to, pad_;      // NEXT-2: species born at the wall when this one is absorbed (-1 = none)
+  double recycle_vth;
 };
 
 // SoA particle store: 41 B per particle.
@@ -78,7 +80,7 @@ struct DevState {
   unsigned ovf_valid; // side-list entries that k_mid placed (ovf_count minus dropped births)
   unsigned long long wall_count[2][kMaxSpecies];
   long long wall_charge[2];
-  unsigned long long nu_overflow, dir_fallback, escape, births, reinject;
+  unsigned long long nu_overflow, dir_fallback, escape, births, reinject, recycled;
   unsigned long long candidates[kMaxSpecies];
   unsigned long long events[kMaxSpecies][3];
   unsigned long long far_movers, max_far_movers;

@@ -55,6 +55,7 @@ def assert_state_equal(g, o, *, tol_state=1e-12, where=""):
         f"{where} MC event counters"
     assert (mg["births"], mg["reinject"], mg["nu_overflow"], mg["dir_fallback"], mg["escape"]) == \
         (d["births"], d["reinject"], d["nu_overflow"], d["dir_fallback"], d["escape"]), f"{where} diagnostics"
+    assert mg["recycled"] == o.recycled, f"{where} recycling events"
     assert mg["flags"] == o.flagword, f"{where} flags {mg['flags']} vs {o.flagword}"
     assert mg["rho_total"] == int(o.rho().sum())
     return exact
