@@ -202,6 +202,17 @@ bit1_status bit1_checkpoint(bit1_ctx *ctx, void *pinned_host, size_t cap, size_t
 bit1_status bit1_checkpoint_wait(bit1_ctx *ctx);
 bit1_status bit1_restart(bit1_ctx *ctx, const void *blob_host, size_t bytes);
 
+/* Export of one species in the paper's checkpoint layout ("per-species particle records ... the vector of
+ * particle counts per cell ... local extents and offsets ... load the position and velocity records"; SURVEY 8(f)
+ * NEXT-4): counts_per_cell (HOST, nc entries) and the species' records in cell order, inside a cell in the store's
+ * order (HOST, *n_out entries each; any of them may be NULL; pid is the library's own addition, needed to continue a
+ * run with the same random streams).  With all record pointers NULL it only returns *n_out and the counts (size
+ * query); BIT1_ERR_CAPACITY (with *n_out set) if capacity_out < *n_out.  Waits for a pending checkpoint and for the
+ * compute stream; uses the idle half of the particle store as staging, the live state is untouched. */
+bit1_status bit1_export_species(bit1_ctx *ctx, int species, uint64_t capacity_out, uint64_t *n_out,
+                                int64_t *counts_per_cell, double *x, double *vx, double *vy, double *vz,
+                                uint32_t *pid_or_null);
+
 void bit1_destroy(bit1_ctx *ctx);
 const char *bit1_error_string(bit1_status s);
 /* Per-kernel device timing for the roofline report.  While enabled, bit1_step

@@ -111,6 +111,8 @@ def load_library(path: Optional[str] = None):
     L.bit1_checkpoint_wait.argtypes = [vp]
     L.bit1_restart.restype = C.c_int
     L.bit1_restart.argtypes = [vp, vp, C.c_size_t]
+    L.bit1_export_species.restype = C.c_int
+    L.bit1_export_species.argtypes = [vp, C.c_int, C.c_uint64, C.POINTER(C.c_uint64), vp, vp, vp, vp, vp, vp]
     L.bit1_destroy.restype = None
     L.bit1_destroy.argtypes = [vp]
     L.bit1_error_string.restype = C.c_char_p
@@ -363,6 +365,20 @@ class Bit1:
 
     def restart(self, blob):
         _check(self.lib.bit1_restart(self.h, blob.data_ptr(), blob.numel()), "bit1_restart")
+
+    def export_species(self, species: int):
+        """One species in the paper's checkpoint layout: dict(counts[nc] int64, x, vx, vy, vz, pid) in cell order."""
+        n = C.c_uint64()
+        counts = np.zeros(self.nc, np.int64)
+        _check(self.lib.bit1_export_species(self.h, int(species), 0, C.byref(n), counts.ctypes.data, None, None, None,
+                                            None, None), "bit1_export_species (size query)")
+        m = int(n.value)
+        d = dict(x=np.zeros(m), vx=np.zeros(m), vy=np.zeros(m), vz=np.zeros(m), pid=np.zeros(m, np.uint32))
+        _check(self.lib.bit1_export_species(self.h, int(species), m, C.byref(n), counts.ctypes.data, d["x"].ctypes.data,
+                                            d["vx"].ctypes.data, d["vy"].ctypes.data, d["vz"].ctypes.data,
+                                            d["pid"].ctypes.data), "bit1_export_species")
+        d["counts"] = counts
+        return d
 
     def profile(self, enable: bool = True):
         _check(self.lib.bit1_profile(self.h, int(enable)), "bit1_profile")

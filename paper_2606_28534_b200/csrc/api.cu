@@ -137,6 +137,7 @@ Layout make_layout(int nc, int bc, int ns, size_t cap, int staging) {
   l.part[0] = take(pl.bytes);
   l.part[1] = take(pl.bytes);
   l.scratch_bytes = load_scratch_bytes((unsigned)cap);
+  if (export_scratch_bytes(nc, (unsigned)cap) > l.scratch_bytes) l.scratch_bytes = export_scratch_bytes(nc, (unsigned)cap);
   if (staging) {
     const size_t cb = ckpt_layout(nc, l.ng, ns, cap).bytes;
     if (cb > l.scratch_bytes) l.scratch_bytes = cb;
@@ -708,6 +709,43 @@ bit1_status bit1_get_particles(bit1_ctx* c, double* x, double* vx, double* vy, d
     free(cs32);
   }
   return e == cudaSuccess ? BIT1_OK : BIT1_ERR_CUDA;
+}
+
+bit1_status bit1_export_species(bit1_ctx* c, int species, uint64_t capacity_out, uint64_t* n_out,
+                                int64_t* counts_per_cell, double* x, double* vx, double* vy, double* vz,
+                                uint32_t* pid) {
+  if (!c || species < 0 || species >= c->P.ns || !n_out) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; }  // staging area = scratch
+  char* sc = c->ws + c->lay.scratch;
+  c->launches += launch_export_count(c->P, c->buf[c->cur], species, c->P.capacity, sc, c->cs);
+  unsigned long long total = 0;
+  CUDA_OK(cudaMemcpyAsync(&total, sc, 8, cudaMemcpyDeviceToHost, c->cs));
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  *n_out = total;
+  if (counts_per_cell) {
+    int32_t* tmp = static_cast<int32_t*>(malloc((size_t)c->P.nc * 4));
+    if (!tmp) return BIT1_ERR_INVALID_ARG;
+    cudaError_t e = cudaMemcpyAsync(tmp, sc + 256, (size_t)c->P.nc * 4, cudaMemcpyDeviceToHost, c->cs);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->cs);
+    if (e == cudaSuccess) for (int j = 0; j < c->P.nc; ++j) counts_per_cell[j] = tmp[j];
+    free(tmp);
+    if (e != cudaSuccess) return BIT1_ERR_CUDA;
+  }
+  if (!x && !vx && !vy && !vz && !pid) return BIT1_OK;   // size query
+  if (capacity_out < total) return BIT1_ERR_CAPACITY;
+  // the other particle buffer is free between steps: the records are compacted into it, then copied out
+  const Particles& out = c->buf[c->cur ^ 1];
+  c->launches += launch_export_scatter(c->P, c->buf[c->cur], out, species, sc, c->cs);
+  const size_t n = (size_t)total;
+  if (x) CUDA_OK(cudaMemcpyAsync(x, out.x, n * 8, cudaMemcpyDeviceToHost, c->cs));
+  if (vx) CUDA_OK(cudaMemcpyAsync(vx, out.vx, n * 8, cudaMemcpyDeviceToHost, c->cs));
+  if (vy) CUDA_OK(cudaMemcpyAsync(vy, out.vy, n * 8, cudaMemcpyDeviceToHost, c->cs));
+  if (vz) CUDA_OK(cudaMemcpyAsync(vz, out.vz, n * 8, cudaMemcpyDeviceToHost, c->cs));
+  if (pid) CUDA_OK(cudaMemcpyAsync(pid, out.pid, n * 4, cudaMemcpyDeviceToHost, c->cs));
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  CUDA_OK(cudaGetLastError());
+  return BIT1_OK;
 }
 
 bit1_status bit1_set_E(bit1_ctx* c, const double* E, int freeze) {

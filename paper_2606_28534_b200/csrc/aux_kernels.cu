@@ -259,3 +259,102 @@ int launch_moments(const Params& P, const Particles& cur, double* partial, doubl
 size_t moments_scratch_bytes() { return ((size_t)kMomBlocks + 2) * kMaxSpecies * 3 * 8 + 256; }
 
 }  // namespace bit1
+
+// ---------------------------------------------------------------------------------------------
+// Export of one species in the paper's checkpoint layout (per species, a counts-per-cell vector, then the
+// position and velocity records in that order).  The store is sorted by cell, so the records of one
+// species in cell order are a stable compaction: count per 1024-particle chunk, exclusive scan, scatter.
+namespace bit1 {
+constexpr int kExpChunk = 1024;
+
+__global__ void __launch_bounds__(256) k_export_count(const __grid_constant__ Params P, Particles cur, int species,
+                                                      unsigned* chunk_cnt, int* cell_cnt, unsigned long long* total) {
+  __shared__ unsigned s_cnt;
+  const unsigned n = P.st->n;
+  const unsigned nchunks = (n + kExpChunk - 1) / kExpChunk;
+  for (unsigned ch = blockIdx.x; ch < nchunks; ch += gridDim.x) {
+    if (threadIdx.x == 0) s_cnt = 0;
+    __syncthreads();
+    unsigned mine = 0;
+    for (int r = 0; r < kExpChunk / 256; ++r) {
+      const unsigned i = ch * kExpChunk + r * 256 + threadIdx.x;
+      const bool hit = i < n && cur.sp[i] == (unsigned char)species;
+      // neighbours mostly share the cell: one atomic per run of the warp
+      const unsigned key = hit ? (unsigned)cur.cell[i] : 0xffffffffu - (threadIdx.x & 31);
+      const unsigned m = __match_any_sync(0xffffffffu, key);
+      if (hit) {
+        mine++;
+        if ((int)(threadIdx.x & 31) == __ffs(m) - 1) atomicAdd(&cell_cnt[key], __popc(m));
+      }
+    }
+    if (mine) atomicAdd(&s_cnt, mine);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      chunk_cnt[ch] = s_cnt;
+      if (s_cnt) atomicAdd(total, (unsigned long long)s_cnt);
+    }
+    __syncthreads();
+  }
+}
+
+__global__ void __launch_bounds__(256) k_export_scatter(const __grid_constant__ Params P, Particles cur, Particles out,
+                                                        int species, const unsigned* chunk_off) {
+  __shared__ unsigned s_warp[8];
+  __shared__ unsigned s_base;
+  const unsigned n = P.st->n;
+  const unsigned nchunks = (n + kExpChunk - 1) / kExpChunk;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (unsigned ch = blockIdx.x; ch < nchunks; ch += gridDim.x) {
+    if (threadIdx.x == 0) s_base = chunk_off[ch];
+    __syncthreads();
+    for (int r = 0; r < kExpChunk / 256; ++r) {
+      const unsigned i = ch * kExpChunk + r * 256 + threadIdx.x;
+      const bool hit = i < n && cur.sp[i] == (unsigned char)species;
+      const unsigned b = __ballot_sync(0xffffffffu, hit);
+      if (lane == 0) s_warp[warp] = __popc(b);
+      __syncthreads();
+      unsigned before = 0, tot = 0;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) {
+        const unsigned c = s_warp[w];
+        if (w < warp) before += c;
+        tot += c;
+      }
+      if (hit) {
+        const unsigned d = s_base + before + __popc(b & ((1u << lane) - 1u));
+        out.x[d] = cur.x[i]; out.vx[d] = cur.vx[i]; out.vy[d] = cur.vy[i]; out.vz[d] = cur.vz[i];
+        out.pid[d] = cur.pid[i];
+      }
+      __syncthreads();
+      if (threadIdx.x == 0) s_base += tot;
+      __syncthreads();
+    }
+  }
+}
+
+// scratch: [total u64 | pad to 256][cell_cnt int[nc]][chunk_cnt unsigned[nchunks]]
+size_t export_scratch_bytes(int nc, unsigned capacity) {
+  return 256 + (((size_t)nc * 4 + 255) & ~(size_t)255) + ((size_t)(capacity + kExpChunk - 1) / kExpChunk) * 4 + 256;
+}
+
+int launch_export_count(const Params& P, const Particles& cur, int species, unsigned capacity, void* scratch,
+                        cudaStream_t s) {
+  char* b = static_cast<char*>(scratch);
+  unsigned long long* total = reinterpret_cast<unsigned long long*>(b);
+  int* cell_cnt = reinterpret_cast<int*>(b + 256);
+  unsigned* chunk_cnt = reinterpret_cast<unsigned*>(b + 256 + (((size_t)P.nc * 4 + 255) & ~(size_t)255));
+  const size_t nchunks_max = ((size_t)capacity + kExpChunk - 1) / kExpChunk;
+  cudaMemsetAsync(b, 0, 256 + (((size_t)P.nc * 4 + 255) & ~(size_t)255) + nchunks_max * 4, s);
+  k_export_count<<<148 * 8, 256, 0, s>>>(P, cur, species, chunk_cnt, cell_cnt, total);
+  k_scan_u32<<<1, 1024, 0, s>>>(chunk_cnt, nchunks_max);
+  return 2;
+}
+
+int launch_export_scatter(const Params& P, const Particles& cur, const Particles& out, int species, void* scratch,
+                          cudaStream_t s) {
+  char* b = static_cast<char*>(scratch);
+  const unsigned* chunk_off = reinterpret_cast<const unsigned*>(b + 256 + (((size_t)P.nc * 4 + 255) & ~(size_t)255));
+  k_export_scatter<<<148 * 8, 256, 0, s>>>(P, cur, out, species, chunk_off);
+  return 1;
+}
+}  // namespace bit1

@@ -11,3 +11,13 @@ size_t load_scratch_bytes(unsigned capacity);
 int launch_moments(const Params& P, const Particles& cur, double* partial, double* out, cudaStream_t s);
 size_t moments_scratch_bytes();
 }  // namespace bit1
+
+namespace bit1 {
+// NEXT-4: one species in the paper's checkpoint layout (counts per cell, then records in cell order)
+size_t export_scratch_bytes(int nc, unsigned capacity);
+// scratch afterwards: [0] total (u64), [256] cell_cnt int[nc], then exclusive chunk offsets
+int launch_export_count(const Params& P, const Particles& cur, int species, unsigned capacity, void* scratch,
+                        cudaStream_t s);
+int launch_export_scatter(const Params& P, const Particles& cur, const Particles& out, int species, void* scratch,
+                          cudaStream_t s);
+}  // namespace bit1
