@@ -177,6 +177,10 @@ struct bit1_ctx {
   double m[BIT1_MAX_SPECIES], weight[BIT1_MAX_SPECIES];
   double dt;
   bool profiling;
+  // two timesteps captured as one CUDA graph per starting parity of the ping-pong buffers (small workloads are bound by
+  // launch overhead: 8-10 launches, two of them cooperative, replayed with one call)
+  cudaGraphExec_t graph[2];
+  bool use_graph;
   std::vector<cudaEvent_t> prof_ev;  // 5 per timed step
   size_t prof_steps;
 };
@@ -254,6 +258,9 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   if (const char* ev = getenv("BIT1_VARIANT")) { const int v = atoi(ev); if (v == 1 || v == 2) c->variant = v; }
   c->cur = 0; c->loaded = false; c->ckpt_pending = false; c->launches = 0; c->dt = dt;
   c->profiling = false; c->prof_steps = 0;
+  c->graph[0] = c->graph[1] = nullptr;
+  c->use_graph = true;
+  if (const char* ev = getenv("BIT1_NO_GRAPH")) { if (atoi(ev) != 0) c->use_graph = false; }
 
   Params& P = c->P;
   P.nc = g->nc; P.bc = g->bc; P.ng = lay.ng; P.ns = ns;
@@ -380,9 +387,16 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   return BIT1_OK;
 }
 
+// the captured launches hold the settings by value: any change to them drops the graphs
+static void drop_graphs(bit1_ctx* c) {
+  for (int k = 0; k < 2; ++k)
+    if (c->graph[k]) { cudaGraphExecDestroy(c->graph[k]); c->graph[k] = nullptr; }
+}
+
 void bit1_destroy(bit1_ctx* c) {
   if (!c) return;
   cudaStreamSynchronize(c->cs);
+  drop_graphs(c);
   if (c->ss != c->cs) cudaStreamSynchronize(c->ss);
   cudaEventDestroy(c->ev_snap);
   cudaEventDestroy(c->ev_done);
@@ -424,6 +438,7 @@ static bit1_status read_state(bit1_ctx* c, DevState* h) {
 // The NEXT-1 settings live in the host-side Params (the launches read them) and ride along in DevState so that a
 // checkpoint carries them; clear_sums also zeroes the running and latched averaging sums.
 static bit1_status push_settings(bit1_ctx* c, bool clear_sums) {
+  drop_graphs(c);
   const int v[4] = {c->P.smooth, c->P.avg_window, c->P.avg_interval, 0};
   CUDA_OK(cudaMemcpyAsync(&c->P.st->smooth_passes, v, sizeof(v), cudaMemcpyHostToDevice, c->cs));
   if (clear_sums) {
@@ -436,6 +451,7 @@ static bit1_status push_settings(bit1_ctx* c, bool clear_sums) {
 
 bit1_status bit1_set_recycling(bit1_ctx* c, int species, int to, double vth) {
   if (!c || species < 0 || species >= c->P.ns || to >= c->P.ns || (to >= 0 && !(vth >= 0.0))) return BIT1_ERR_INVALID_ARG;
+  drop_graphs(c);
   c->P.sp[species].recycle_to = to < 0 ? -1 : to;
   c->P.sp[species].recycle_vth = to < 0 ? 0.0 : vth;
   // configuration hash: recomputed from the base hash and every species' setting, so the order of calls is irrelevant
@@ -487,6 +503,7 @@ bit1_status bit1_load_particles(bit1_ctx* c, uint64_t n, const double* x, const 
   if (!c || (n && (!x || !vx || !vy || !vz || !sp))) return BIT1_ERR_INVALID_ARG;
   if (n > c->P.capacity) return BIT1_ERR_CAPACITY;
   if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; }
+  drop_graphs(c);   // the buffer parity restarts at 0 while the cell_start swap keeps its state
   const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   Particles in = c->buf[1], outp = c->buf[0];
   CUDA_OK(cudaMemsetAsync(c->P.st, 0, sizeof(DevState), c->cs));
@@ -513,9 +530,48 @@ bit1_status bit1_load_particles(bit1_ctx* c, uint64_t n, const double* x, const 
   return BIT1_OK;
 }
 
+// one timestep enqueued on the compute stream (also under stream capture)
+static void enqueue_step(bit1_ctx* c, cudaEvent_t* ev) {
+  // the arrangement the last step (or load / restart) produced is this step's input
+  { int* t = c->P.cell_start; c->P.cell_start = c->P.cell_start_old; c->P.cell_start_old = t; }
+  c->launches += launch_step(c->P, c->buf[c->cur], c->buf[c->cur ^ 1], c->variant, c->cs, ev);
+  c->cur ^= 1;
+}
+
+// Two steps bring the buffer parity and the cell_start swap back to where they were, so a graph of two steps can be
+// replayed any number of times.  Returns false when capture is not possible (the caller then launches directly).
+static bool build_graph(bit1_ctx* c) {
+  const int par = c->cur;
+  const uint64_t launches0 = c->launches;
+  if (cudaStreamBeginCapture(c->cs, cudaStreamCaptureModeRelaxed) != cudaSuccess) { cudaGetLastError(); return false; }
+  enqueue_step(c, nullptr);
+  enqueue_step(c, nullptr);
+  cudaGraph_t g = nullptr;
+  const cudaError_t e = cudaStreamEndCapture(c->cs, &g);
+  c->launches = launches0;   // nothing ran yet
+  if (e != cudaSuccess || !g) { cudaGetLastError(); return false; }
+  cudaGraphExec_t ge = nullptr;
+  const cudaError_t e2 = cudaGraphInstantiate(&ge, g, 0);
+  cudaGraphDestroy(g);
+  if (e2 != cudaSuccess) { cudaGetLastError(); return false; }
+  c->graph[par] = ge;
+  return true;
+}
+
 bit1_status bit1_step(bit1_ctx* c, uint64_t nsteps) {
   if (!c) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
+  if (c->use_graph && !c->profiling && nsteps >= 4) {
+    if (!c->graph[c->cur] && !build_graph(c)) c->use_graph = false;
+    if (c->graph[c->cur]) {
+      const uint64_t per_step = (uint64_t)(c->P.avg_window > 0 ? 5 : 4);
+      while (nsteps >= 2) {
+        if (cudaGraphLaunch(c->graph[c->cur], c->cs) != cudaSuccess) return BIT1_ERR_CUDA;
+        c->launches += 2 * per_step;
+        nsteps -= 2;
+      }
+    }
+  }
   for (uint64_t k = 0; k < nsteps; ++k) {
     cudaEvent_t* ev = nullptr;
     if (c->profiling && c->prof_steps < kMaxProfSteps) {
@@ -527,10 +583,7 @@ bit1_status bit1_step(bit1_ctx* c, uint64_t nsteps) {
       ev = &c->prof_ev[c->prof_steps * 5];
       c->prof_steps++;
     }
-    // the arrangement the last step (or load / restart) produced is this step's input
-    { int* t = c->P.cell_start; c->P.cell_start = c->P.cell_start_old; c->P.cell_start_old = t; }
-    c->launches += launch_step(c->P, c->buf[c->cur], c->buf[c->cur ^ 1], c->variant, c->cs, ev);
-    c->cur ^= 1;
+    enqueue_step(c, ev);
   }
   CUDA_OK(cudaGetLastError());
   return BIT1_OK;
@@ -829,6 +882,7 @@ bit1_status bit1_restart(bit1_ctx* c, const void* blob, size_t bytes) {
       hd.bc != c->P.bc || hd.capacity != c->P.capacity || hd.cfg_hash != c->cfg_hash || hd.bytes != cl.bytes)
     return BIT1_ERR_CHECKPOINT;
   if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; }
+  drop_graphs(c);
   const PartLayout pl = part_layout(c->P.capacity);
   const char* hb = static_cast<const char*>(blob);
   DevState h;
