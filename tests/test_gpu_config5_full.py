@@ -20,6 +20,57 @@ pytestmark = pytest.mark.gpu
 FULL = os.environ.get("BIT1_FULL_C5") == "1"
 
 
+_ORDER = ["x", "vx", "vy", "vz", "cell", "pid", "sp"]
+_DT = dict(x=np.float64, vx=np.float64, vy=np.float64, vz=np.float64, cell=np.int32, pid=np.uint32, sp=np.uint8)
+
+
+def _fetch(g, name):
+    """One live array (8 GB at most) through bit1_get_particles, every other pointer NULL."""
+    a = np.empty(g.n_live(), _DT[name])
+    args = [None] * 8
+    args[_ORDER.index(name)] = a.ctypes.data
+    assert g.lib.bit1_get_particles(g.h, *args) == 0
+    return a
+
+
+def _sampled_oracle_step(g, w, k):
+    """Parity at full size on sampled outputs: 200 000 random particles plus the 20 000 nearest to each wall are advanced
+    one step by the oracle from the GPU's state and field at step k, and compared bit for bit (order included) with
+    what the GPU's own step k+1 makes of them."""
+    from oracle.oracle import Oracle
+
+    n = g.n_live()
+    rng = np.random.default_rng(20260628)
+    idx = np.unique(np.concatenate([rng.choice(n, size=200_000, replace=False), np.arange(0, 20_000),
+                                    np.arange(n - 20_000, n)]))
+    before = {name: _fetch(g, name)[idx] for name in ("x", "vx", "vy", "vz", "sp", "pid")}
+    E = g.get_E()
+    ws = W.make_config(5, particles=False)
+    ws.capacity = idx.shape[0] + 4096
+    o = Oracle(ws, load=False)
+    o.load(before["x"], before["vx"], before["vy"], before["vz"], before["sp"], pid=before["pid"])
+    o.set_E(E)
+    o.set_step(k)
+    o.step(1, freeze_field=True)
+    po = o.particles()
+    g.step(1)
+    g.sync()
+    m = g.get_moments()
+    pid_after = _fetch(g, "pid")
+    where = np.full(int(m["next_pid"]), -1, np.int64)
+    where[pid_after] = np.arange(pid_after.shape[0])
+    del pid_after
+    parents = np.isin(po["pid"], before["pid"])     # the oracle's own births carry other pids
+    pos = where[po["pid"][parents]]
+    del where
+    assert np.all(pos >= 0) and int(parents.sum()) == idx.shape[0]      # under SRC_SELF nobody dies
+    for name in ("x", "vx", "vy", "vz", "cell", "sp"):
+        a = _fetch(g, name)[pos]
+        assert np.array_equal(a, po[name][parents]), f"sampled particles at full size: {name} differs"
+    assert np.all(np.diff(pos) > 0), "sampled particles are not in the oracle's stable order"
+    return int(idx.shape[0])
+
+
 def _digest(g):
     """blake2b of every live array, fetched one at a time with bit1_get_particles (other pointers null)."""
     n = g.n_live()
@@ -61,7 +112,8 @@ def test_config5_full_size_checkpoint_every_50_steps_and_bit_identical_restart()
     blob = torch.empty(g.checkpoint_size(), dtype=torch.uint8).pin_memory()
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
     cs = g.compute_stream
-    g.step(3)   # warm-up (part of the 100)
+    g.step(2)   # warm-up (part of the 100)
+    n_sampled = _sampled_oracle_step(g, w, 2)   # takes step 3
     ev[0].record(cs)
     g.step(47)
     ev[1].record(cs)
@@ -100,7 +152,8 @@ def test_config5_full_size_checkpoint_every_50_steps_and_bit_identical_restart()
               "particle_steps_per_s_during_d2h": n0 / (ms_b * 1e-3),
               "checkpoint_bytes": int(blob.numel()), "steps_50_wall_s": t_steps_with_ckpt,
               "checkpoint_complete_wall_s": t_ckpt_done, "restart_s": t_restart, "births": m["births"],
-              "far_movers_per_step": far, "n_final": want["n"], "bit_identical": got == want}
+              "far_movers_per_step": far, "n_final": want["n"], "bit_identical": got == want,
+              "sampled_particles_bit_identical_to_oracle": n_sampled}
     os.makedirs("gpurun_out", exist_ok=True)
     with open("gpurun_out/config5_full.json", "w") as f:
         json.dump(report, f, indent=1)
