@@ -117,6 +117,8 @@ typedef struct {
   int32_t recycle_to[ORC_MAX_SPECIES];
   double recycle_vth[ORC_MAX_SPECIES];
   uint64_t diag_recycled;
+  int32_t target_species; /* -1: analytic uniform background n0; else the stored species whose density is the target */
+  double kn;
   /* NEXT-1: density smoothing and time-averaged diagnostics */
   int32_t smooth_passes; /* 0 = off */
   int64_t *rho_s;        /* ng: 4^passes * smoothed rho, what the field solve used */
@@ -264,6 +266,7 @@ orc *orc_create(int32_t nc, double dx, int32_t bc, double area, const double B[3
     o->two_e_over_m[s] = (2.0 * E_CHARGE) / m[s];
     o->el_loss[s] = (2.0 * m[s]) / m_n;
     o->recycle_to[s] = -1;
+    o->target_species = -1;
     o->Q[s] = (int64_t)llrint((E_CHARGE * weight[s]) * 1099511627776.0);
     o->sign[s] = q[s] > 0.0 ? 1 : (q[s] < 0.0 ? -1 : 0);
     if (o->Q[s] < 1 || o->Q[s] >= ((int64_t)1 << 31)) { free(o); return NULL; }
@@ -511,6 +514,12 @@ int orc_set_recycling(orc *o, int32_t s, int32_t to, double vth) {
   return 0;
 }
 uint64_t orc_recycled(const orc *o) { return o->diag_recycled; }
+int orc_set_neutral_target(orc *o, int32_t species) {
+  if (species >= o->ns) return 1;
+  o->target_species = species < 0 ? -1 : species;
+  if (species >= 0) o->kn = (0.5 * o->weight[species]) / (((double)o->Q[species] * o->area) * o->dx);
+  return 0;
+}
 
 void orc_set_smoothing(orc *o, int32_t passes) { o->smooth_passes = passes < 0 ? 0 : (passes > 8 ? 8 : passes); }
 /* (re)arms the averaging: running and latched sums are cleared */
@@ -669,10 +678,23 @@ void orc_phase_push(orc *o) {
         double g = sqrt(g2);
         double EeV = o->kin_eV[s] * g2;
         double r = u1 * o->numax[s];
+        /* NEXT-2, second half ("neutral particles as the collision target (density from dens_n instead
+         * of constant n0)"; reading N2-b): with a target species set, the neutral density a candidate sees is
+         * that species' density in the candidate's (new) cell, from the deposit of the previous step: the mean of the
+         * cell's two nodes, n = (D[c] + D[c+1]) * kn with kn = (0.5*weight_n) / ((Q_n*area)*dx).  o->dens still holds
+         * the previous step's deposit here (this step's comes after the sort).  numax keeps bounding the rate: it is
+         * the caller's, computed for the largest density it expects; beyond it nu_overflow counts, as before. */
+        double nloc = o->n0;
+        if (o->target_species >= 0) {
+          int32_t j1 = cn + 1;
+          if (!o->bc && j1 == o->nc) j1 = 0;
+          const int64_t *D = o->dens + (size_t)o->target_species * (size_t)o->ng;
+          nloc = (double)(D[cn] + D[j1]) * o->kn;
+        }
         double cum = 0.0;
         int chosen = -1;
         if (fl & F_ELASTIC) {
-          cum = cum + (o->n0 * sigma_lookup(o, o->sig_el, EeV)) * g;
+          cum = cum + (nloc * sigma_lookup(o, o->sig_el, EeV)) * g;
           if (chosen < 0 && r < cum) chosen = 0;
         }
         if (fl & F_IONISE) {
@@ -681,11 +703,11 @@ void orc_phase_push(orc *o) {
            * holds the threshold (13.5..14.0 eV for SURVEY's 0.5 eV table), and an ionisation picked there would
            * share out a negative energy E - E_ion (sqrt of a negative number: NaN velocities). */
           double sig_i = EeV > o->E_ion ? sigma_lookup(o, o->sig_ion, EeV) : 0.0;
-          cum = cum + (o->n0 * sig_i) * g;
+          cum = cum + (nloc * sig_i) * g;
           if (chosen < 0 && r < cum) chosen = 1;
         }
         if (fl & F_CX) {
-          cum = cum + (o->n0 * sigma_lookup(o, o->sig_cx, EeV)) * g;
+          cum = cum + (nloc * sigma_lookup(o, o->sig_cx, EeV)) * g;
           if (chosen < 0 && r < cum) chosen = 2;
         }
         if (cum > o->numax[s]) o->diag_nu_overflow += 1;

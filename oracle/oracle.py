@@ -82,6 +82,8 @@ def lib():
         L.orc_set_smoothing.argtypes = [C.c_void_p, C.c_int32]
         L.orc_set_recycling.restype = C.c_int
         L.orc_set_recycling.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double]
+        L.orc_set_neutral_target.restype = C.c_int
+        L.orc_set_neutral_target.argtypes = [C.c_void_p, C.c_int32]
         L.orc_recycled.restype = C.c_uint64
         L.orc_recycled.argtypes = [C.c_void_p]
         L.orc_set_averaging.restype = C.c_int
@@ -167,6 +169,8 @@ class Oracle:
                               int(inv_norm.shape[0] - 1))
         if not self.h:
             raise ValueError("orc_create rejected the configuration")
+        if getattr(w, "target_species", -1) >= 0:
+            self.set_neutral_target(w.target_species)
         for k, spc in enumerate(sp):
             if getattr(spc, "recycle_to", -1) >= 0:
                 self.set_recycling(k, spc.recycle_to, spc.recycle_vth)
@@ -271,6 +275,9 @@ class Oracle:
         r = np.zeros(self.ng, np.int64)
         lib().orc_get_rho(self.h, _p(r, c_i64p))
         return r
+
+    def set_neutral_target(self, species: int):
+        assert lib().orc_set_neutral_target(self.h, int(species)) == 0
 
     def set_recycling(self, s: int, to: int, vth: float):
         assert lib().orc_set_recycling(self.h, int(s), int(to), float(vth)) == 0

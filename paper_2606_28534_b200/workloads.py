@@ -78,6 +78,7 @@ class Workload:
     dE_eV: float
     inv_norm: np.ndarray
     steps: int
+    target_species: int = -1   # NEXT-2: species whose particle density is the collision target (-1: uniform n0)
     x: np.ndarray = field(repr=False, default=None)
     vx: np.ndarray = field(repr=False, default=None)
     vy: np.ndarray = field(repr=False, default=None)

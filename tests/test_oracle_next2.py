@@ -88,3 +88,81 @@ def test_every_absorbed_ion_becomes_one_inward_moving_neutral_and_charge_bookkee
     n_e, n_i = int((p["sp"] == 0).sum()), int((p["sp"] == 1).sum())
     assert int(o.rho().sum()) == -int(Q[0]) * n_e + int(Q[1]) * n_i
     assert np.array_equal(o.dens()[2].sum(), int(Q[2]) * int((p["sp"] == 2).sum()))
+
+
+# ---- second half of NEXT-2: the neutral particles' own density is the collision target (reading N2-b) ----------------
+
+AREA = 1e-10   # m^2: brings 1e9 real particles per macro-particle to 1e19 m^-3 while Q = e*weight*2^40 = 176 stays in range
+
+
+def _beam_in_neutrals(per_cell, E_eV=50.0, n_e_per_cell=400, nc=64, dt=1e-9):
+    """Electrons (elastic only, all at E_eV along +y so that they stay in their cells) in a periodic box whose cell c
+    holds per_cell[c] motionless neutrals at the cell centre: the target density of cell c is exactly
+    per_cell-averaged-over-its-two-nodes * weight / (area dx)."""
+    import math
+    dx, wgt = 1.0, 1e9
+    per_cell = np.asarray(per_cell)
+    v = math.sqrt(2 * E_eV * E_CH / M_E)
+    xe = np.repeat(np.arange(nc) + 0.5, n_e_per_cell)
+    xn = np.repeat(np.arange(nc) + 0.5, per_cell)
+    ne, nn = xe.shape[0], xn.shape[0]
+    n_max = per_cell.max() * wgt / (AREA * dx)
+    sp = [W.Species("e", -E_CH, M_E, wgt, flags=W.ELASTIC), W.Species("n", 0.0, M_D, wgt)]
+    w = W.make_custom(nc, dx, 0, dt, sp, capacity=ne + nn + 16, n0=n_max, seed=77, area=AREA,
+                      x=np.concatenate([xe, xn]), vx=np.zeros(ne + nn), vy=np.concatenate([np.full(ne, v), np.zeros(nn)]),
+                      vz=np.zeros(ne + nn), sp=np.concatenate([np.zeros(ne, np.uint8), np.ones(nn, np.uint8)]))
+    w.target_species = 1
+    return w, v, n_max
+
+
+def test_uniform_neutral_particles_reproduce_the_analytic_rate():
+    nc, k = 64, 5
+    w, v, n_max = _beam_in_neutrals(np.full(nc, k))
+    o = O.Oracle(w)
+    o.set_E(np.zeros(nc + 1))
+    o.step(1, freeze_field=True)
+    d = o.diag()
+    s = w.species[0]
+    n_e = int((w.sp == 0).sum())
+    p = s.pnull * (n_max * 1e-19 * v) / s.numax       # every cell sits at n_max: nodes hold Q*k, their mean is k
+    ev = int(d["events"][0][0])
+    assert ev > 300 and abs(ev - n_e * p) <= 4.0 * np.sqrt(n_e * p * (1 - p)) + 1
+    assert d["nu_overflow"] == 0
+    # same box, analytic background at the same density: the same particles collide (identical random streams)
+    w.target_species = -1
+    o2 = O.Oracle(w)
+    o2.set_E(np.zeros(nc + 1))
+    o2.step(1, freeze_field=True)
+    assert int(o2.diag()["events"][0][0]) == ev
+
+
+def test_event_rate_follows_the_local_neutral_density_and_vanishes_where_there_are_no_neutrals():
+    nc = 64
+    per = np.zeros(nc, np.int64)
+    per[8:24] = 2          # region A
+    per[40:56] = 6         # region B: three times denser
+    w, v, n_max = _beam_in_neutrals(per)
+    o = O.Oracle(w)
+    o.set_E(np.zeros(nc + 1))
+    before = o.particles()
+    o.step(1, freeze_field=True)
+    after = o.particles()
+    # an elastic event turns the velocity: find the electrons whose vy changed, by pid
+    b = {int(p): (c, vy) for p, c, vy, s in zip(before["pid"], before["cell"], before["vy"], before["sp"]) if s == 0}
+    hit_cells = [b[int(p)][0] for p, vy, s in zip(after["pid"], after["vy"], after["sp"]) if s == 0 and vy != b[int(p)][1]]
+    hits = np.bincount(hit_cells, minlength=nc)
+    assert hits.sum() == int(o.diag()["events"][0][0]) > 100
+    interior_a, interior_b = slice(9, 23), slice(41, 55)   # cells whose two nodes both sit inside the region
+    s = w.species[0]
+    n_e_cell = 400
+    for sl, k in ((interior_a, 2), (interior_b, 6)):
+        n = hits[sl].shape[0] * n_e_cell
+        p = s.pnull * ((k * 1e9 / AREA) * 1e-19 * v) / s.numax
+        assert abs(hits[sl].sum() - n * p) <= 4.0 * np.sqrt(n * p * (1 - p)) + 1
+    # no neutrals on either node of the cell: no events at all
+    empty = np.r_[0:7, 25:39, 57:64]
+    assert hits[empty].sum() == 0
+    # edge cells see the mean of their two nodes (half the region's density)
+    n = 2 * n_e_cell
+    p = s.pnull * ((3.0 * 1e9 / AREA) * 1e-19 * v) / s.numax
+    assert abs(hits[39] + hits[56] - n * p) <= 4.0 * np.sqrt(n * p * (1 - p)) + 1
