@@ -167,6 +167,15 @@ bit1_status bit1_get_particles(bit1_ctx *ctx, double *x, double *vx, double *vy,
  * configuration hash a checkpoint is validated against).  BIT1_ERR_INVALID_ARG for bad indices or vth < 0. */
 bit1_status bit1_set_recycling(bit1_ctx *ctx, int species, int to_species, double vth);
 
+/* Neutral particles as the collision target ("density from dens_n instead of constant n0"; PAPER.md:37
+ * natural sorting "accelerates collision operators"; reading N2-b): with `species` >= 0 every null-collision
+ * candidate uses the density of that stored species in its own (new) cell -- the mean of the cell's two nodes of the
+ * previous step's deposit -- in place of bit1_options.n0.  numax / pnull stay the caller's bound (computed for the
+ * largest density expected; beyond it bit1_moments.nu_overflow counts).  The neutrals themselves are not depleted or
+ * heated by the events.  -1 returns to the uniform background.  Part of the configuration hash: call before
+ * bit1_load_particles / bit1_restart. */
+bit1_status bit1_set_neutral_target(bit1_ctx *ctx, int species);
+
 /* Density smoothing ("density smoothing", "smoothing operators"; SURVEY 8(f) NEXT-1;
  * DESIGN.md reading N1-a): `passes` (0..8, 0 = off) passes of the 1-2-1 binomial filter over rho before every
  * field solve, in exact integers (each pass yields 4 x the smoothed array; the 1/4 is folded into the field

@@ -91,6 +91,8 @@ def load_library(path: Optional[str] = None):
     L.bit1_get_particles.argtypes = [vp] + [vp] * 8
     L.bit1_set_recycling.restype = C.c_int
     L.bit1_set_recycling.argtypes = [vp, C.c_int, C.c_int, C.c_double]
+    L.bit1_set_neutral_target.restype = C.c_int
+    L.bit1_set_neutral_target.argtypes = [vp, C.c_int]
     L.bit1_set_smoothing.restype = C.c_int
     L.bit1_set_smoothing.argtypes = [vp, C.c_int]
     L.bit1_get_rho_smoothed.restype = C.c_int
@@ -203,6 +205,8 @@ class Bit1:
         h = C.c_void_p()
         _check(self.lib.bit1_create(C.byref(g), sp, self.ns, w.dt, C.byref(o), C.byref(h)), "bit1_create")
         self.h = h
+        if getattr(w, "target_species", -1) >= 0:
+            self.set_neutral_target(w.target_species)
         for k, s in enumerate(w.species):   # NEXT-2: part of the configuration, set before any load or restart
             if getattr(s, "recycle_to", -1) >= 0:
                 self.set_recycling(k, s.recycle_to, s.recycle_vth)
@@ -316,6 +320,9 @@ class Bit1:
         if cell_start:
             d["cell_start"] = cs
         return d
+
+    def set_neutral_target(self, species: int):
+        _check(self.lib.bit1_set_neutral_target(self.h, int(species)), "bit1_set_neutral_target")
 
     def set_recycling(self, species: int, to_species: int, vth: float):
         _check(self.lib.bit1_set_recycling(self.h, int(species), int(to_species), float(vth)), "bit1_set_recycling")

@@ -101,20 +101,29 @@ __device__ __noinline__ void collide(const Params& P, const SpeciesP* S, unsigne
   const double g = sqrt(g2);
   const double EeV = s.kin_eV * g2;
   const double r = u1 * s.numax;
+  // NEXT-2 (reading N2-b): the target density is the neutral particles' own, in the candidate's new cell, from the
+  // previous step's deposit (mean of the cell's two nodes)
+  double nloc = P.n0;
+  if (P.target_species >= 0) {
+    int j1 = cn + 1;
+    if (!P.bc && j1 == P.nc) j1 = 0;
+    const long long* D = P.dens_old + (size_t)P.target_species * (size_t)P.ng;
+    nloc = (double)(D[cn] + D[j1]) * P.kn;
+  }
   double cum = 0.0;
   int chosen = -1;
   if (fl & kElastic) {
-    cum = cum + (P.n0 * sigma_lookup(P, P.sig_el, EeV)) * g;
+    cum = cum + (nloc * sigma_lookup(P, P.sig_el, EeV)) * g;
     if (chosen < 0 && r < cum) chosen = 0;
   }
   if (fl & kIonise) {
     // reading R-thr: zero at or below the threshold, whatever the table interpolates to there
     const double sig_i = EeV > P.E_ion ? sigma_lookup(P, P.sig_ion, EeV) : 0.0;
-    cum = cum + (P.n0 * sig_i) * g;
+    cum = cum + (nloc * sig_i) * g;
     if (chosen < 0 && r < cum) chosen = 1;
   }
   if (fl & kCx) {
-    cum = cum + (P.n0 * sigma_lookup(P, P.sig_cx, EeV)) * g;
+    cum = cum + (nloc * sigma_lookup(P, P.sig_cx, EeV)) * g;
     if (chosen < 0 && r < cum) chosen = 2;
   }
   if (EMIT && cum > s.numax) atomicAdd(&P.st->nu_overflow, 1ull);

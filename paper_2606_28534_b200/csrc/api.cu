@@ -88,7 +88,7 @@ CkptLayout ckpt_layout(int nc, int ng, int ns, size_t cap) {
 }
 
 struct Layout {
-  size_t st, tables, dens, rho, rho_s, rho_t, avg, phi, E, cell_count, cell_start, cell_start_old, scan_part, coop_scratch, cell_base, ovf_before, tile_hist, tile_base, tile_pre, evt,
+  size_t st, tables, dens, dens_old, rho, rho_s, rho_t, avg, phi, E, cell_count, cell_start, cell_start_old, scan_part, coop_scratch, cell_base, ovf_before, tile_hist, tile_base, tile_pre, evt,
       ovf_key, ovf_idx, ovf_dst, tmp_key, tmp_idx, ovf_rec, part[2], scratch, mom, total;
   unsigned ovf_cap, ovf_pow2;
   int max_tiles, ng;
@@ -109,6 +109,7 @@ Layout make_layout(int nc, int bc, int ns, size_t cap, int staging) {
   l.st = take(sizeof(DevState));
   l.tables = take(((size_t)3 * kMaxSig + kMaxNorm + 1) * 8);
   l.dens = take((size_t)ns * l.ng * 8);
+  l.dens_old = take((size_t)ns * l.ng * 8);
   l.rho = take((size_t)l.ng * 8);
   l.rho_s = take((size_t)l.ng * 8);
   l.rho_t = take((size_t)l.ng * 8);
@@ -191,6 +192,17 @@ constexpr size_t kMaxProfSteps = 4096;
     cudaError_t e_ = (call);                       \
     if (e_ != cudaSuccess) return BIT1_ERR_CUDA;   \
   } while (0)
+
+// configuration hash: recomputed from the base hash and the NEXT-2 settings, so the order of the calls is irrelevant
+static void rehash(bit1_ctx* c) {
+  uint64_t h = c->cfg_hash_base;
+  for (int s = 0; s < c->P.ns; ++s) {
+    h = fnv1a(h, &c->P.sp[s].recycle_to, 4);
+    h = fnv1a(h, &c->P.sp[s].recycle_vth, 8);
+  }
+  h = fnv1a(h, &c->P.target_species, 4);
+  c->cfg_hash = h;
+}
 
 extern "C" {
 
@@ -315,6 +327,8 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   double* tab = reinterpret_cast<double*>(ws + lay.tables);
   P.sig_el = tab; P.sig_ion = tab + kMaxSig; P.sig_cx = tab + 2 * kMaxSig; P.inv_norm = tab + 3 * kMaxSig;
   P.dens = reinterpret_cast<long long*>(ws + lay.dens);
+  P.dens_old = reinterpret_cast<long long*>(ws + lay.dens_old);
+  P.target_species = -1; P.kn = 0.0;
   P.rho = reinterpret_cast<long long*>(ws + lay.rho);
   P.rho_s = reinterpret_cast<long long*>(ws + lay.rho_s);
   P.rho_t = reinterpret_cast<long long*>(ws + lay.rho_t);
@@ -364,11 +378,7 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   }
   h = fnv1a(h, o->inv_norm, (size_t)(o->n_norm + 1) * 8);
   c->cfg_hash_base = h;
-  for (int s = 0; s < ns; ++s) {   // the recycling settings (bit1_set_recycling) are hashed on top of the base
-    h = fnv1a(h, &P.sp[s].recycle_to, 4);
-    h = fnv1a(h, &P.sp[s].recycle_vth, 8);
-  }
-  c->cfg_hash = h;
+  rehash(c);   // the NEXT-2 settings (bit1_set_recycling, bit1_set_neutral_target) are hashed on top of the base
 
   bool ok = true;
   ok = ok && cudaMemsetAsync(ws + lay.st, 0, lay.part[0] - lay.st, c->cs) == cudaSuccess;  // state, grids, lists
@@ -454,13 +464,17 @@ bit1_status bit1_set_recycling(bit1_ctx* c, int species, int to, double vth) {
   drop_graphs(c);
   c->P.sp[species].recycle_to = to < 0 ? -1 : to;
   c->P.sp[species].recycle_vth = to < 0 ? 0.0 : vth;
-  // configuration hash: recomputed from the base hash and every species' setting, so the order of calls is irrelevant
-  uint64_t h = c->cfg_hash_base;
-  for (int s = 0; s < c->P.ns; ++s) {
-    h = fnv1a(h, &c->P.sp[s].recycle_to, 4);
-    h = fnv1a(h, &c->P.sp[s].recycle_vth, 8);
-  }
-  c->cfg_hash = h;
+  rehash(c);
+  return BIT1_OK;
+}
+
+bit1_status bit1_set_neutral_target(bit1_ctx* c, int species) {
+  if (!c || species >= c->P.ns) return BIT1_ERR_INVALID_ARG;
+  drop_graphs(c);
+  c->P.target_species = species < 0 ? -1 : species;
+  c->P.kn = species < 0 ? 0.0
+                        : (0.5 * c->weight[species]) / (((double)c->P.sp[species].Q * c->P.area) * c->P.dx);
+  rehash(c);
   return BIT1_OK;
 }
 
@@ -534,6 +548,7 @@ bit1_status bit1_load_particles(bit1_ctx* c, uint64_t n, const double* x, const 
 static void enqueue_step(bit1_ctx* c, cudaEvent_t* ev) {
   // the arrangement the last step (or load / restart) produced is this step's input
   { int* t = c->P.cell_start; c->P.cell_start = c->P.cell_start_old; c->P.cell_start_old = t; }
+  { long long* t = c->P.dens; c->P.dens = c->P.dens_old; c->P.dens_old = t; }
   c->launches += launch_step(c->P, c->buf[c->cur], c->buf[c->cur ^ 1], c->variant, c->cs, ev);
   c->cur ^= 1;
 }

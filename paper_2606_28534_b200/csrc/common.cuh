@@ -107,7 +107,10 @@ struct Params {
   const double *sig_el, *sig_ion, *sig_cx, *inv_norm;
   DevState *st;
   // grids
-  long long *dens;  // ns * ng
+  long long *dens;  // ns * ng: this step's deposit (cleared in pass A, accumulated in pass B)
+  long long *dens_old;  // ns * ng: the previous step's deposit (swapped with dens every step); read by collide()
+  int target_species;   // NEXT-2 (reading N2-b): species whose density is the collision target, -1 = uniform n0
+  double kn;            // (0.5 * weight_n) / ((Q_n * area) * dx): node pair sum -> density of the cell
   long long *rho;   // ng
   double *phi, *E;  // nc + 1
   // NEXT-1 (density smoothing, time-averaged diagnostics; readings N1-a, N1-b)

@@ -64,3 +64,67 @@ def test_restart_with_recycling_and_rejection_without_it():
     with pytest.raises(Bit1Error):
         k.set_recycling(1, 2, -1.0)
     k.close()
+
+
+# ---- second half of NEXT-2: neutral particles as the collision target (reading N2-b) ---------------------------------
+
+def _boost_collisions(w, f=3000.0):
+    """Cut-down runs see few events at physical rates: scale the cross-section tables by f and bound the rate for 1.5 x
+    the largest neutral-particle density of the load (inputs only: the library sees tables, numax and pnull)."""
+    import math
+    neutrals = w.x[w.sp == 2]
+    peak = np.bincount(np.minimum((neutrals / w.dx).astype(np.int64), w.nc - 1), minlength=w.nc).max()
+    n_bound = 1.5 * peak * w.species[2].weight / (w.area * w.dx)
+    for name in ("sig_el", "sig_ion", "sig_cx"):
+        setattr(w, name, getattr(w, name) * f)
+    for s in w.species:
+        if s.numax > 0.0:
+            s.numax = s.numax * f * n_bound / w.n0
+            s.pnull = 1.0 - math.exp(-s.numax * w.dt)
+    w.target_species = 2
+
+
+@pytest.mark.parametrize("cfg,scale,steps", [(4, 1 / 2048, 100), (5, 1 / 8192, 60)])
+def test_neutral_particle_target_matches_oracle_bit_for_bit(cfg, scale, steps):
+    w = W.make_config(cfg, scale=scale, recycle=True)
+    _boost_collisions(w)
+    g, o = run_pair(w, steps)
+    d = o.diag()
+    assert d["events"].sum() > 200 and d["births"] > 20, "the workload was meant to collide"
+    assert assert_state_equal(g, o, where=f"c{cfg} neutral-particle target, {steps} steps")
+    assert_moments_close(g, o, tol=1e-9)
+    g.close()
+
+
+def test_neutral_particle_target_in_a_periodic_box_and_restart():
+    import torch
+    from oracle.oracle import Oracle
+    from paper_2606_28534_b200.binding import Bit1, Bit1Error, ERR_CHECKPOINT
+    from test_oracle_next2 import _beam_in_neutrals
+
+    per = np.zeros(64, np.int64)
+    per[8:24] = 2
+    per[40:64] = 6          # reaches the last cell: its right node is node 0 (periodic wrap)
+    w, v, n_max = _beam_in_neutrals(per)
+    g, o = run_pair(w, 6)
+    assert o.diag()["events"].sum() > 300
+    assert assert_state_equal(g, o, where="periodic box, neutral-particle target")
+    blob = torch.empty(g.checkpoint_size(), dtype=torch.uint8).pin_memory()
+    g.checkpoint(blob)
+    g.checkpoint_wait()
+    g.close()
+    h = Bit1(w)
+    h.restart(blob)
+    h.step(6)
+    h.sync(check_flags=False)
+    o.step(6)
+    assert assert_state_equal(h, o, where="restart, neutral-particle target")
+    h.close()
+    w.target_species = -1      # another configuration: the blob is rejected
+    k = Bit1(w)
+    with pytest.raises(Bit1Error) as e:
+        k.restart(blob)
+    assert e.value.status == ERR_CHECKPOINT
+    with pytest.raises(Bit1Error):
+        k.set_neutral_target(5)
+    k.close()
