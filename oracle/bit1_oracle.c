@@ -28,7 +28,12 @@
  * compile with -ffp-contract=off; no libm call inside a step (llrint, used
  * once at create time, is the only libm routine).
  *
- * Pins: see tests/test_oracle_*.py.  No function here is "parity unpinned".
+ * Beyond the hot path: density smoothing and time-averaged diagnostics (NEXT-1, readings N1-a/b),
+ * wall recycling and neutral particles as the collision target (NEXT-2, readings N2-a/b), and reading R-thr
+ * (ionisation cross-section zero at or below the threshold).
+ *
+ * Pins: see tests/test_oracle_*.py (NEXT-1: test_oracle_next1.py, NEXT-2: test_oracle_next2.py).  No function here
+ * is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
