@@ -93,6 +93,14 @@ def test_config4_full_size_invariants_and_sampled_oracle_parity():
     m = g.get_moments()
     before = g.get_particles()
     E = g.get_E()
+    # the field solve on 64 CTAs against the oracle's plain serial solve of the same rho (exact integers: any scan order
+    # must give these bits)
+    from oracle import oracle as OM
+    ob = Oracle(W.make_config(4, scale=scale, particles=False), load=False)
+    cst = ob.constants()
+    phi_o, E_o = OM.poisson(w.nc, w.bc, cst["Kphi"], cst["KE"], g.get_rho())
+    assert np.array_equal(E, E_o) and np.array_equal(g.get_phi(), phi_o), "field solve at full size"
+    del ob
     _check_invariants(w, before, g.get_rho(), g.get_dens(), m, n0 + m["births"], f"step {k}")
 
     # a sample of the particles: random ones, plus the ones nearest to both walls (they are absorbed and

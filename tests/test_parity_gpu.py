@@ -52,3 +52,17 @@ def test_hundred_steps_match_oracle(cfg, scale, kw, steps, variant):
     g, o = run_pair(w, steps, variant=variant)
     assert_state_equal(g, o, where=f"c{cfg} {steps} steps")
     assert_moments_close(g, o, tol=1e-9)
+
+
+@pytest.mark.parametrize("cfg,scale,kw", [
+    (4, 1 / 16, dict(n0_scale=30.0)),     # 1.25e7 particles, 4096 cells: 4 CTAs in the cooperative kernels, 41 tiles per CTA
+    (5, 1 / 64, dict(n0_scale=30.0)),     # 1.56e7 particles, 16384 cells: 16 CTAs in k_mid and k_field
+])
+def test_mid_size_state_matches_oracle_element_by_element(cfg, scale, kw):
+    """Large enough that the persistent passes reload their stages dozens of times and the cooperative kernels (cell
+    scan, column scan, field solve) run on several CTAs, small enough for the oracle: every element compared."""
+    w = small(cfg, scale, **kw)
+    g, o = run_pair(w, 3)
+    exact = assert_state_equal(g, o, where=f"c{cfg} x{scale:g}, 3 steps")
+    assert exact, "fp64 state, phi and E are within tolerance but not bit-identical"
+    g.close()
