@@ -261,6 +261,10 @@ def run_cuda(args):
     e2e_ms_max, e2e_units = aggregate(1e3 * e2e_s, float(n0) * args.steps, world, dev)
     d2h_bytes = rho.nbytes
 
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
     if rank != 0:
         return
     peak, peak_src = _peaks()
