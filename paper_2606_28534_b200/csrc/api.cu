@@ -171,7 +171,7 @@ struct bit1_ctx {
   int cur;
   char* ws;
   cudaStream_t cs, ss;
-  cudaEvent_t ev_snap, ev_done;
+  cudaEvent_t ev_snap, ev_done, ev_load0, ev_load1;
   bool ckpt_pending, staging, loaded;
   int variant;
   uint64_t launches, cfg_hash, cfg_hash_base;
@@ -392,6 +392,8 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   ok = ok && configure_kernels() == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&c->ev_snap, cudaEventDisableTiming) == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&c->ev_done, cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaEventCreateWithFlags(&c->ev_load0, cudaEventDisableTiming) == cudaSuccess;
+  ok = ok && cudaEventCreateWithFlags(&c->ev_load1, cudaEventDisableTiming) == cudaSuccess;
   if (!ok) { delete c; return BIT1_ERR_CUDA; }
   *out = c;
   return BIT1_OK;
@@ -410,6 +412,8 @@ void bit1_destroy(bit1_ctx* c) {
   if (c->ss != c->cs) cudaStreamSynchronize(c->ss);
   cudaEventDestroy(c->ev_snap);
   cudaEventDestroy(c->ev_done);
+  cudaEventDestroy(c->ev_load0);
+  cudaEventDestroy(c->ev_load1);
   for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
   delete c;
 }
@@ -522,17 +526,27 @@ bit1_status bit1_load_particles(bit1_ctx* c, uint64_t n, const double* x, const 
   Particles in = c->buf[1], outp = c->buf[0];
   CUDA_OK(cudaMemsetAsync(c->P.st, 0, sizeof(DevState), c->cs));
   { bit1_status ps = push_settings(c, true); if (ps != BIT1_OK) return ps; }
+  // x, species and pid feed the sort keys and go first on the compute stream; the velocities follow on the side stream
+  // while the sort runs and are only needed by its final gather
+  const bool split = n && c->ss != c->cs;
   if (n) {
     CUDA_OK(cudaMemcpyAsync(in.x, x, n * 8, kind, c->cs));
-    CUDA_OK(cudaMemcpyAsync(in.vx, vx, n * 8, kind, c->cs));
-    CUDA_OK(cudaMemcpyAsync(in.vy, vy, n * 8, kind, c->cs));
-    CUDA_OK(cudaMemcpyAsync(in.vz, vz, n * 8, kind, c->cs));
     CUDA_OK(cudaMemcpyAsync(in.sp, sp, n, kind, c->cs));
     if (pid) CUDA_OK(cudaMemcpyAsync(in.pid, pid, n * 4, kind, c->cs));
+    cudaStream_t vs = split ? c->ss : c->cs;
+    if (split) {
+      CUDA_OK(cudaEventRecord(c->ev_load0, c->cs));          // everything that used this half of the store is done
+      CUDA_OK(cudaStreamWaitEvent(c->ss, c->ev_load0, 0));
+    }
+    CUDA_OK(cudaMemcpyAsync(in.vx, vx, n * 8, kind, vs));
+    CUDA_OK(cudaMemcpyAsync(in.vy, vy, n * 8, kind, vs));
+    CUDA_OK(cudaMemcpyAsync(in.vz, vz, n * 8, kind, vs));
+    if (split) CUDA_OK(cudaEventRecord(c->ev_load1, c->ss));
   }
   const unsigned n32 = (unsigned)n;
   CUDA_OK(cudaMemcpyAsync(&c->P.st->n, &n32, 4, cudaMemcpyHostToDevice, c->cs));
-  c->launches += launch_load_sort(c->P, in, outp, n32, pid ? 1 : 0, c->ws + c->lay.scratch, c->cs);
+  c->launches += launch_load_sort(c->P, in, outp, n32, pid ? 1 : 0, c->ws + c->lay.scratch, c->cs,
+                                  split ? c->ev_load1 : nullptr);
   c->cur = 0;
   c->launches += launch_rebuild(c->P, c->buf[0], c->cs);
   CUDA_OK(cudaGetLastError());

@@ -214,7 +214,7 @@ __global__ void __launch_bounds__(256) k_gather(Particles in, Particles out, con
 }
 
 int launch_load_sort(const Params& P, const Particles& in, const Particles& out, unsigned n, int have_pid,
-                     void* scratch, cudaStream_t s) {
+                     void* scratch, cudaStream_t s, cudaEvent_t before_gather) {
   if (n == 0) return 0;
   int launches = 0;
   const unsigned nblocks = (n + kRadixChunk - 1) / kRadixChunk;
@@ -235,6 +235,7 @@ int launch_load_sort(const Params& P, const Particles& in, const Particles& out,
     unsigned* t = k0; k0 = k1; k1 = t;
     t = v0; v0 = v1; v1 = t;
   }
+  if (before_gather) cudaStreamWaitEvent(s, before_gather, 0);   // the velocity arrays arrive on another stream
   k_gather<<<148 * 8, 256, 0, s>>>(in, out, v0, n);
   return launches + 1;
 }

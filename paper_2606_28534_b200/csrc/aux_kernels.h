@@ -4,8 +4,9 @@
 
 namespace bit1 {
 // validate + cell index + general stable sort by cell of `in` (n particles) into `out`
+// before_gather: NULL, or an event the final gather waits for (arrays other than x, sp, pid still being copied)
 int launch_load_sort(const Params& P, const Particles& in, const Particles& out, unsigned n, int have_pid,
-                     void* scratch, cudaStream_t s);
+                     void* scratch, cudaStream_t s, cudaEvent_t before_gather);
 size_t load_scratch_bytes(unsigned capacity);
 // out: [kMaxSpecies*3] = (count, sum v^2, sum vx) per species, then sum g_j E_j^2
 int launch_moments(const Params& P, const Particles& cur, double* partial, double* out, cudaStream_t s);
