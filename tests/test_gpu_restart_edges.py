@@ -248,3 +248,39 @@ def test_error_behaviour_of_the_c_abi():
     with pytest.raises(Bit1Error) as e:
         Bit1(w)
     assert e.value.status == ERR_RANGE
+
+
+@pytest.mark.parametrize("cfg,scale,kw", [(2, 1 / 64, dict(pair_source=True)), (3, 1 / 256, dict(n0_scale=300.0))])
+def test_heavy_macro_particles_take_the_64_bit_deposit_path(cfg, scale, kw):
+    """Q_s >= 2^21 (here 400 x the workload's weight, with the cross-section area scaled alike so that the physics is
+    unchanged): the shared-memory uint32 deposit counters could overflow, so the kernel deposits with 64-bit global
+    reductions instead.  Same bits as the oracle."""
+    w = W.make_config(cfg, scale=scale, **kw)
+    w.area *= 400.0
+    for s in w.species:
+        s.weight *= 400.0
+    g, o = run_pair(w, 25)
+    assert int(o.Q().max()) >= 2**21
+    assert assert_state_equal(g, o, where=f"c{cfg} heavy macro-particles")
+    g.close()
+
+
+def test_eight_species():
+    """BIT1_MAX_SPECIES stored species with different masses, charges and weights in one periodic box."""
+    rng = np.random.default_rng(8)
+    nc, dx, n_per = 96, 2e-5, 900
+    sp = []
+    for k in range(8):
+        q = (-1.0, 1.0, 0.0, 2.0)[k % 4] * W.E_CHARGE
+        sp.append(W.Species(f"s{k}", q, W.M_E * (1 + 400 * k), 3e9 * (1 + k), src_vth=1e5))
+    n = 8 * n_per
+    tags = np.repeat(np.arange(8, dtype=np.uint8), n_per)
+    vth = np.array([4e5 / np.sqrt(1 + 400 * k) for k in range(8)])[tags]
+    w = W.make_custom(nc, dx, 0, 2e-12, sp, B=(0.3, 0.1, 0.2), capacity=n + 64, seed=88,
+                      x=rng.random(n) * nc * dx, vx=vth * rng.standard_normal(n), vy=vth * rng.standard_normal(n),
+                      vz=vth * rng.standard_normal(n), sp=tags)
+    g, o = run_pair(w, 30)
+    assert assert_state_equal(g, o, where="eight species")
+    assert_moments = __import__("parity").assert_moments_close
+    assert_moments(g, o, tol=1e-9)
+    g.close()
