@@ -341,6 +341,13 @@ __device__ void grid_bitonic(cg::grid_group& grid, unsigned long long* gkey, uns
   }
 }
 
+// One-CTA cooperative grids (small workloads) need no grid-wide barrier: a CTA barrier orders the block's own global
+// writes for its own threads, and saves the round trip through the barrier word in global memory.
+__device__ __forceinline__ void grid_or_cta_sync(cg::grid_group& grid) {
+  if (gridDim.x == 1) __syncthreads();
+  else grid.sync();
+}
+
 __device__ int block_exclusive_scan_int(int v, int* s_warp, int* total) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   int inc = v;
@@ -519,16 +526,19 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
       }
       __syncthreads();
       cta_sort(P.ovf_key, P.ovf_idx, P2, s_key, s_val);
-      Mv = lower_bound_u64(P.ovf_key, P2, kInvalidKey);
+      // the sorted keys are still in shared memory (P2 <= kSortSmem here): the binary searches below are chains of
+      // dependent loads, a few dozen ns each there against most of a microsecond each in global memory
+      const unsigned long long* K = s_key;
+      Mv = lower_bound_u64(K, P2, kInvalidKey);
       // (c) groups per cell: rank inside the group, group size joins the cell count
       for (unsigned p = threadIdx.x; p < Mv; p += blockDim.x) {
-        const unsigned long long key = P.ovf_key[p];
+        const unsigned long long key = K[p];
         const unsigned long long c = key >> kCellShift;
-        const unsigned lb = lower_bound_u64(P.ovf_key, Mv, c << kCellShift);
-        const unsigned ub = lower_bound_u64(P.ovf_key, Mv, (c + 1ull) << kCellShift);
+        const unsigned lb = lower_bound_u64(K, Mv, c << kCellShift);
+        const unsigned ub = lower_bound_u64(K, Mv, (c + 1ull) << kCellShift);
         const unsigned cls = (unsigned)((key >> kClsShift) & 3ull);
         if (p == lb) {
-          const unsigned ub0 = lower_bound_u64(P.ovf_key, Mv, (c << kCellShift) | (1ull << kClsShift));
+          const unsigned ub0 = lower_bound_u64(K, Mv, (c << kCellShift) | (1ull << kClsShift));
           P.cell_count[c] += (int)(ub - lb);
           P.ovf_before[c] = (int)(ub0 - lb);
         }
@@ -543,7 +553,7 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
     }
   }
   __threadfence();
-  grid.sync();
+  grid_or_cta_sync(grid);
 
   // phase 1: scan of the cell counts.  CTA b owns cells [c_lo, c_hi).
   const int nc = P.nc;
@@ -557,7 +567,7 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
     if (threadIdx.x == 0) P.scan_part[b] = sum;
   }
   __threadfence();
-  grid.sync();
+  grid_or_cta_sync(grid);
   int carry, total;
   {
     int mine = 0, all = 0;
@@ -598,7 +608,7 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
     st->n_next = (unsigned)total;
   }
   __threadfence();
-  grid.sync();
+  grid_or_cta_sync(grid);
 
   // phase 2
   const unsigned Mv = st->ovf_valid;
@@ -1009,7 +1019,7 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
     for (int k = 0; k < smooth; ++k) {
       long long* out = ((smooth - 1 - k) & 1) ? P.rho_t : P.rho_s;   // the last pass lands in rho_s
       __threadfence();
-      grid.sync();
+      grid_or_cta_sync(grid);
       for (int j = b * kFieldThreads + (int)threadIdx.x; j < ng; j += G * kFieldThreads) {
         long long v;
         if (bc) {
@@ -1025,7 +1035,7 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
       in = out;
     }
     __threadfence();
-    grid.sync();
+    grid_or_cta_sync(grid);
     R = P.rho_s;
     const double scale = 1.0 / (double)(1ll << (2 * smooth));   // exact power of two
     Kphi = Kphi * scale;
@@ -1048,7 +1058,7 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
   wsum = block_sum_128(wsum, s_warp);
   if (threadIdx.x == 0) { part[b] = tot; part[G + b] = wsum; }
   __threadfence();
-  grid.sync();
+  grid_or_cta_sync(grid);
   tot = 0; wsum = 0;
   for (int i = threadIdx.x; i < G; i += kFieldThreads) { tot += part[i]; wsum += part[G + i]; }
   tot = block_sum_128(tot, s_warp);
@@ -1069,7 +1079,7 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
     field_range<false>(P, R, Kphi, KE, j_lo, j_hi, tot, Tn, (i128)0, (i128)0, s_warp, &A, &C);
     if (threadIdx.x == 0) { part[2 * G + b] = A; part[3 * G + b] = C; }
     __threadfence();
-    grid.sync();
+    grid_or_cta_sync(grid);
     // phase C: S_{j_lo-1} = sum of A over earlier CTAs; T_{j_lo} = sum over earlier CTAs of (len * S_before + C)
     i128 myA = 0, myLen = 0, myC = 0;
     if ((int)threadIdx.x < G) {
