@@ -297,6 +297,9 @@ def run_cuda(args):
                      "achieved": b_bytes / (b_ms * 1e-3) / 1e9 if b_ms > 0 else None, "peak": peak, "unit": "GB/s",
                      "frac": (b_bytes / (b_ms * 1e-3) / 1e9 / peak) if b_ms > 0 else None,
                      "traffic": _traffic("k_pass_b", args), "peak_source": peak_src,
+                     "measured_in": f"a second leg of {int(psteps)} steps right after the timed region, same state, direct "
+                                    "launches with CUDA events around every kernel on the compute stream (the timed "
+                                    "region itself replays two-step CUDA graphs and has no per-kernel events)",
                      "bytes_per_particle": b_bpp,
                      "pass_a": {"achieved": a_bytes / (a_ms * 1e-3) / 1e9 if a_ms > 0 else None,
                                 "bytes_per_particle": a_bytes / n_mean, "traffic": _traffic("k_pass_a", args)},
