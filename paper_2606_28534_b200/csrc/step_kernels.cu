@@ -630,14 +630,29 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
       if (lo >= (int)n || hi < 0) continue;
       const int t0 = lo / kTile, t1 = hi / kTile;
       int run = P.cell_base[c];
-      for (int t = t0; t <= t1; ++t) {
-        const int2 d = cur.desc[t];
-        const TileWin tw = make_window(d.x, d.y, R);
-        const int k = c - tw.wlo;
-        if (k >= 0 && k < tw.W) {
-          const size_t off = tile_row_offset(d.x, t, R) + (size_t)k;
-          P.tile_base[off] = run;
-          run += (int)P.tile_hist[off];
+      // four tiles at a time: the descriptor and count loads of a batch are independent of one another, only the running
+      // sum is serial (a dense cell is covered by dozens of tiles, and every load is a trip to L2)
+      for (int tb4 = t0; tb4 <= t1; tb4 += 4) {
+        int2 d[4];
+        size_t off[4];
+        unsigned cnt[4];
+        bool in[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) d[q] = cur.desc[min(tb4 + q, t1)];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const TileWin tw = make_window(d[q].x, d[q].y, R);
+          const int k = c - tw.wlo;
+          in[q] = tb4 + q <= t1 && k >= 0 && k < tw.W;
+          off[q] = tile_row_offset(d[q].x, min(tb4 + q, t1), R) + (size_t)(in[q] ? k : 0);
+          cnt[q] = in[q] ? P.tile_hist[off[q]] : 0u;
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          if (in[q]) {
+            P.tile_base[off[q]] = run;
+            run += (int)cnt[q];
+          }
         }
       }
     }
