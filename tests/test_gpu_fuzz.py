@@ -1,6 +1,7 @@
 """Randomised parity: seeded random combinations of workload, size, collision rate, sources, recycling, neutral target,
 smoothing, averaging, window radius, velocity scale and step chunking, CUDA path vs oracle, every element compared.
-BIT1_FUZZ_CASES (default 24) sets how many cases run; BIT1_FUZZ_SEED shifts the sequence."""
+BIT1_FUZZ_CASES (default 24) sets how many cases run; BIT1_FUZZ_SEED shifts the sequence; BIT1_FUZZ_BIG=1 draws 4e5 to
+2.5e6 particles per case instead of 7e2 to 7e4."""
 import os
 
 import numpy as np
@@ -19,7 +20,10 @@ def _case(seed):
     rng = np.random.default_rng(1000003 * SEED0 + seed)
     cfg = int(rng.integers(1, 6))
     full_n = {1: 204800, 2: 1638400, 3: 1e7, 4: 2e8, 5: 1e9}[cfg]
-    n_target = float(rng.choice([700, 3000, 9000, 30000, 70000]))
+    sizes = [700, 3000, 9000, 30000, 70000]
+    if os.environ.get("BIT1_FUZZ_BIG") == "1":       # several tiles per CTA: the stages are reloaded, cooperative grids > 1
+        sizes = [400000, 900000, 2500000]
+    n_target = float(rng.choice(sizes))
     thin = float(rng.choice([1.0, 1.0, 0.25, 0.04]))     # keep this fraction: fewer particles per cell, more cells
     kw = dict(scale=n_target / full_n / thin)
     if cfg >= 3:
