@@ -142,7 +142,9 @@ bit1_status bit1_load_particles(bit1_ctx *ctx, uint64_t n, const double *x, cons
                                 const double *vy, const double *vz, const uint8_t *species,
                                 const uint32_t *pid_or_null, int ptrs_on_device);
 
-/* Enqueue nsteps timesteps on the compute stream; returns without waiting. */
+/* Enqueue nsteps timesteps on the compute stream; returns without waiting.  For nsteps >= 4 (and profiling off) the steps
+ * are replays of a CUDA graph that holds two timesteps, captured on first use and again after any call that changes the
+ * captured launches (load, restart, the bit1_set_* calls); the environment variable BIT1_NO_GRAPH=1 launches directly. */
 bit1_status bit1_step(bit1_ctx *ctx, uint64_t nsteps);
 /* Wait for the compute stream; BIT1_ERR_DEVICE_FLAG if the sticky flag word is non-zero. */
 bit1_status bit1_sync(bit1_ctx *ctx);
