@@ -203,7 +203,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
       if (!(key & 0x80000000u) && lane == __ffs(m) - 1) s_hist[key * kWarps + warp] += (unsigned)__popc(m);
       __syncwarp();
     }
-    fence_proxy_async();
+    if (evm) fence_proxy_async();   // only the slow path writes into the stage (generic proxy) before its reload
     __syncthreads();
     // per window cell: the warps' counts become exclusive prefixes (tile_pre, read back by pass B: this warp's
     // particles for that cell start that far into the tile's run), their sum is the tile's count
@@ -813,7 +813,7 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
         nxt.cell[dst] = tw.wlo + key[r]; nxt.pid[dst] = S->pid[off]; nxt.sp[dst] = (unsigned char)sp[r];
       }
     }
-    fence_proxy_async();
+    if (evm) fence_proxy_async();   // only the slow path writes into the stage (generic proxy) before its reload
     __syncthreads();  // the stage may be overwritten; the tile's deposit is complete
     if (threadIdx.x == 0 && tnext < ntiles)
       issue_tile(P, cur, S, &bar[it & 1], tnext, dn, kRecompute, kRecompute, true, VARIANT == 1);
