@@ -9,6 +9,8 @@
 #include <new>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>   // header-only; ranges show up in Nsight Systems timelines (PAPER.md:105-113 used the same)
+
 #include "../../include/bit1.h"
 #include "aux_kernels.h"
 #include "step_kernels.h"
@@ -162,6 +164,13 @@ uint64_t fnv1a(uint64_t h, const void* data, size_t n) {
   return h;
 }
 
+}  // namespace
+
+namespace {
+struct NvtxRange {   // RAII range around an entry point
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+};
 }  // namespace
 
 struct bit1_ctx {
@@ -518,6 +527,7 @@ bit1_status bit1_get_average(bit1_ctx* c, int64_t* dens_sum, double* phi_sum, ui
 
 bit1_status bit1_load_particles(bit1_ctx* c, uint64_t n, const double* x, const double* vx, const double* vy,
                                 const double* vz, const uint8_t* sp, const uint32_t* pid, int on_device) {
+  NvtxRange nvtx_("bit1_load_particles");
   if (!c || (n && (!x || !vx || !vy || !vz || !sp))) return BIT1_ERR_INVALID_ARG;
   if (n > c->P.capacity) return BIT1_ERR_CAPACITY;
   if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; }
@@ -588,6 +598,7 @@ static bool build_graph(bit1_ctx* c) {
 }
 
 bit1_status bit1_step(bit1_ctx* c, uint64_t nsteps) {
+  NvtxRange nvtx_("bit1_step");
   if (!c) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
   if (c->use_graph && !c->profiling && nsteps >= 4) {
@@ -703,6 +714,7 @@ bit1_status bit1_get_dens(bit1_ctx* c, int64_t* dens) {
 }
 
 bit1_status bit1_get_moments(bit1_ctx* c, bit1_moments* out) {
+  NvtxRange nvtx_("bit1_get_moments");
   if (!c || !out) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
   const Params& P = c->P;
@@ -854,6 +866,7 @@ size_t bit1_checkpoint_size(bit1_ctx* c) {
 }
 
 bit1_status bit1_checkpoint(bit1_ctx* c, void* host, size_t cap, size_t* written) {
+  NvtxRange nvtx_("bit1_checkpoint");
   if (!c || !host) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
   const CkptLayout cl = ckpt_layout(c->P.nc, c->P.ng, c->P.ns, c->P.capacity);
@@ -902,6 +915,7 @@ bit1_status bit1_checkpoint_wait(bit1_ctx* c) {
 }
 
 bit1_status bit1_restart(bit1_ctx* c, const void* blob, size_t bytes) {
+  NvtxRange nvtx_("bit1_restart");
   if (!c || !blob) return BIT1_ERR_INVALID_ARG;
   const CkptLayout cl = ckpt_layout(c->P.nc, c->P.ng, c->P.ns, c->P.capacity);
   if (bytes < cl.bytes) return BIT1_ERR_CHECKPOINT;
