@@ -78,3 +78,4 @@ def test_config4_runs_its_500_steps():
                         kinetic_J=m["kinetic_J"].tolist(), field_J=m["field_J"])
     _save()
     g.close()
+
