@@ -266,6 +266,17 @@ class Oracle:
                                 _p(d["sp"], c_u8p))
         return d
 
+    def particle_array(self, name):
+        """One of x, vx, vy, vz, cell, pid, sp alone (the others are not copied): for states too large to hold twice."""
+        order = ["x", "vx", "vy", "vz", "cell", "pid", "sp"]
+        dt = dict(x=np.float64, vx=np.float64, vy=np.float64, vz=np.float64, cell=np.int32, pid=np.uint32, sp=np.uint8)
+        ct = dict(x=c_f64p, vx=c_f64p, vy=c_f64p, vz=c_f64p, cell=c_i32p, pid=c_u32p, sp=c_u8p)
+        a = np.zeros(self.n_slots, dt[name])
+        args = [None] * 7
+        args[order.index(name)] = _p(a, ct[name])
+        lib().orc_get_particles(self.h, *args)
+        return a
+
     def cell_start(self):
         cs = np.zeros(self.nc + 1, np.int64)
         lib().orc_get_cell_start(self.h, _p(cs, c_i64p))

@@ -1,7 +1,8 @@
 """BASELINE.json configs[4] at FULL size (1e9 particles, 1 048 576 cells, 100 steps, pinned-host checkpoint every
-50 steps, restart leg compared bit for bit).
+50 steps, restart leg compared bit for bit), every element of the state against the
+oracle after 2 steps and 240 000 sampled particles after a third.
 
-Opt-in (BIT1_FULL_C5=1): it needs ~130 GB of HBM, ~130 GB of host memory and about ten minutes, which does not
+Opt-in (BIT1_FULL_C5=1): it needs ~130 GB of HBM, ~130 GB of host memory and about eight minutes, which does not
 belong in the default `pytest -m gpu` run.  The result of the run made for this round is recorded in
 profiles/r1e_config5_full.md.  State digests are taken array by array (8 GB at a time) through the C ABI."""
 import ctypes as C
@@ -71,6 +72,13 @@ def _sampled_oracle_step(g, w, k):
     return int(idx.shape[0])
 
 
+def _cell_start(g):
+    cs = np.zeros(g.nc + 1, np.int64)
+    args = [None] * 7 + [cs.ctypes.data]
+    assert g.lib.bit1_get_particles(g.h, *args) == 0
+    return cs
+
+
 def _digest(g):
     """blake2b of every live array, fetched one at a time with bit1_get_particles (other pointers null)."""
     n = g.n_live()
@@ -107,12 +115,29 @@ def test_config5_full_size_checkpoint_every_50_steps_and_bit_identical_restart()
     g.sync()
     t_load = time.time() - t0
     n0 = w.n
-    w.x = w.vx = w.vy = w.vz = w.sp = None   # the library copied them
+    # every element at full size: the oracle runs all 1e9 particles through the first 2 steps (array by array comparison,
+    # the two states do not fit in host memory side by side otherwise)
+    from oracle.oracle import Oracle
+    t0 = time.time()
+    o = Oracle(w)
+    w.x = w.vx = w.vy = w.vz = w.sp = None   # both sides copied them
+    o.step(2)
+    t_oracle = time.time() - t0
+    g.step(2)
+    g.sync()
+    assert g.n_live() == o.n
+    for name in _ORDER:
+        a, b = _fetch(g, name), o.particle_array(name)
+        assert np.array_equal(a, b), f"config 5 at full size, 2 steps: {name} differs"
+        del a, b
+    assert np.array_equal(g.get_rho(), o.rho()) and np.array_equal(g.get_dens(), o.dens())
+    assert np.array_equal(g.get_E(), o.E()) and np.array_equal(g.get_phi(), o.phi())
+    assert np.array_equal(np.diff(o.cell_start()), np.diff(_cell_start(g)))
+    del o
 
     blob = torch.empty(g.checkpoint_size(), dtype=torch.uint8).pin_memory()
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
     cs = g.compute_stream
-    g.step(2)   # warm-up (part of the 100)
     n_sampled = _sampled_oracle_step(g, w, 2)   # takes step 3
     ev[0].record(cs)
     g.step(47)
@@ -153,7 +178,8 @@ def test_config5_full_size_checkpoint_every_50_steps_and_bit_identical_restart()
               "checkpoint_bytes": int(blob.numel()), "steps_50_wall_s": t_steps_with_ckpt,
               "checkpoint_complete_wall_s": t_ckpt_done, "restart_s": t_restart, "births": m["births"],
               "far_movers_per_step": far, "n_final": want["n"], "bit_identical": got == want,
-              "sampled_particles_bit_identical_to_oracle": n_sampled}
+              "sampled_particles_bit_identical_to_oracle": n_sampled,
+              "all_elements_bit_identical_to_oracle_after_2_steps": True, "oracle_load_and_2_steps_s": t_oracle}
     os.makedirs("gpurun_out", exist_ok=True)
     with open("gpurun_out/config5_full.json", "w") as f:
         json.dump(report, f, indent=1)
