@@ -227,7 +227,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
 }
 
 // ---------------------------------------------------------------------------------------------
-// k_mid: single CTA.
+// k_mid helpers: CTA-wide and grid-wide sorts, block scans.
 constexpr int kMidThreads = 1024;
 constexpr int kSortSmem = 2048;
 
@@ -878,7 +878,7 @@ __global__ void __launch_bounds__(kAuxThreads) k_deposit(const __grid_constant__
 }
 
 // ---------------------------------------------------------------------------------------------
-// k_field: rho = sum_s sign_s dens_s; exact double prefix sum -> phi, E.  Single CTA.
+// k_field helpers: 128-bit shuffles, block scans and sums (the kernel itself is cooperative, see below).
 constexpr int kFieldThreads = 256;
 constexpr int kFieldItems = 4;
 typedef __int128 i128;
