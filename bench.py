@@ -10,6 +10,11 @@ cells, exponential sheath profile, 3 species, config-3 collisions) -- the first 
 host-side generation and load take several minutes (python bench.py --config 5 --steps 10 runs it).
 Inputs are larger than L2 (8.2 GB state vs 126 MB), so no L2 flush is needed between steps.
 
+Legs of one run: (1) W warm-up steps, then K timed steps bracketed by CUDA events on the compute stream (`value`;
+bit1_step replays two-step CUDA graphs); (2) min(K, 50) more steps with CUDA events around every kernel (`roofline`);
+(3) end to end: bit1_load_particles from pinned host arrays + K steps + bit1_get_rho to the host, wall clock (`e2e`);
+(4) at N = 1, the CPU oracle on a bounded cut-down of the same workload (`cpu_baseline`).
+
 The path does not shard (BASELINE.json north_star: no multi-GPU sharding or collectives): --gpus N runs N
 independent replicas, one process per GPU, and reports the aggregate ("replicas only").
 """
