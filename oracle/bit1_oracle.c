@@ -18,7 +18,7 @@
  * PAPER.md:95 (Table 3: walls absorb plasma and take its charge),
  * PAPER.md:111/121 (mover move0/moveb followed by arranger arrj/narrj).  It
  * prints no equation.  Every numerical rule is therefore the reading recorded
- * in SURVEY.md section 8(c) and DESIGN.md "Readings" (R1..R27), which follow
+ * in SURVEY.md section 8(c) and DESIGN.md "Readings" (A1..A27 and the R-/N- readings added while building), which follow
  * BASELINE.json's north_star and textbook PIC-MCC (Birdsall-Langdon leapfrog
  * and Boris rotation; Vahedi-Surendra null collision; Salmon et al. Philox).
  * Each function cites the reading it implements.
@@ -32,7 +32,8 @@
  * wall recycling and neutral particles as the collision target (NEXT-2, readings N2-a/b), and reading R-thr
  * (ionisation cross-section zero at or below the threshold).
  *
- * Pins: see tests/test_oracle_*.py (NEXT-1: test_oracle_next1.py, NEXT-2: test_oracle_next2.py).  No function here
+ * Pins: see tests/test_oracle_*.py (moments and density: test_oracle_moments.py; NEXT-1: test_oracle_next1.py;
+ * NEXT-2: test_oracle_next2.py).  No function here
  * is "parity unpinned".
  */
 #include <math.h>

@@ -26,18 +26,23 @@ def test_philox_matches_independent_python_on_random_counters():
 
 
 def test_uniforms_are_exact_rationals():
+    """DESIGN.md reading R-U: the two-word uniform is (((a<<32|b)>>12) + 1/2) / 2^52, exactly (53 significant bits at
+    most), not SURVEY's (>>11, 2^-53) form, whose top value rounds to 1.0."""
     rng = np.random.default_rng(2)
-    cases = [(0, 0), (2**32 - 1, 2**32 - 1), (1, 0), (0, 4095), (0, 4096)]
-    cases += [tuple(int(v) for v in rng.integers(0, 2**32, 2, dtype=np.uint64)) for _ in range(100)]
+    cases = [(0, 0), (2**32 - 1, 2**32 - 1), (1, 0), (0, 4095), (0, 4096), (0, 2048), (0, 6144), (2**31, 0)]
+    cases += [tuple(int(v) for v in rng.integers(0, 2**32, 2, dtype=np.uint64)) for _ in range(200)]
+    differs_from_survey_form = 0
     for a, b in cases:
-        w = ((a << 32) | b) >> 11
-        exact = (Fraction(w) + Fraction(1, 2)) / Fraction(2**53)
         got = O.u53(a, b)
         assert 0.0 < got < 1.0
-        # (w + 0.5) needs 54 bits when w >= 2^52: one rounding, so <= 1 ulp(2^-53 * 2^53)=2^-53 relative
-        assert abs(Fraction(got) - exact) <= Fraction(1, 2**53)
+        w12 = ((a << 32) | b) >> 12
+        assert Fraction(got) == (Fraction(w12) + Fraction(1, 2)) / Fraction(2**52), (a, b)
+        survey = (Fraction(((a << 32) | b) >> 11) + Fraction(1, 2)) / Fraction(2**53)
+        differs_from_survey_form += Fraction(got) != survey
         exact32 = (Fraction(a) + Fraction(1, 2)) / Fraction(2**32)
         assert Fraction(O.u32(a)) == exact32  # 33 significant bits: exact
+    assert differs_from_survey_form > 100          # the two readings are told apart by this test
+    assert O.u53(0, 0) == 2.0**-53 and O.u53(2**32 - 1, 2**32 - 1) == 1.0 - 2.0**-53
     assert O.u32(0) == 2.0**-33 and O.u32(2**32 - 1) == 1.0 - 2.0**-33
 
 
