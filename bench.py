@@ -202,7 +202,7 @@ def run_cuda(args):
 
     w, wname = _workload(args, rank)
     n0 = w.n
-    sim = Bit1(w, device=f"cuda:{local}", variant=args.variant)
+    sim = Bit1(w, device=f"cuda:{local}")
     # pinned host copies of the inputs for the end-to-end leg
     pin = {}
     for k in ("x", "vx", "vy", "vz", "sp"):
@@ -274,11 +274,10 @@ def run_cuda(args):
         return
     peak, peak_src = _peaks()
     n_mean = n_prof   # particles per launch in the per-kernel leg
-    variant = 1 if args.variant == 1 else 2
-    # dominant kernel: the arranger (pass B).  Algorithmic bytes per particle: V2 reads the 41 B
-    # state minus the 4 B cell index (recomputed from x) in both passes and writes 41 B in pass B: 37 + 78 = 115 B;
-    # V1 writes x, v, cell in place in pass A (37 + 36) and reads everything in pass B (41 + 41).
-    a_bpp, b_bpp = (37, 78) if variant == 2 else (73, 82)
+    # dominant kernel: the arranger (pass B).  Algorithmic bytes per particle: both passes read
+    # x, v, pid, species (37 B; the cell index is cell_of(x) and is neither stored nor fetched), pass B writes the
+    # same 37 B to the sorted position: 37 + 74 = 111 B per particle-step
+    a_bpp, b_bpp = 37, 74
     b_bytes = b_bpp * n_mean
     b_ms = prof["pass_b"] / max(psteps, 1)
     a_bytes = a_bpp * n_mean
@@ -290,7 +289,7 @@ def run_cuda(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": wname, "particles": n0, "cells": w.nc, "species": len(w.species),
-                   "variant": f"V{variant}", "launch": "two-step CUDA graphs replayed on the compute stream", "parallelism": "replicas only" if world > 1 else "1 GPU",
+                   "launch": "two-step CUDA graphs replayed on the compute stream", "parallelism": "replicas only" if world > 1 else "1 GPU",
                    "l2": "inputs larger than L2 (no flush)" if n0 * STATE_BYTES > 126e6 else
                    "state fits L2: launch-latency bound, no HBM roofline claimed"},
         "e2e": {"value": e2e_units / (e2e_ms_max * 1e-3), "unit": "particle-steps/s",
@@ -298,7 +297,7 @@ def run_cuda(args):
                 "what": "bit1_load_particles(host arrays) + bit1_step(K) + bit1_get_rho(host), wall clock"},
         "gpu_launches": int(launches),
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": f"k_pass_b<{variant}> (arranger: stable scatter + fused deposit)",
+        "roofline": {"bound": "hbm", "kernel": "k_pass_b (arranger: recompute push, stable scatter, fused deposit)",
                      "achieved": b_bytes / (b_ms * 1e-3) / 1e9 if b_ms > 0 else None, "peak": peak, "unit": "GB/s",
                      "frac": (b_bytes / (b_ms * 1e-3) / 1e9 / peak) if b_ms > 0 else None,
                      "traffic": _traffic("k_pass_b", args), "peak_source": peak_src,
@@ -329,7 +328,6 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--scale", type=float, default=1.0)
-    ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()

@@ -22,8 +22,11 @@
  *    bit1_workspace_size() bytes, 256-byte aligned, alive until bit1_destroy.  All input arrays and
  *    tables are copied at the call; the caller keeps them.  Streams are borrowed cudaStream_t handles.
  *  - Errors: every call returns a bit1_status; nothing throws or aborts; out-parameters are untouched
- *    on error.  Device-side faults (capacity exceeded, particle escaped the domain, overflow list full)
- *    set a sticky flag word that bit1_sync and the getters report as BIT1_ERR_DEVICE_FLAG.
+ *    on error.  Device-side faults (capacity exceeded, particle escaped the domain) set a sticky flag
+ *    word that bit1_sync reports as BIT1_ERR_DEVICE_FLAG (details in bit1_moments.flags).
+ *  - Every input the oracle's algorithm accepts is accepted here: a step whose far movers and births do
+ *    not fit the arranger's side list is redone by a general path (full radix sort of the store) at the
+ *    next call that waits for the device; results are the same bits either way.
  *  - Threading: one context, one caller thread.
  *  - There is no CPU fallback: without a CUDA device bit1_create returns BIT1_ERR_CUDA.
  */
@@ -55,7 +58,7 @@ typedef enum {
 /* sticky device flag bits (bit1_moments.flags) */
 #define BIT1_FLAG_CAPACITY 1u  /* births beyond capacity were dropped (SURVEY 8(c) "A") */
 #define BIT1_FLAG_ESCAPE 2u    /* a particle crossed more than one domain length (reading A21) */
-#define BIT1_FLAG_OVERFLOW 4u  /* far-mover/birth list full: results after this step are invalid */
+#define BIT1_FLAG_PID_WRAP 8u  /* the 32-bit particle-id counter wrapped: newborn particles share random streams with old ones */
 
 /* species process flags */
 #define BIT1_ELASTIC 1u             /* e-D elastic, isotropic (reading A14) */
@@ -103,8 +106,14 @@ typedef struct {
   size_t workspace_bytes;
   void *compute_stream;    /* cudaStream_t, borrowed; NULL = default stream */
   void *side_stream;       /* cudaStream_t for checkpoint device->host copies; NULL = compute stream */
-  int32_t checkpoint_staging; /* 1: reserve a device snapshot area so bit1_checkpoint overlaps later steps */
-  int32_t variant;         /* 0 default; 1 = in-place push then scatter ("V1"); 2 = recompute in the scatter pass ("V2") */
+  int32_t checkpoint_staging; /* 1: reserve a device snapshot area so that every later step overlaps bit1_checkpoint's copy */
+  int32_t launch_mode;     /* 0 default: bit1_step(n >= 4) replays CUDA graphs of two timesteps; 1: direct launches */
+  /* Arranger internals (readings R-win, R-side); 0 = default everywhere.  None of them changes a result. */
+  int32_t window_radius_max;   /* upper bound, in cells, of the adaptive sort-window radius (default 16, at most 60);
+                                  the workspace holds 2*radius_max + 4 row entries per 1024-particle tile */
+  int32_t window_radius_fixed; /* k >= 1 pins the radius to k - 1 cells instead of adapting it every step */
+  uint64_t side_list_capacity; /* far movers + births one step may route through the sorted side list (default
+                                  max(65536, capacity/16)); a step with more takes the general path (slower, same bits) */
 } bit1_options;
 
 typedef struct {
@@ -123,11 +132,15 @@ typedef struct {
   uint64_t events[BIT1_MAX_SPECIES][3]; /* elastic, ionise, cx */
   uint64_t far_movers, max_far_movers_per_step; /* entries that took the sorted side list */
   uint64_t recycled;                  /* wall-recycling events (NEXT-2) */
+  uint64_t general_steps;             /* steps that took the general path (side list beyond its capacity) */
+  uint32_t window_radius;             /* sort-window radius, in cells, that the next step will use */
+  uint32_t _pad;
   double *density[BIT1_MAX_SPECIES];  /* HOST, optional (NULL to skip), ng entries each, m^-3 */
 } bit1_moments;
 
-/* Bytes of device workspace for this configuration (staging: see bit1_options.checkpoint_staging). */
-size_t bit1_workspace_size(const bit1_grid *grid, int nspecies, uint64_t capacity, int checkpoint_staging);
+/* Bytes of device workspace for this configuration.  Reads capacity, checkpoint_staging, window_radius_max,
+ * window_radius_fixed and side_list_capacity of `opt` (the pointers in it are ignored); 0 for invalid arguments. */
+size_t bit1_workspace_size(const bit1_grid *grid, int nspecies, const bit1_options *opt);
 
 /* Create a context.  grid/species/opt are HOST structs, copied.  BIT1_ERR_RANGE if any Q_s is out of
  * range; BIT1_ERR_INVALID_ARG for nc < 2, non-positive dx/dt/m/weight, bad species indices, IONISE set
@@ -144,7 +157,7 @@ bit1_status bit1_load_particles(bit1_ctx *ctx, uint64_t n, const double *x, cons
 
 /* Enqueue nsteps timesteps on the compute stream; returns without waiting.  For nsteps >= 4 (and profiling off) the steps
  * are replays of a CUDA graph that holds two timesteps, captured on first use and again after any call that changes the
- * captured launches (load, restart, the bit1_set_* calls); the environment variable BIT1_NO_GRAPH=1 launches directly. */
+ * captured launches (load, restart, the bit1_set_* calls); bit1_options.launch_mode = 1 launches directly. */
 bit1_status bit1_step(bit1_ctx *ctx, uint64_t nsteps);
 /* Wait for the compute stream; BIT1_ERR_DEVICE_FLAG if the sticky flag word is non-zero. */
 bit1_status bit1_sync(bit1_ctx *ctx);
@@ -197,17 +210,20 @@ bit1_status bit1_get_rho_smoothed(bit1_ctx *ctx, int64_t *rho_s_fixed);
 bit1_status bit1_set_averaging(bit1_ctx *ctx, int window, int interval);
 bit1_status bit1_get_average(bit1_ctx *ctx, int64_t *dens_sum, double *phi_sum, uint64_t *count, uint64_t *step);
 
-/* Test hook: overwrite E (HOST, nc+1 entries) and optionally freeze the field solve (E stays as set
- * while rho keeps being deposited) -- used by closed-form push tests. */
+/* Prescribed field: overwrite E (HOST, nc+1 entries) and optionally freeze the field solve (E stays as set while rho
+ * keeps being deposited): test-particle runs in a given field; the closed-form push tests use it too. */
 bit1_status bit1_set_E(bit1_ctx *ctx, const double *E, int freeze_field);
-/* Test hook: set the step counter (Philox counter words 1-2). */
+/* Set the step counter (Philox counter words 1-2), e.g. to continue a run that was loaded from exported records. */
 bit1_status bit1_set_step(bit1_ctx *ctx, uint64_t step);
 
-/* Checkpoint: header + counts per cell + the SoA particle records, snapshotted on the
- * compute stream and copied to PINNED HOST memory on the side stream; later bit1_step calls overlap the
- * copy when the context was created with checkpoint_staging = 1.  The blob is valid after
- * bit1_checkpoint_wait.  bit1_restart needs a context created with the identical configuration and
- * reproduces the run bit-identically (BASELINE.json north_star). */
+/* Checkpoint: header + device state + the SoA records of the LIVE particles (x, v, id, species; the
+ * cell index and the counts per cell are functions of x and are rebuilt at restart), copied to PINNED HOST memory on
+ * the side stream behind an event.  bit1_checkpoint waits for the steps enqueued so far (the live count sizes the blob)
+ * and returns with the copy in flight: with checkpoint_staging = 1 the state is first snapshotted on the device and
+ * every later step overlaps the copy; without it the copy reads the store directly, the next step overlaps it and the
+ * one after waits.  *written <= bit1_checkpoint_size() (the size at full capacity).  The blob is valid after
+ * bit1_checkpoint_wait.  bit1_restart needs a context created with the identical configuration, validates the blob
+ * (BIT1_ERR_CHECKPOINT) and reproduces the run bit-identically (BASELINE.json north_star). */
 size_t bit1_checkpoint_size(bit1_ctx *ctx);
 bit1_status bit1_checkpoint(bit1_ctx *ctx, void *pinned_host, size_t cap, size_t *written);
 bit1_status bit1_checkpoint_wait(bit1_ctx *ctx);

@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libbit1.so")
 
 OK, ERR_INVALID_ARG, ERR_RANGE, ERR_CAPACITY, ERR_STATE, ERR_CUDA, ERR_CHECKPOINT, ERR_DEVICE_FLAG = range(8)
-FLAG_CAPACITY, FLAG_ESCAPE, FLAG_OVERFLOW = 1, 2, 4
+FLAG_CAPACITY, FLAG_ESCAPE, FLAG_PID_WRAP = 1, 2, 8
 
 c_f64p = C.POINTER(C.c_double)
 
@@ -39,7 +39,8 @@ class bit1_options(C.Structure):
                 ("sig_el", c_f64p), ("sig_ion", c_f64p), ("sig_cx", c_f64p), ("n_sig", C.c_int32),
                 ("n_norm", C.c_int32), ("dE_eV", C.c_double), ("inv_norm", c_f64p), ("workspace", C.c_void_p),
                 ("workspace_bytes", C.c_size_t), ("compute_stream", C.c_void_p), ("side_stream", C.c_void_p),
-                ("checkpoint_staging", C.c_int32), ("variant", C.c_int32)]
+                ("checkpoint_staging", C.c_int32), ("launch_mode", C.c_int32), ("window_radius_max", C.c_int32),
+                ("window_radius_fixed", C.c_int32), ("side_list_capacity", C.c_uint64)]
 
 
 class bit1_moments(C.Structure):
@@ -50,7 +51,8 @@ class bit1_moments(C.Structure):
                 ("nu_overflow", C.c_uint64), ("dir_fallback", C.c_uint64), ("escape", C.c_uint64),
                 ("births", C.c_uint64), ("reinject", C.c_uint64), ("candidates", C.c_uint64 * MAX_SPECIES),
                 ("events", (C.c_uint64 * 3) * MAX_SPECIES), ("far_movers", C.c_uint64),
-                ("max_far_movers_per_step", C.c_uint64), ("recycled", C.c_uint64), ("density", c_f64p * MAX_SPECIES)]
+                ("max_far_movers_per_step", C.c_uint64), ("recycled", C.c_uint64), ("general_steps", C.c_uint64),
+                ("window_radius", C.c_uint32), ("_pad", C.c_uint32), ("density", c_f64p * MAX_SPECIES)]
 
 
 _lib = None
@@ -68,7 +70,7 @@ def load_library(path: Optional[str] = None):
     L = C.CDLL(p)
     vp = C.c_void_p
     L.bit1_workspace_size.restype = C.c_size_t
-    L.bit1_workspace_size.argtypes = [C.POINTER(bit1_grid), C.c_int, C.c_uint64, C.c_int]
+    L.bit1_workspace_size.argtypes = [C.POINTER(bit1_grid), C.c_int, C.POINTER(bit1_options)]
     L.bit1_create.restype = C.c_int
     L.bit1_create.argtypes = [C.POINTER(bit1_grid), C.POINTER(bit1_species), C.c_int, C.c_double,
                               C.POINTER(bit1_options), C.POINTER(vp)]
@@ -158,8 +160,10 @@ def _ptr(a):
 class Bit1:
     """One libbit1 context.  Methods mirror the C entry points one to one."""
 
-    def __init__(self, w, *, checkpoint_staging: bool = False, variant: int = 0, device: str = "cuda:0",
-                 side_stream: bool = True):
+    def __init__(self, w, *, checkpoint_staging: bool = False, device: str = "cuda:0", side_stream: bool = True,
+                 direct_launch: bool = False, window_radius_max: int = 0, window_radius: Optional[int] = None,
+                 side_list_capacity: int = 0):
+        """window_radius: None = adaptive (default), k = pinned to k cells; the other keywords are bit1_options fields."""
         import torch
 
         if not torch.cuda.is_available():
@@ -177,7 +181,14 @@ class Bit1:
         for k, s in enumerate(w.species):
             sp[k] = bit1_species(s.q, s.m, s.weight, s.flags, s.src_mode, s.src_partner, 0, s.src_vth, s.pnull,
                                  s.numax)
-        nbytes = self.lib.bit1_workspace_size(C.byref(g), self.ns, int(w.capacity), int(checkpoint_staging))
+        o = bit1_options()
+        o.seed, o.capacity = int(w.seed), int(w.capacity)
+        o.checkpoint_staging = int(checkpoint_staging)
+        o.launch_mode = int(direct_launch)
+        o.window_radius_max = int(window_radius_max)
+        o.window_radius_fixed = 0 if window_radius is None else int(window_radius) + 1
+        o.side_list_capacity = int(side_list_capacity)
+        nbytes = self.lib.bit1_workspace_size(C.byref(g), self.ns, C.byref(o))
         if nbytes == 0:
             raise Bit1Error(ERR_INVALID_ARG, "bit1_workspace_size")
         self.workspace_bytes = nbytes
@@ -186,8 +197,6 @@ class Bit1:
         self.compute_stream = torch.cuda.Stream(device=self.device)
         self.side_stream = torch.cuda.Stream(device=self.device) if side_stream else None
         self._keep = [_f8(w.sig_el), _f8(w.sig_ion), _f8(w.sig_cx), _f8(w.inv_norm)]
-        o = bit1_options()
-        o.seed, o.capacity = int(w.seed), int(w.capacity)
         o.src_lo, o.src_hi = w.src_lo, w.src_hi
         o.n0, o.vth_n, o.E_ion, o.m_n = w.n0, w.vth_n, w.E_ion, w.m_n
         o.sig_el = self._keep[0].ctypes.data_as(c_f64p)
@@ -200,8 +209,6 @@ class Bit1:
         o.workspace, o.workspace_bytes = base, nbytes
         o.compute_stream = self.compute_stream.cuda_stream
         o.side_stream = self.side_stream.cuda_stream if self.side_stream is not None else None
-        o.checkpoint_staging = int(checkpoint_staging)
-        o.variant = int(variant)
         h = C.c_void_p()
         _check(self.lib.bit1_create(C.byref(g), sp, self.ns, w.dt, C.byref(o), C.byref(h)), "bit1_create")
         self.h = h
@@ -303,7 +310,7 @@ class Bit1:
                    reinject=int(m.reinject), candidates=np.array(m.candidates[:ns], np.uint64),
                    events=np.array([list(m.events[k][:]) for k in range(ns)], np.uint64),
                    far_movers=int(m.far_movers), max_far_movers_per_step=int(m.max_far_movers_per_step),
-                   recycled=int(m.recycled))
+                   recycled=int(m.recycled), general_steps=int(m.general_steps), window_radius=int(m.window_radius))
         if density:
             out["density"] = dens
         return out

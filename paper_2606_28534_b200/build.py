@@ -12,7 +12,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libbit1.so")
-SOURCES = ["api.cu", "step_kernels.cu", "aux_kernels.cu"]
+SOURCES = ["api.cu", "step_kernels.cu", "general_kernels.cu", "aux_kernels.cu"]
 HEADERS = ["common.cuh", "device_math.cuh", "advance.cuh", "pipeline.cuh", "step_kernels.h", "aux_kernels.h",
            os.path.join("..", "..", "include", "bit1.h")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-fmad=false", "-lineinfo",

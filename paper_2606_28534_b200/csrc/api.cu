@@ -24,15 +24,32 @@ constexpr double kEps0 = 8.8541878128e-12;     // F/m
 constexpr double kTwoM40 = 9.094947017729282379150390625e-13;
 constexpr int kMaxSig = 16384;
 constexpr int kMaxNorm = 1 << 20;
-constexpr int kMaxR = 4;
+constexpr int kDefaultRmax = 16;
 constexpr size_t kAlign = 256;
-constexpr uint32_t kCkptVersion = 3;   // 2: + averaging sums (NEXT-1); 3: + recycling counter (NEXT-2)
+// 2: + averaging sums (NEXT-1); 3: + recycling counter (NEXT-2); 4: live prefix only, no cell array, no cell_start
+constexpr uint32_t kCkptVersion = 4;
 
-// sort window radius in cells (reading R-win); BIT1_WINDOW_R overrides it for the tests
-inline int window_R() {
-  int R = 1;
-  if (const char* ev = getenv("BIT1_WINDOW_R")) { const int r = atoi(ev); if (r >= 0 && r <= kMaxR) R = r; }
-  return R;
+// settings of bit1_options that shape the workspace
+struct Shape {
+  size_t cap;        // particle capacity
+  int staging;       // device snapshot area for overlapped checkpoints
+  int r_max;         // upper bound of the adaptive sort-window radius
+  size_t ovf_cap;    // side-list capacity
+};
+inline bool shape_of(const bit1_options* o, Shape* sh) {
+  if (!o || o->capacity == 0 || o->capacity >= (1ull << 31)) return false;
+  sh->cap = (size_t)o->capacity;
+  sh->staging = o->checkpoint_staging ? 1 : 0;
+  sh->r_max = o->window_radius_max == 0 ? kDefaultRmax : o->window_radius_max;
+  if (sh->r_max < 1 || sh->r_max > kMaxR) return false;
+  if (o->window_radius_fixed < 0 || o->window_radius_fixed > kMaxR + 1) return false;
+  if (o->window_radius_fixed > 0 && o->window_radius_fixed - 1 > sh->r_max) sh->r_max = o->window_radius_fixed - 1;
+  if (sh->r_max < 1) sh->r_max = 1;
+  size_t oc = o->side_list_capacity;
+  if (oc == 0) { oc = sh->cap / 16; if (oc < 65536) oc = 65536; }
+  if (oc < 16 || oc >= (1ull << 31)) return false;
+  sh->ovf_cap = oc;
+  return true;
 }
 
 inline size_t align_up(size_t v) { return (v + kAlign - 1) & ~(kAlign - 1); }
@@ -75,37 +92,42 @@ Particles part_at(void* base, const PartLayout& l) {
 // acc_dens[ns*ng] | avg_dens[ns*ng] (int64) | acc_phi[nc+1] | avg_phi[nc+1] (fp64)
 size_t avg_bytes(int nc, int ng, int ns) { return 2 * ((size_t)ns * ng + (size_t)(nc + 1)) * 8; }
 
+// Checkpoint blob: header | DevState | averaging sums | x | vx | vy | vz | pid |
+// species, each array holding the n live particles only (256-byte aligned).  The cell index and the counts per cell
+// are functions of x and are rebuilt at restart.
 struct CkptLayout {
-  size_t header, state, cell_start, avg, part, bytes;
+  size_t header, state, avg, x, vx, vy, vz, pid, sp, bytes;
 };
-CkptLayout ckpt_layout(int nc, int ng, int ns, size_t cap) {
+CkptLayout ckpt_layout(int nc, int ng, int ns, size_t n) {
   CkptLayout c;
   c.header = 0;
   c.state = 256;
-  c.cell_start = c.state + align_up(sizeof(DevState));
-  c.avg = c.cell_start + align_up((size_t)(nc + 1) * 4);
-  c.part = c.avg + align_up(avg_bytes(nc, ng, ns));
-  c.bytes = c.part + part_layout(cap).bytes;
+  c.avg = c.state + align_up(sizeof(DevState));
+  size_t o = c.avg + align_up(avg_bytes(nc, ng, ns));
+  c.x = o; o += align_up(n * 8);
+  c.vx = o; o += align_up(n * 8);
+  c.vy = o; o += align_up(n * 8);
+  c.vz = o; o += align_up(n * 8);
+  c.pid = o; o += align_up(n * 4);
+  c.sp = o; o += align_up(n);
+  c.bytes = o;
   return c;
 }
 
 struct Layout {
-  size_t st, tables, dens, dens_old, rho, rho_s, rho_t, avg, phi, E, cell_count, cell_start, cell_start_old, scan_part, coop_scratch, cell_base, ovf_before, tile_hist, tile_base, tile_pre, evt,
-      ovf_key, ovf_idx, ovf_dst, tmp_key, tmp_idx, ovf_rec, part[2], scratch, mom, total;
-  unsigned ovf_cap, ovf_pow2;
+  size_t st, tables, dens, dens_old, rho, rho_s, rho_t, avg, phi, E, cell_count, cell_start, cell_start_old, scan_part, coop_scratch, cell_base, ovf_before, ovf_lb, ovf_ub, radix_hist, tile_hist, tile_base, tile_pre, evt,
+      ovf_key, ovf_idx, ovf_dst, tmp_key, tmp_idx, tmp2_key, tmp2_idx, ovf_rec, part[2], scratch, small, mom, total;
+  unsigned ovf_cap;
   int max_tiles, ng;
   size_t scratch_bytes;
 };
-Layout make_layout(int nc, int bc, int ns, size_t cap, int staging) {
+Layout make_layout(int nc, int bc, int ns, const Shape& sh) {
   Layout l;
+  const size_t cap = sh.cap;
   l.ng = bc ? nc + 1 : nc;
   l.max_tiles = (int)((cap + kTile - 1) / kTile);
-  size_t oc = cap / 16;
-  if (oc < 65536) oc = 65536;
-  l.ovf_cap = (unsigned)oc;
-  unsigned p2 = 1;
-  while (p2 < l.ovf_cap) p2 <<= 1;
-  l.ovf_pow2 = p2;
+  l.ovf_cap = (unsigned)sh.ovf_cap;
+  const size_t oc = l.ovf_cap;
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t at = o; o += align_up(bytes); return at; };
   l.st = take(sizeof(DevState));
@@ -125,27 +147,35 @@ Layout make_layout(int nc, int bc, int ns, size_t cap, int staging) {
   l.coop_scratch = take(4 * 1024 * 16);
   l.cell_base = take((size_t)nc * 4);
   l.ovf_before = take((size_t)nc * 4);
-  const size_t rw = tile_row_words(nc, l.max_tiles, window_R());
+  l.ovf_lb = take((size_t)nc * 4);
+  l.ovf_ub = take((size_t)nc * 4);
+  l.radix_hist = take((size_t)256 * 256 * 4);
+  const size_t rw = tile_row_words(nc, l.max_tiles, sh.r_max);
   l.tile_hist = take(rw * 4);
   l.tile_base = take(rw * 4);
   l.tile_pre = take(rw * 4 * kWarps);
   l.evt = take((size_t)(l.max_tiles + 1) * (kTile / 8));
-  l.ovf_key = take((size_t)p2 * 8);
-  l.tmp_key = take((size_t)p2 * 8);
-  l.ovf_idx = take((size_t)p2 * 4);
-  l.ovf_dst = take((size_t)p2 * 4);
-  l.tmp_idx = take((size_t)p2 * 4);
-  l.ovf_rec = take((size_t)l.ovf_cap * sizeof(OvfRec));
+  l.ovf_key = take(oc * 8);
+  l.tmp_key = take(oc * 8);
+  l.tmp2_key = take(oc * 8);
+  l.ovf_idx = take(oc * 4);
+  l.ovf_dst = take(oc * 4);
+  l.tmp_idx = take(oc * 4);
+  l.tmp2_idx = take(oc * 4);
+  l.ovf_rec = take(oc * sizeof(OvfRec));
   const PartLayout pl = part_layout(cap);
   l.part[0] = take(pl.bytes);
   l.part[1] = take(pl.bytes);
-  l.scratch_bytes = load_scratch_bytes((unsigned)cap);
+  // one scratch area for the calls that never overlap one another: load-time sort, general-path step, export, and
+  // the device snapshot of an overlapped checkpoint (a general-path step first waits for a pending checkpoint)
+  l.scratch_bytes = general_scratch_bytes((unsigned)cap);
   if (export_scratch_bytes(nc, (unsigned)cap) > l.scratch_bytes) l.scratch_bytes = export_scratch_bytes(nc, (unsigned)cap);
-  if (staging) {
+  if (sh.staging) {
     const size_t cb = ckpt_layout(nc, l.ng, ns, cap).bytes;
     if (cb > l.scratch_bytes) l.scratch_bytes = cb;
   }
   l.scratch = take(l.scratch_bytes);
+  l.small = take(ckpt_layout(nc, l.ng, ns, 0).bytes);   // DevState + averaging sums of a checkpoint without staging
   l.mom = take(moments_scratch_bytes());
   l.total = o;
   return l;
@@ -155,7 +185,7 @@ struct CkptHeader {
   char magic[8];
   uint32_t version;
   int32_t nc, ns, bc;
-  uint64_t capacity, cfg_hash, bytes;
+  uint64_t capacity, cfg_hash, bytes, n;
 };
 
 uint64_t fnv1a(uint64_t h, const void* data, size_t n) {
@@ -176,13 +206,14 @@ struct NvtxRange {   // RAII range around an entry point
 struct bit1_ctx {
   Params P;
   Layout lay;
+  Shape shape;
   Particles buf[2];
   int cur;
   char* ws;
   cudaStream_t cs, ss;
   cudaEvent_t ev_snap, ev_done, ev_load0, ev_load1;
   bool ckpt_pending, staging, loaded;
-  int variant;
+  bool ckpt_reads_live;   // a checkpoint without staging is still copying out of the live half of the store
   uint64_t launches, cfg_hash, cfg_hash_base;
   double m[BIT1_MAX_SPECIES], weight[BIT1_MAX_SPECIES];
   double dt;
@@ -193,6 +224,13 @@ struct bit1_ctx {
   bool use_graph;
   std::vector<cudaEvent_t> prof_ev;  // 5 per timed step
   size_t prof_steps;
+  // Steps are enqueued without looking at the device.  step_target is the value the device's step counter has
+  // when everything enqueued has really run; a step whose side list did not fit stalls on the device (it and the
+  // steps behind it return at once) and settle() takes it through the general path at the next call that waits.
+  uint64_t step_target;
+  uint64_t last_general_step;   // step index the general path last took
+  unsigned burst;               // steps to take by the general path outright after the next stall
+  uint64_t general_steps_host;
 };
 constexpr size_t kMaxProfSteps = 4096;
 
@@ -200,6 +238,11 @@ constexpr size_t kMaxProfSteps = 4096;
   do {                                             \
     cudaError_t e_ = (call);                       \
     if (e_ != cudaSuccess) return BIT1_ERR_CUDA;   \
+  } while (0)
+#define BIT1_OK_OR_RETURN(call)                    \
+  do {                                             \
+    bit1_status s_ = (call);                       \
+    if (s_ != BIT1_OK) return s_;                  \
   } while (0)
 
 // configuration hash: recomputed from the base hash and the NEXT-2 settings, so the order of the calls is irrelevant
@@ -211,6 +254,12 @@ static void rehash(bit1_ctx* c) {
   }
   h = fnv1a(h, &c->P.target_species, 4);
   c->cfg_hash = h;
+}
+
+static int bits_for(unsigned long long v) {   // bits needed to write values 0 .. v
+  int b = 1;
+  while (b < 63 && (v >> b) != 0ull) ++b;
+  return b;
 }
 
 extern "C" {
@@ -229,9 +278,10 @@ const char* bit1_error_string(bit1_status s) {
   return "unknown";
 }
 
-size_t bit1_workspace_size(const bit1_grid* g, int ns, uint64_t capacity, int staging) {
-  if (!g || g->nc < 2 || ns < 1 || ns > BIT1_MAX_SPECIES || capacity == 0 || capacity >= (1ull << 31)) return 0;
-  return make_layout(g->nc, g->bc, ns, (size_t)capacity, staging).total;
+size_t bit1_workspace_size(const bit1_grid* g, int ns, const bit1_options* o) {
+  Shape sh;
+  if (!g || g->nc < 2 || g->nc >= (1 << 28) || ns < 1 || ns > BIT1_MAX_SPECIES || !shape_of(o, &sh)) return 0;
+  return make_layout(g->nc, g->bc, ns, sh).total;
 }
 
 bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, double dt, const bit1_options* o,
@@ -240,17 +290,20 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   if (g->nc < 2 || g->nc >= (1 << 28) || (g->bc != 0 && g->bc != 1) || !(g->dx > 0.0) || !(g->area > 0.0) ||
       !(dt > 0.0) || ns < 1 || ns > BIT1_MAX_SPECIES)
     return BIT1_ERR_INVALID_ARG;
-  if (o->capacity == 0 || o->capacity >= (1ull << 31)) return BIT1_ERR_INVALID_ARG;
+  Shape sh;
+  if (!shape_of(o, &sh)) return BIT1_ERR_INVALID_ARG;
+  if (o->launch_mode != 0 && o->launch_mode != 1) return BIT1_ERR_INVALID_ARG;
   if (o->n_sig < 0 || o->n_sig > kMaxSig || o->n_norm < 1 || o->n_norm > kMaxNorm || !o->inv_norm)
     return BIT1_ERR_INVALID_ARG;
   if (!o->workspace || (reinterpret_cast<uintptr_t>(o->workspace) & (kAlign - 1))) return BIT1_ERR_INVALID_ARG;
   int sp_ep = -1, sp_ip = -1;
-  bool any_coll = false, any_ion = false;
+  bool any_coll = false, any_ion = false, any_src = false;
   for (int s = 0; s < ns; ++s) {
     if (!(sp[s].m > 0.0) || !(sp[s].weight > 0.0)) return BIT1_ERR_INVALID_ARG;
     if (sp[s].src_mode < 0 || sp[s].src_mode > 2) return BIT1_ERR_INVALID_ARG;
     if (sp[s].src_mode == BIT1_SRC_PAIR && (sp[s].src_partner < 0 || sp[s].src_partner >= ns))
       return BIT1_ERR_INVALID_ARG;
+    if (sp[s].src_mode != BIT1_SRC_NONE) any_src = true;
     if ((sp[s].flags & BIT1_ELECTRON_PRODUCT) && sp_ep < 0) sp_ep = s;
     if ((sp[s].flags & BIT1_ION_PRODUCT) && sp_ip < 0) sp_ip = s;
     if (sp[s].flags & (BIT1_ELASTIC | BIT1_IONISE | BIT1_CX)) any_coll = true;
@@ -259,36 +312,43 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   if (any_coll && (o->n_sig < 2 || !o->sig_el || !o->sig_ion || !o->sig_cx || !(o->dE_eV > 0.0) || !(o->m_n > 0.0)))
     return BIT1_ERR_INVALID_ARG;
   if (any_ion && (sp_ep < 0 || sp_ip < 0 || sp[sp_ep].weight != sp[sp_ip].weight)) return BIT1_ERR_INVALID_ARG;
+  // a re-injection source only acts at absorbing walls and must put particles inside the domain
+  if (any_src && g->bc == 1 &&
+      !(o->src_lo >= 0.0 && o->src_lo < o->src_hi && o->src_hi <= (double)g->nc * g->dx))
+    return BIT1_ERR_INVALID_ARG;
 
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return BIT1_ERR_CUDA;
 
-  const int staging = o->checkpoint_staging ? 1 : 0;
-  const Layout lay = make_layout(g->nc, g->bc, ns, (size_t)o->capacity, staging);
+  const Layout lay = make_layout(g->nc, g->bc, ns, sh);
   if (o->workspace_bytes < lay.total) return BIT1_ERR_CAPACITY;
 
   bit1_ctx* c = new (std::nothrow) bit1_ctx();
   if (!c) return BIT1_ERR_INVALID_ARG;
   memset(&c->P, 0, sizeof(Params));
   c->lay = lay;
+  c->shape = sh;
   c->ws = static_cast<char*>(o->workspace);
   c->cs = static_cast<cudaStream_t>(o->compute_stream);
   c->ss = o->side_stream ? static_cast<cudaStream_t>(o->side_stream) : c->cs;
-  c->staging = staging != 0;
-  c->variant = o->variant == 1 ? 1 : 2;
-  if (const char* ev = getenv("BIT1_VARIANT")) { const int v = atoi(ev); if (v == 1 || v == 2) c->variant = v; }
-  c->cur = 0; c->loaded = false; c->ckpt_pending = false; c->launches = 0; c->dt = dt;
+  c->staging = sh.staging != 0;
+  c->cur = 0; c->loaded = false; c->ckpt_pending = false; c->ckpt_reads_live = false; c->launches = 0; c->dt = dt;
   c->profiling = false; c->prof_steps = 0;
   c->graph[0] = c->graph[1] = nullptr;
-  c->use_graph = true;
-  if (const char* ev = getenv("BIT1_NO_GRAPH")) { if (atoi(ev) != 0) c->use_graph = false; }
+  c->use_graph = o->launch_mode == 0;
+  c->step_target = 0; c->last_general_step = ~0ull; c->burst = 0; c->general_steps_host = 0;
 
   Params& P = c->P;
   P.nc = g->nc; P.bc = g->bc; P.ng = lay.ng; P.ns = ns;
-  P.R = window_R();
+  P.R_max = sh.r_max;
+  P.R_fixed = o->window_radius_fixed > 0 ? o->window_radius_fixed - 1 : -1;
+  // side-list key: cell | class (2 bits) | order (array index * 4 + birth kind)
+  P.ord_bits = bits_for((unsigned long long)sh.cap * 4ull + 3ull);
+  P.cell_shift = P.ord_bits + 2;
+  P.key_bits = P.cell_shift + bits_for((unsigned long long)(g->nc - 1));
   P.n_sig = o->n_sig; P.n_norm = o->n_norm; P.sp_ep = sp_ep; P.sp_ip = sp_ip;
   P.seed_lo = (unsigned)o->seed; P.seed_hi = (unsigned)(o->seed >> 32);
-  P.capacity = (unsigned)o->capacity; P.ovf_cap = lay.ovf_cap; P.ovf_pow2 = lay.ovf_pow2;
+  P.capacity = (unsigned)o->capacity; P.ovf_cap = lay.ovf_cap;
   P.max_tiles = lay.max_tiles;
   // derived constants, one documented expression each
   P.inv_dx = 1.0 / g->dx;
@@ -354,15 +414,20 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   P.coop_scratch = ws + lay.coop_scratch;
   P.cell_base = reinterpret_cast<int*>(ws + lay.cell_base);
   P.ovf_before = reinterpret_cast<int*>(ws + lay.ovf_before);
+  P.ovf_lb = reinterpret_cast<int*>(ws + lay.ovf_lb);
+  P.ovf_ub = reinterpret_cast<int*>(ws + lay.ovf_ub);
+  P.radix_hist = reinterpret_cast<unsigned*>(ws + lay.radix_hist);
   P.tile_base = reinterpret_cast<int*>(ws + lay.tile_base);
   P.evt = reinterpret_cast<unsigned*>(ws + lay.evt);
   P.tile_hist = reinterpret_cast<unsigned*>(ws + lay.tile_hist);
   P.tile_pre = reinterpret_cast<unsigned*>(ws + lay.tile_pre);
   P.ovf_key = reinterpret_cast<unsigned long long*>(ws + lay.ovf_key);
   P.tmp_key = reinterpret_cast<unsigned long long*>(ws + lay.tmp_key);
+  P.tmp2_key = reinterpret_cast<unsigned long long*>(ws + lay.tmp2_key);
   P.ovf_idx = reinterpret_cast<unsigned*>(ws + lay.ovf_idx);
   P.ovf_dst = reinterpret_cast<int*>(ws + lay.ovf_dst);
   P.tmp_idx = reinterpret_cast<unsigned*>(ws + lay.tmp_idx);
+  P.tmp2_idx = reinterpret_cast<unsigned*>(ws + lay.tmp2_idx);
   P.ovf_rec = reinterpret_cast<OvfRec*>(ws + lay.ovf_rec);
   const PartLayout pl = part_layout((size_t)o->capacity);
   c->buf[0] = part_at(ws + lay.part[0], pl);
@@ -436,145 +501,40 @@ bit1_status bit1_profile(bit1_ctx* c, int enable) {
   return BIT1_OK;
 }
 
-bit1_status bit1_get_profile(bit1_ctx* c, double ms[4], uint64_t* steps) {
-  if (!c || !ms) return BIT1_ERR_INVALID_ARG;
-  CUDA_OK(cudaStreamSynchronize(c->cs));
-  double acc[4] = {0, 0, 0, 0};
-  for (size_t k = 0; k < c->prof_steps; ++k)
-    for (int j = 0; j < 4; ++j) {
-      float t = 0.f;
-      CUDA_OK(cudaEventElapsedTime(&t, c->prof_ev[k * 5 + j], c->prof_ev[k * 5 + j + 1]));
-      acc[j] += (double)t;
-    }
-  for (int j = 0; j < 4; ++j) ms[j] = acc[j];
-  if (steps) *steps = c->prof_steps;
-  c->prof_steps = 0;
-  return BIT1_OK;
-}
-
 static bit1_status read_state(bit1_ctx* c, DevState* h) {
   CUDA_OK(cudaMemcpyAsync(h, c->P.st, sizeof(DevState), cudaMemcpyDeviceToHost, c->cs));
   CUDA_OK(cudaStreamSynchronize(c->cs));
   return BIT1_OK;
 }
 
-// The NEXT-1 settings live in the host-side Params (the launches read them) and ride along in DevState so that a
-// checkpoint carries them; clear_sums also zeroes the running and latched averaging sums.
-static bit1_status push_settings(bit1_ctx* c, bool clear_sums) {
-  drop_graphs(c);
-  const int v[4] = {c->P.smooth, c->P.avg_window, c->P.avg_interval, 0};
-  CUDA_OK(cudaMemcpyAsync(&c->P.st->smooth_passes, v, sizeof(v), cudaMemcpyHostToDevice, c->cs));
-  if (clear_sums) {
-    CUDA_OK(cudaMemsetAsync(c->P.acc_dens, 0, avg_bytes(c->P.nc, c->P.ng, c->P.ns), c->cs));
-    CUDA_OK(cudaMemsetAsync(&c->P.st->acc_count, 0, 3 * sizeof(unsigned long long), c->cs));
-  }
-  CUDA_OK(cudaStreamSynchronize(c->cs));   // v is a stack object
-  return BIT1_OK;
-}
-
-bit1_status bit1_set_recycling(bit1_ctx* c, int species, int to, double vth) {
-  if (!c || species < 0 || species >= c->P.ns || to >= c->P.ns || (to >= 0 && !(vth >= 0.0))) return BIT1_ERR_INVALID_ARG;
-  drop_graphs(c);
-  c->P.sp[species].recycle_to = to < 0 ? -1 : to;
-  c->P.sp[species].recycle_vth = to < 0 ? 0.0 : vth;
-  rehash(c);
-  return BIT1_OK;
-}
-
-bit1_status bit1_set_neutral_target(bit1_ctx* c, int species) {
-  if (!c || species >= c->P.ns) return BIT1_ERR_INVALID_ARG;
-  drop_graphs(c);
-  c->P.target_species = species < 0 ? -1 : species;
-  c->P.kn = species < 0 ? 0.0
-                        : (0.5 * c->weight[species]) / (((double)c->P.sp[species].Q * c->P.area) * c->P.dx);
-  rehash(c);
-  return BIT1_OK;
-}
-
-bit1_status bit1_set_smoothing(bit1_ctx* c, int passes) {
-  if (!c || passes < 0 || passes > 8) return BIT1_ERR_INVALID_ARG;
-  c->P.smooth = passes;
-  return push_settings(c, false);
-}
-
-bit1_status bit1_set_averaging(bit1_ctx* c, int window, int interval) {
-  if (!c || window < 0 || (window > 0 && interval < window)) return BIT1_ERR_INVALID_ARG;
-  c->P.avg_window = window;
-  c->P.avg_interval = window > 0 ? interval : 0;
-  return push_settings(c, true);
-}
-
-bit1_status bit1_get_rho_smoothed(bit1_ctx* c, int64_t* out) {
-  if (!c || !out) return BIT1_ERR_INVALID_ARG;
-  if (!c->loaded) return BIT1_ERR_STATE;
-  CUDA_OK(cudaMemcpyAsync(out, c->P.smooth > 0 ? c->P.rho_s : c->P.rho, (size_t)c->P.ng * 8, cudaMemcpyDeviceToHost, c->cs));
-  CUDA_OK(cudaStreamSynchronize(c->cs));
-  return BIT1_OK;
-}
-
-bit1_status bit1_get_average(bit1_ctx* c, int64_t* dens_sum, double* phi_sum, uint64_t* count, uint64_t* step) {
-  if (!c) return BIT1_ERR_INVALID_ARG;
-  if (!c->loaded) return BIT1_ERR_STATE;
-  if (dens_sum) CUDA_OK(cudaMemcpyAsync(dens_sum, c->P.avg_dens, (size_t)c->P.ns * c->P.ng * 8, cudaMemcpyDeviceToHost, c->cs));
-  if (phi_sum) CUDA_OK(cudaMemcpyAsync(phi_sum, c->P.avg_phi, (size_t)(c->P.nc + 1) * 8, cudaMemcpyDeviceToHost, c->cs));
-  DevState h;
-  CUDA_OK(cudaMemcpyAsync(&h, c->P.st, sizeof(DevState), cudaMemcpyDeviceToHost, c->cs));
-  CUDA_OK(cudaStreamSynchronize(c->cs));
-  if (count) *count = h.avg_count;
-  if (step) *step = h.avg_step;
-  return BIT1_OK;
-}
-
-bit1_status bit1_load_particles(bit1_ctx* c, uint64_t n, const double* x, const double* vx, const double* vy,
-                                const double* vz, const uint8_t* sp, const uint32_t* pid, int on_device) {
-  NvtxRange nvtx_("bit1_load_particles");
-  if (!c || (n && (!x || !vx || !vy || !vz || !sp))) return BIT1_ERR_INVALID_ARG;
-  if (n > c->P.capacity) return BIT1_ERR_CAPACITY;
-  if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; }
-  drop_graphs(c);   // the buffer parity restarts at 0 while the cell_start swap keeps its state
-  const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
-  Particles in = c->buf[1], outp = c->buf[0];
-  CUDA_OK(cudaMemsetAsync(c->P.st, 0, sizeof(DevState), c->cs));
-  { bit1_status ps = push_settings(c, true); if (ps != BIT1_OK) return ps; }
-  // x, species and pid feed the sort keys and go first on the compute stream; the velocities follow on the side stream
-  // while the sort runs and are only needed by its final gather
-  const bool split = n && c->ss != c->cs;
-  if (n) {
-    CUDA_OK(cudaMemcpyAsync(in.x, x, n * 8, kind, c->cs));
-    CUDA_OK(cudaMemcpyAsync(in.sp, sp, n, kind, c->cs));
-    if (pid) CUDA_OK(cudaMemcpyAsync(in.pid, pid, n * 4, kind, c->cs));
-    cudaStream_t vs = split ? c->ss : c->cs;
-    if (split) {
-      CUDA_OK(cudaEventRecord(c->ev_load0, c->cs));          // everything that used this half of the store is done
-      CUDA_OK(cudaStreamWaitEvent(c->ss, c->ev_load0, 0));
-    }
-    CUDA_OK(cudaMemcpyAsync(in.vx, vx, n * 8, kind, vs));
-    CUDA_OK(cudaMemcpyAsync(in.vy, vy, n * 8, kind, vs));
-    CUDA_OK(cudaMemcpyAsync(in.vz, vz, n * 8, kind, vs));
-    if (split) CUDA_OK(cudaEventRecord(c->ev_load1, c->ss));
-  }
-  const unsigned n32 = (unsigned)n;
-  CUDA_OK(cudaMemcpyAsync(&c->P.st->n, &n32, 4, cudaMemcpyHostToDevice, c->cs));
-  c->launches += launch_load_sort(c->P, in, outp, n32, pid ? 1 : 0, c->ws + c->lay.scratch, c->cs,
-                                  split ? c->ev_load1 : nullptr);
-  c->cur = 0;
-  c->launches += launch_rebuild(c->P, c->buf[0], c->cs);
-  CUDA_OK(cudaGetLastError());
-  DevState h;
-  bit1_status s = read_state(c, &h);
-  if (s != BIT1_OK) return s;
-  if (h.load_error) { c->loaded = false; return BIT1_ERR_INVALID_ARG; }
-  c->loaded = true;
-  return BIT1_OK;
+// ---- enqueueing steps ---------------------------------------------------------------------------------------
+// host-side view of "which half of the store, which cell_start, which dens is this step's input": flips every step
+static void flip_parity(bit1_ctx* c) {
+  { int* t = c->P.cell_start; c->P.cell_start = c->P.cell_start_old; c->P.cell_start_old = t; }
+  { long long* t = c->P.dens; c->P.dens = c->P.dens_old; c->P.dens_old = t; }
+  c->cur ^= 1;
 }
 
 // one timestep enqueued on the compute stream (also under stream capture)
 static void enqueue_step(bit1_ctx* c, cudaEvent_t* ev) {
   // the arrangement the last step (or load / restart) produced is this step's input
-  { int* t = c->P.cell_start; c->P.cell_start = c->P.cell_start_old; c->P.cell_start_old = t; }
-  { long long* t = c->P.dens; c->P.dens = c->P.dens_old; c->P.dens_old = t; }
-  c->launches += launch_step(c->P, c->buf[c->cur], c->buf[c->cur ^ 1], c->variant, c->cs, ev);
-  c->cur ^= 1;
+  const int in = c->cur;
+  flip_parity(c);
+  c->launches += launch_step(c->P, c->buf[in], c->buf[in ^ 1], c->cs, ev);
+}
+
+// one timestep by the general path (general_kernels.cu)
+static bit1_status enqueue_general_step(bit1_ctx* c, int count_side_effects) {
+  if (c->ckpt_pending) {   // the scratch area may hold a checkpoint's device snapshot that is still being copied out
+    CUDA_OK(cudaEventSynchronize(c->ev_done));
+    c->ckpt_pending = false;
+    c->ckpt_reads_live = false;
+  }
+  const int in = c->cur;
+  flip_parity(c);
+  c->launches += launch_general_step(c->P, c->buf[in], c->buf[in ^ 1], count_side_effects, c->ws + c->lay.scratch, c->cs);
+  c->general_steps_host++;
+  return BIT1_OK;
 }
 
 // Two steps bring the buffer parity and the cell_start swap back to where they were, so a graph of two steps can be
@@ -597,10 +557,15 @@ static bool build_graph(bit1_ctx* c) {
   return true;
 }
 
-bit1_status bit1_step(bit1_ctx* c, uint64_t nsteps) {
-  NvtxRange nvtx_("bit1_step");
-  if (!c) return BIT1_ERR_INVALID_ARG;
-  if (!c->loaded) return BIT1_ERR_STATE;
+static bit1_status enqueue_steps(bit1_ctx* c, uint64_t nsteps) {
+  if (nsteps && c->ckpt_reads_live) {
+    // a checkpoint without staging reads the live half of the store on the side stream: the next step only reads
+    // that half too and may overlap the copy; the step after it writes there and has to wait
+    enqueue_step(c, nullptr);
+    --nsteps;
+    CUDA_OK(cudaStreamWaitEvent(c->cs, c->ev_done, 0));
+    c->ckpt_reads_live = false;
+  }
   if (c->use_graph && !c->profiling && nsteps >= 4) {
     if (!c->graph[c->cur] && !build_graph(c)) c->use_graph = false;
     if (c->graph[c->cur]) {
@@ -629,11 +594,196 @@ bit1_status bit1_step(bit1_ctx* c, uint64_t nsteps) {
   return BIT1_OK;
 }
 
+// Wait for the compute stream and bring the device to step_target: a stalled step (side list beyond its capacity,
+// DESIGN.md reading R-side) goes through the general path, the steps enqueued behind it (they returned at once)
+// are enqueued again.  After two stalls in a row a growing burst of steps takes the general path outright, so a
+// run whose every step overflows does not pay for a wasted mover pass and a host round trip each time.
+static bit1_status settle(bit1_ctx* c, DevState* out) {
+  DevState h;
+  for (;;) {
+    BIT1_OK_OR_RETURN(read_state(c, &h));
+    if (!h.stalled) break;
+    if (h.step >= c->step_target) return BIT1_ERR_CUDA;   // cannot happen: a stall leaves its step undone
+    uint64_t left = c->step_target - h.step;              // the stalled step and the no-ops behind it
+    if (left & 1ull) flip_parity(c);                      // back to the parity the stalled step found
+    c->burst = (c->last_general_step != ~0ull && h.step <= c->last_general_step + 2) ? (c->burst ? 2 * c->burst : 1) : 0;
+    if (c->burst > 64) c->burst = 64;
+    BIT1_OK_OR_RETURN(enqueue_general_step(c, 0));        // pass A has already counted this step's side effects
+    --left;
+    uint64_t b = c->burst < left ? c->burst : left;
+    left -= b;
+    for (; b; --b) BIT1_OK_OR_RETURN(enqueue_general_step(c, 1));
+    c->last_general_step = c->step_target - left - 1;
+    BIT1_OK_OR_RETURN(enqueue_steps(c, left));
+  }
+  if (out) *out = h;
+  return BIT1_OK;
+}
+
+bit1_status bit1_get_profile(bit1_ctx* c, double ms[4], uint64_t* steps) {
+  if (!c || !ms) return BIT1_ERR_INVALID_ARG;
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  double acc[4] = {0, 0, 0, 0};
+  for (size_t k = 0; k < c->prof_steps; ++k)
+    for (int j = 0; j < 4; ++j) {
+      float t = 0.f;
+      CUDA_OK(cudaEventElapsedTime(&t, c->prof_ev[k * 5 + j], c->prof_ev[k * 5 + j + 1]));
+      acc[j] += (double)t;
+    }
+  for (int j = 0; j < 4; ++j) ms[j] = acc[j];
+  if (steps) *steps = c->prof_steps;
+  c->prof_steps = 0;
+  return settle(c, nullptr);
+}
+
+// The NEXT-1 settings live in the host-side Params (the launches read them) and ride along in DevState so that a
+// checkpoint carries them; clear_sums also zeroes the running and latched averaging sums.
+static bit1_status push_settings(bit1_ctx* c, bool clear_sums) {
+  drop_graphs(c);
+  const int v[4] = {c->P.smooth, c->P.avg_window, c->P.avg_interval, 0};
+  CUDA_OK(cudaMemcpyAsync(&c->P.st->smooth_passes, v, sizeof(v), cudaMemcpyHostToDevice, c->cs));
+  if (clear_sums) {
+    CUDA_OK(cudaMemsetAsync(c->P.acc_dens, 0, avg_bytes(c->P.nc, c->P.ng, c->P.ns), c->cs));
+    CUDA_OK(cudaMemsetAsync(&c->P.st->acc_count, 0, 3 * sizeof(unsigned long long), c->cs));
+  }
+  CUDA_OK(cudaStreamSynchronize(c->cs));   // v is a stack object
+  return BIT1_OK;
+}
+
+bit1_status bit1_set_recycling(bit1_ctx* c, int species, int to, double vth) {
+  if (!c || species < 0 || species >= c->P.ns || to >= c->P.ns || (to >= 0 && !(vth >= 0.0))) return BIT1_ERR_INVALID_ARG;
+  if (c->loaded) BIT1_OK_OR_RETURN(settle(c, nullptr));
+  drop_graphs(c);
+  c->P.sp[species].recycle_to = to < 0 ? -1 : to;
+  c->P.sp[species].recycle_vth = to < 0 ? 0.0 : vth;
+  rehash(c);
+  return BIT1_OK;
+}
+
+bit1_status bit1_set_neutral_target(bit1_ctx* c, int species) {
+  if (!c || species >= c->P.ns) return BIT1_ERR_INVALID_ARG;
+  if (c->loaded) BIT1_OK_OR_RETURN(settle(c, nullptr));
+  drop_graphs(c);
+  c->P.target_species = species < 0 ? -1 : species;
+  c->P.kn = species < 0 ? 0.0
+                        : (0.5 * c->weight[species]) / (((double)c->P.sp[species].Q * c->P.area) * c->P.dx);
+  rehash(c);
+  return BIT1_OK;
+}
+
+bit1_status bit1_set_smoothing(bit1_ctx* c, int passes) {
+  if (!c || passes < 0 || passes > 8) return BIT1_ERR_INVALID_ARG;
+  if (c->loaded) BIT1_OK_OR_RETURN(settle(c, nullptr));   // steps already asked for run with the old setting
+  c->P.smooth = passes;
+  return push_settings(c, false);
+}
+
+bit1_status bit1_set_averaging(bit1_ctx* c, int window, int interval) {
+  if (!c || window < 0 || (window > 0 && interval < window)) return BIT1_ERR_INVALID_ARG;
+  if (c->loaded) BIT1_OK_OR_RETURN(settle(c, nullptr));
+  c->P.avg_window = window;
+  c->P.avg_interval = window > 0 ? interval : 0;
+  return push_settings(c, true);
+}
+
+bit1_status bit1_get_rho_smoothed(bit1_ctx* c, int64_t* out) {
+  if (!c || !out) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  BIT1_OK_OR_RETURN(settle(c, nullptr));
+  CUDA_OK(cudaMemcpyAsync(out, c->P.smooth > 0 ? c->P.rho_s : c->P.rho, (size_t)c->P.ng * 8, cudaMemcpyDeviceToHost, c->cs));
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  return BIT1_OK;
+}
+
+bit1_status bit1_get_average(bit1_ctx* c, int64_t* dens_sum, double* phi_sum, uint64_t* count, uint64_t* step) {
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  DevState h;
+  BIT1_OK_OR_RETURN(settle(c, &h));
+  if (dens_sum) CUDA_OK(cudaMemcpyAsync(dens_sum, c->P.avg_dens, (size_t)c->P.ns * c->P.ng * 8, cudaMemcpyDeviceToHost, c->cs));
+  if (phi_sum) CUDA_OK(cudaMemcpyAsync(phi_sum, c->P.avg_phi, (size_t)(c->P.nc + 1) * 8, cudaMemcpyDeviceToHost, c->cs));
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  if (count) *count = h.avg_count;
+  if (step) *step = h.avg_step;
+  return BIT1_OK;
+}
+
+// DevState of a freshly loaded / restarted context: the sort window starts at its smallest radius
+static void fresh_window(const Params& P, DevState* h) {
+  h->R_cur = P.R_fixed >= 0 ? (unsigned)P.R_fixed : 1u;
+  h->R_next = h->R_cur;
+  h->stalled = 0;
+  for (int e = 0; e < kMaxR + 2; ++e) h->excess[e] = 0;
+}
+
+bit1_status bit1_load_particles(bit1_ctx* c, uint64_t n, const double* x, const double* vx, const double* vy,
+                                const double* vz, const uint8_t* sp, const uint32_t* pid, int on_device) {
+  NvtxRange nvtx_("bit1_load_particles");
+  if (!c || (n && (!x || !vx || !vy || !vz || !sp))) return BIT1_ERR_INVALID_ARG;
+  if (n > c->P.capacity) return BIT1_ERR_CAPACITY;
+  if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; c->ckpt_reads_live = false; }
+  CUDA_OK(cudaStreamSynchronize(c->cs));   // whatever was enqueued (stalled or not) is superseded by the load
+  drop_graphs(c);   // the buffer parity restarts at 0 while the cell_start swap keeps its state
+  c->loaded = false;
+  c->step_target = 0; c->last_general_step = ~0ull; c->burst = 0;
+  const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  Particles in = c->buf[1], outp = c->buf[0];
+  DevState h0;
+  memset(&h0, 0, sizeof(h0));
+  fresh_window(c->P, &h0);
+  h0.n = (unsigned)n;
+  CUDA_OK(cudaMemcpyAsync(c->P.st, &h0, sizeof(DevState), cudaMemcpyHostToDevice, c->cs));
+  { bit1_status ps = push_settings(c, true); if (ps != BIT1_OK) return ps; }   // synchronises: h0 is a stack object
+  // x, species and pid feed the sort keys and go first on the compute stream; the velocities follow on the side stream
+  // while the sort runs and are only needed by its final gather
+  const bool split = n && c->ss != c->cs;
+  if (n) {
+    CUDA_OK(cudaMemcpyAsync(in.x, x, n * 8, kind, c->cs));
+    CUDA_OK(cudaMemcpyAsync(in.sp, sp, n, kind, c->cs));
+    if (pid) CUDA_OK(cudaMemcpyAsync(in.pid, pid, n * 4, kind, c->cs));
+    cudaStream_t vs = split ? c->ss : c->cs;
+    if (split) {
+      CUDA_OK(cudaEventRecord(c->ev_load0, c->cs));          // everything that used this half of the store is done
+      CUDA_OK(cudaStreamWaitEvent(c->ss, c->ev_load0, 0));
+    }
+    CUDA_OK(cudaMemcpyAsync(in.vx, vx, n * 8, kind, vs));
+    CUDA_OK(cudaMemcpyAsync(in.vy, vy, n * 8, kind, vs));
+    CUDA_OK(cudaMemcpyAsync(in.vz, vz, n * 8, kind, vs));
+    if (split) CUDA_OK(cudaEventRecord(c->ev_load1, c->ss));
+  }
+  const unsigned n32 = (unsigned)n;
+  // validate before anything indexes by species or cell: a bad species tag or a position outside [0, L) is refused
+  // here, not carried into the deposit (which would index past the per-species arrays)
+  c->launches += launch_load_validate(c->P, in, n32, c->cs);
+  DevState h;
+  BIT1_OK_OR_RETURN(read_state(c, &h));
+  if (h.load_error) {
+    if (split) CUDA_OK(cudaStreamSynchronize(c->ss));
+    return BIT1_ERR_INVALID_ARG;
+  }
+  c->launches += launch_load_sort(c->P, in, outp, n32, pid ? 1 : 0, c->ws + c->lay.scratch, c->cs,
+                                  split ? c->ev_load1 : nullptr);
+  c->cur = 0;
+  c->launches += launch_rebuild(c->P, c->buf[0], c->cs);
+  CUDA_OK(cudaGetLastError());
+  BIT1_OK_OR_RETURN(read_state(c, &h));
+  c->loaded = true;
+  return BIT1_OK;
+}
+
+bit1_status bit1_step(bit1_ctx* c, uint64_t nsteps) {
+  NvtxRange nvtx_("bit1_step");
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded) return BIT1_ERR_STATE;
+  c->step_target += nsteps;
+  return enqueue_steps(c, nsteps);
+}
+
 bit1_status bit1_sync(bit1_ctx* c) {
   if (!c) return BIT1_ERR_INVALID_ARG;
   DevState h;
-  bit1_status s = read_state(c, &h);
-  if (s != BIT1_OK) return s;
+  if (!c->loaded) { BIT1_OK_OR_RETURN(read_state(c, &h)); return BIT1_OK; }
+  BIT1_OK_OR_RETURN(settle(c, &h));
   return h.flags ? BIT1_ERR_DEVICE_FLAG : BIT1_OK;
 }
 
@@ -657,9 +807,7 @@ bit1_status bit1_get_count(bit1_ctx* c, uint64_t* n_live, uint64_t* step, uint64
     return BIT1_OK;
   }
   DevState h;
-  bit1_status s = read_state(c, &h);
-  if (s != BIT1_OK) return s;
-  if (h.flags & kFlagOverflow) return BIT1_ERR_DEVICE_FLAG;
+  BIT1_OK_OR_RETURN(settle(c, &h));
   if (n_live) *n_live = h.n;
   if (step) *step = h.step;
   return BIT1_OK;
@@ -668,6 +816,7 @@ bit1_status bit1_get_count(bit1_ctx* c, uint64_t* n_live, uint64_t* step, uint64
 bit1_status bit1_get_rho(bit1_ctx* c, int64_t* rho_fixed, double* rho_si) {
   if (!c) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
+  BIT1_OK_OR_RETURN(settle(c, nullptr));
   const int ng = c->P.ng;
   int64_t* tmp = rho_fixed;
   if (!tmp) tmp = static_cast<int64_t*>(malloc((size_t)ng * 8));
@@ -689,8 +838,8 @@ bit1_status bit1_get_rho(bit1_ctx* c, int64_t* rho_fixed, double* rho_si) {
 bit1_status bit1_get_phi(bit1_ctx* c, double* phi) {
   if (!c || !phi) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
-  bit1_status s = fetch(c, phi, c->P.phi, (size_t)(c->P.nc + 1) * 8);
-  if (s != BIT1_OK) return s;
+  BIT1_OK_OR_RETURN(settle(c, nullptr));
+  BIT1_OK_OR_RETURN(fetch(c, phi, c->P.phi, (size_t)(c->P.nc + 1) * 8));
   CUDA_OK(cudaStreamSynchronize(c->cs));
   return BIT1_OK;
 }
@@ -698,8 +847,8 @@ bit1_status bit1_get_phi(bit1_ctx* c, double* phi) {
 bit1_status bit1_get_E(bit1_ctx* c, double* E) {
   if (!c || !E) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
-  bit1_status s = fetch(c, E, c->P.E, (size_t)(c->P.nc + 1) * 8);
-  if (s != BIT1_OK) return s;
+  BIT1_OK_OR_RETURN(settle(c, nullptr));
+  BIT1_OK_OR_RETURN(fetch(c, E, c->P.E, (size_t)(c->P.nc + 1) * 8));
   CUDA_OK(cudaStreamSynchronize(c->cs));
   return BIT1_OK;
 }
@@ -707,8 +856,8 @@ bit1_status bit1_get_E(bit1_ctx* c, double* E) {
 bit1_status bit1_get_dens(bit1_ctx* c, int64_t* dens) {
   if (!c || !dens) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
-  bit1_status s = fetch(c, dens, c->P.dens, (size_t)c->P.ns * c->P.ng * 8);
-  if (s != BIT1_OK) return s;
+  BIT1_OK_OR_RETURN(settle(c, nullptr));
+  BIT1_OK_OR_RETURN(fetch(c, dens, c->P.dens, (size_t)c->P.ns * c->P.ng * 8));
   CUDA_OK(cudaStreamSynchronize(c->cs));
   return BIT1_OK;
 }
@@ -717,6 +866,7 @@ bit1_status bit1_get_moments(bit1_ctx* c, bit1_moments* out) {
   NvtxRange nvtx_("bit1_get_moments");
   if (!c || !out) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
+  BIT1_OK_OR_RETURN(settle(c, nullptr));
   const Params& P = c->P;
   double* partial = reinterpret_cast<double*>(c->ws + c->lay.mom);
   double* dres = partial + (size_t)1024 * kMaxSpecies * 3;
@@ -748,6 +898,7 @@ bit1_status bit1_get_moments(bit1_ctx* c, bit1_moments* out) {
   out->nu_overflow = h.nu_overflow; out->dir_fallback = h.dir_fallback; out->escape = h.escape;
   out->births = h.births; out->reinject = h.reinject; out->recycled = h.recycled;
   out->far_movers = h.far_movers; out->max_far_movers_per_step = h.max_far_movers;
+  out->general_steps = h.general_steps; out->window_radius = h.R_cur;
   bool any = false;
   for (int k = 0; k < P.ns; ++k) any = any || dens_out[k];
   if (any) {
@@ -776,16 +927,18 @@ bit1_status bit1_get_particles(bit1_ctx* c, double* x, double* vx, double* vy, d
   if (!c) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
   DevState h;
-  bit1_status s = read_state(c, &h);
-  if (s != BIT1_OK) return s;
-  if (h.flags & kFlagOverflow) return BIT1_ERR_DEVICE_FLAG;
+  BIT1_OK_OR_RETURN(settle(c, &h));
   const size_t n = h.n;
   const Particles& p = c->buf[c->cur];
   if (x) CUDA_OK(cudaMemcpyAsync(x, p.x, n * 8, cudaMemcpyDeviceToHost, c->cs));
   if (vx) CUDA_OK(cudaMemcpyAsync(vx, p.vx, n * 8, cudaMemcpyDeviceToHost, c->cs));
   if (vy) CUDA_OK(cudaMemcpyAsync(vy, p.vy, n * 8, cudaMemcpyDeviceToHost, c->cs));
   if (vz) CUDA_OK(cudaMemcpyAsync(vz, p.vz, n * 8, cudaMemcpyDeviceToHost, c->cs));
-  if (cell) CUDA_OK(cudaMemcpyAsync(cell, p.cell, n * 4, cudaMemcpyDeviceToHost, c->cs));
+  if (cell) {
+    // the store's cell index is cell_of(x) by construction; no step reads or writes the array, it is filled on demand
+    c->launches += launch_fill_cells(c->P, p, c->cs);
+    CUDA_OK(cudaMemcpyAsync(cell, p.cell, n * 4, cudaMemcpyDeviceToHost, c->cs));
+  }
   if (pid) CUDA_OK(cudaMemcpyAsync(pid, p.pid, n * 4, cudaMemcpyDeviceToHost, c->cs));
   if (sp) CUDA_OK(cudaMemcpyAsync(sp, p.sp, n, cudaMemcpyDeviceToHost, c->cs));
   int32_t* cs32 = nullptr;
@@ -810,7 +963,9 @@ bit1_status bit1_export_species(bit1_ctx* c, int species, uint64_t capacity_out,
                                 uint32_t* pid) {
   if (!c || species < 0 || species >= c->P.ns || !n_out) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
-  if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; }  // staging area = scratch
+  BIT1_OK_OR_RETURN(settle(c, nullptr));
+  // staging area = scratch; the idle half of the store is also about to be written
+  if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; c->ckpt_reads_live = false; }
   char* sc = c->ws + c->lay.scratch;
   c->launches += launch_export_count(c->P, c->buf[c->cur], species, c->P.capacity, sc, c->cs);
   unsigned long long total = 0;
@@ -845,6 +1000,7 @@ bit1_status bit1_export_species(bit1_ctx* c, int species, uint64_t capacity_out,
 bit1_status bit1_set_E(bit1_ctx* c, const double* E, int freeze) {
   if (!c || !E) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
+  BIT1_OK_OR_RETURN(settle(c, nullptr));
   CUDA_OK(cudaMemcpyAsync(c->P.E, E, (size_t)(c->P.nc + 1) * 8, cudaMemcpyHostToDevice, c->cs));
   const unsigned f = freeze ? 1u : 0u;
   CUDA_OK(cudaMemcpyAsync(&c->P.st->freeze_field, &f, 4, cudaMemcpyHostToDevice, c->cs));
@@ -855,8 +1011,11 @@ bit1_status bit1_set_E(bit1_ctx* c, const double* E, int freeze) {
 bit1_status bit1_set_step(bit1_ctx* c, uint64_t step) {
   if (!c) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
+  BIT1_OK_OR_RETURN(settle(c, nullptr));
   CUDA_OK(cudaMemcpyAsync(&c->P.st->step, &step, 8, cudaMemcpyHostToDevice, c->cs));
   CUDA_OK(cudaStreamSynchronize(c->cs));
+  c->step_target = step;
+  c->last_general_step = ~0ull;
   return BIT1_OK;
 }
 
@@ -869,36 +1028,65 @@ bit1_status bit1_checkpoint(bit1_ctx* c, void* host, size_t cap, size_t* written
   NvtxRange nvtx_("bit1_checkpoint");
   if (!c || !host) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
-  const CkptLayout cl = ckpt_layout(c->P.nc, c->P.ng, c->P.ns, c->P.capacity);
+  if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; c->ckpt_reads_live = false; }
+  // the live particle count sizes the blob, so the steps asked for so far are waited for here; the copy itself
+  // (the expensive part) runs on the side stream behind an event and overlaps the steps that follow
+  DevState h;
+  BIT1_OK_OR_RETURN(settle(c, &h));
+  const size_t n = h.n;
+  const CkptLayout cl = ckpt_layout(c->P.nc, c->P.ng, c->P.ns, n);
   if (cap < cl.bytes) return BIT1_ERR_CAPACITY;
-  const PartLayout pl = part_layout(c->P.capacity);
   CkptHeader hd;
   memset(&hd, 0, sizeof(hd));
   memcpy(hd.magic, "BIT1CKPT", 8);
   hd.version = kCkptVersion; hd.nc = c->P.nc; hd.ns = c->P.ns; hd.bc = c->P.bc;
-  hd.capacity = c->P.capacity; hd.cfg_hash = c->cfg_hash; hd.bytes = cl.bytes;
+  hd.capacity = c->P.capacity; hd.cfg_hash = c->cfg_hash; hd.bytes = cl.bytes; hd.n = n;
   memset(host, 0, 256);
   memcpy(host, &hd, sizeof(hd));
   char* hb = static_cast<char*>(host);
-  const char* live = c->ws + c->lay.part[c->cur];
+  const Particles& p = c->buf[c->cur];
+  const size_t ab = avg_bytes(c->P.nc, c->P.ng, c->P.ns);
+  const cudaMemcpyKind d2d = cudaMemcpyDeviceToDevice, d2h = cudaMemcpyDeviceToHost;
   if (c->staging) {
-    // snapshot on the compute stream, copy out on the side stream: later steps overlap the D2H
-    if (c->ckpt_pending) CUDA_OK(cudaStreamWaitEvent(c->cs, c->ev_done, 0));
+    // snapshot on the compute stream (blob layout, live particles only), one copy out on the side stream: the
+    // steps that follow overlap the D2H and are free to overwrite the store
     char* sg = c->ws + c->lay.scratch;
-    CUDA_OK(cudaMemcpyAsync(sg + cl.state, c->P.st, sizeof(DevState), cudaMemcpyDeviceToDevice, c->cs));
-    CUDA_OK(cudaMemcpyAsync(sg + cl.cell_start, c->P.cell_start, (size_t)(c->P.nc + 1) * 4, cudaMemcpyDeviceToDevice, c->cs));
-    CUDA_OK(cudaMemcpyAsync(sg + cl.avg, c->P.acc_dens, avg_bytes(c->P.nc, c->P.ng, c->P.ns), cudaMemcpyDeviceToDevice, c->cs));
-    CUDA_OK(cudaMemcpyAsync(sg + cl.part, live, pl.bytes, cudaMemcpyDeviceToDevice, c->cs));
+    CUDA_OK(cudaMemcpyAsync(sg + cl.state, c->P.st, sizeof(DevState), d2d, c->cs));
+    CUDA_OK(cudaMemcpyAsync(sg + cl.avg, c->P.acc_dens, ab, d2d, c->cs));
+    if (n) {
+      CUDA_OK(cudaMemcpyAsync(sg + cl.x, p.x, n * 8, d2d, c->cs));
+      CUDA_OK(cudaMemcpyAsync(sg + cl.vx, p.vx, n * 8, d2d, c->cs));
+      CUDA_OK(cudaMemcpyAsync(sg + cl.vy, p.vy, n * 8, d2d, c->cs));
+      CUDA_OK(cudaMemcpyAsync(sg + cl.vz, p.vz, n * 8, d2d, c->cs));
+      CUDA_OK(cudaMemcpyAsync(sg + cl.pid, p.pid, n * 4, d2d, c->cs));
+      CUDA_OK(cudaMemcpyAsync(sg + cl.sp, p.sp, n, d2d, c->cs));
+    }
     CUDA_OK(cudaEventRecord(c->ev_snap, c->cs));
     CUDA_OK(cudaStreamWaitEvent(c->ss, c->ev_snap, 0));
-    CUDA_OK(cudaMemcpyAsync(hb + cl.state, sg + cl.state, cl.bytes - cl.state, cudaMemcpyDeviceToHost, c->ss));
+    CUDA_OK(cudaMemcpyAsync(hb + cl.state, sg + cl.state, cl.bytes - cl.state, d2h, c->ss));
     CUDA_OK(cudaEventRecord(c->ev_done, c->ss));
   } else {
-    CUDA_OK(cudaMemcpyAsync(hb + cl.state, c->P.st, sizeof(DevState), cudaMemcpyDeviceToHost, c->cs));
-    CUDA_OK(cudaMemcpyAsync(hb + cl.cell_start, c->P.cell_start, (size_t)(c->P.nc + 1) * 4, cudaMemcpyDeviceToHost, c->cs));
-    CUDA_OK(cudaMemcpyAsync(hb + cl.avg, c->P.acc_dens, avg_bytes(c->P.nc, c->P.ng, c->P.ns), cudaMemcpyDeviceToHost, c->cs));
-    CUDA_OK(cudaMemcpyAsync(hb + cl.part, live, pl.bytes, cudaMemcpyDeviceToHost, c->cs));
-    CUDA_OK(cudaEventRecord(c->ev_done, c->cs));
+    // no snapshot area: the small mutable pieces are snapshotted, the particle arrays are copied out of the live
+    // half of the store on the side stream; the next step only reads that half and may overlap, the one after
+    // waits for the copy (enqueue_steps)
+    char* sm = c->ws + c->lay.small;
+    const CkptLayout c0 = ckpt_layout(c->P.nc, c->P.ng, c->P.ns, 0);
+    CUDA_OK(cudaMemcpyAsync(sm + c0.state, c->P.st, sizeof(DevState), d2d, c->cs));
+    CUDA_OK(cudaMemcpyAsync(sm + c0.avg, c->P.acc_dens, ab, d2d, c->cs));
+    CUDA_OK(cudaEventRecord(c->ev_snap, c->cs));
+    CUDA_OK(cudaStreamWaitEvent(c->ss, c->ev_snap, 0));
+    CUDA_OK(cudaMemcpyAsync(hb + cl.state, sm + c0.state, sizeof(DevState), d2h, c->ss));
+    CUDA_OK(cudaMemcpyAsync(hb + cl.avg, sm + c0.avg, ab, d2h, c->ss));
+    if (n) {
+      CUDA_OK(cudaMemcpyAsync(hb + cl.x, p.x, n * 8, d2h, c->ss));
+      CUDA_OK(cudaMemcpyAsync(hb + cl.vx, p.vx, n * 8, d2h, c->ss));
+      CUDA_OK(cudaMemcpyAsync(hb + cl.vy, p.vy, n * 8, d2h, c->ss));
+      CUDA_OK(cudaMemcpyAsync(hb + cl.vz, p.vz, n * 8, d2h, c->ss));
+      CUDA_OK(cudaMemcpyAsync(hb + cl.pid, p.pid, n * 4, d2h, c->ss));
+      CUDA_OK(cudaMemcpyAsync(hb + cl.sp, p.sp, n, d2h, c->ss));
+    }
+    CUDA_OK(cudaEventRecord(c->ev_done, c->ss));
+    c->ckpt_reads_live = c->ss != c->cs;
   }
   c->ckpt_pending = true;
   if (written) *written = cl.bytes;
@@ -910,6 +1098,7 @@ bit1_status bit1_checkpoint_wait(bit1_ctx* c) {
   if (c->ckpt_pending) {
     CUDA_OK(cudaEventSynchronize(c->ev_done));
     c->ckpt_pending = false;
+    c->ckpt_reads_live = false;
   }
   return BIT1_OK;
 }
@@ -917,33 +1106,52 @@ bit1_status bit1_checkpoint_wait(bit1_ctx* c) {
 bit1_status bit1_restart(bit1_ctx* c, const void* blob, size_t bytes) {
   NvtxRange nvtx_("bit1_restart");
   if (!c || !blob) return BIT1_ERR_INVALID_ARG;
-  const CkptLayout cl = ckpt_layout(c->P.nc, c->P.ng, c->P.ns, c->P.capacity);
-  if (bytes < cl.bytes) return BIT1_ERR_CHECKPOINT;
+  if (bytes < 256 + sizeof(DevState)) return BIT1_ERR_CHECKPOINT;
   CkptHeader hd;
   memcpy(&hd, blob, sizeof(hd));
   if (memcmp(hd.magic, "BIT1CKPT", 8) != 0 || hd.version != kCkptVersion || hd.nc != c->P.nc || hd.ns != c->P.ns ||
-      hd.bc != c->P.bc || hd.capacity != c->P.capacity || hd.cfg_hash != c->cfg_hash || hd.bytes != cl.bytes)
+      hd.bc != c->P.bc || hd.capacity != c->P.capacity || hd.cfg_hash != c->cfg_hash || hd.n > c->P.capacity)
     return BIT1_ERR_CHECKPOINT;
-  if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; }
+  const size_t n = (size_t)hd.n;
+  const CkptLayout cl = ckpt_layout(c->P.nc, c->P.ng, c->P.ns, n);
+  if (hd.bytes != cl.bytes || bytes < cl.bytes) return BIT1_ERR_CHECKPOINT;
+  if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; c->ckpt_reads_live = false; }
   drop_graphs(c);
-  const PartLayout pl = part_layout(c->P.capacity);
   const char* hb = static_cast<const char*>(blob);
   DevState h;
   memcpy(&h, hb + cl.state, sizeof(DevState));
-  if (h.n > c->P.capacity) return BIT1_ERR_CHECKPOINT;
+  if (h.n != n) return BIT1_ERR_CHECKPOINT;
   h.ovf_count = 0; h.ovf_valid = 0; h.freeze_field = 0; h.load_error = 0; h.n_next = h.n;
+  fresh_window(c->P, &h);
   CUDA_OK(cudaStreamSynchronize(c->cs));
   if (h.smooth_passes < 0 || h.smooth_passes > 8 || h.avg_window < 0 || h.avg_interval < h.avg_window)
     return BIT1_ERR_CHECKPOINT;
+  c->loaded = false;
   CUDA_OK(cudaMemcpyAsync(c->P.st, &h, sizeof(DevState), cudaMemcpyHostToDevice, c->cs));
   CUDA_OK(cudaStreamSynchronize(c->cs));  // h is a stack object
   c->P.smooth = h.smooth_passes; c->P.avg_window = h.avg_window; c->P.avg_interval = h.avg_interval;
   CUDA_OK(cudaMemcpyAsync(c->P.acc_dens, hb + cl.avg, avg_bytes(c->P.nc, c->P.ng, c->P.ns), cudaMemcpyHostToDevice, c->cs));
   c->cur = 0;
-  CUDA_OK(cudaMemcpyAsync(c->ws + c->lay.part[0], hb + cl.part, pl.bytes, cudaMemcpyHostToDevice, c->cs));
+  const Particles& p = c->buf[0];
+  const cudaMemcpyKind h2d = cudaMemcpyHostToDevice;
+  if (n) {
+    CUDA_OK(cudaMemcpyAsync(p.x, hb + cl.x, n * 8, h2d, c->cs));
+    CUDA_OK(cudaMemcpyAsync(p.vx, hb + cl.vx, n * 8, h2d, c->cs));
+    CUDA_OK(cudaMemcpyAsync(p.vy, hb + cl.vy, n * 8, h2d, c->cs));
+    CUDA_OK(cudaMemcpyAsync(p.vz, hb + cl.vz, n * 8, h2d, c->cs));
+    CUDA_OK(cudaMemcpyAsync(p.pid, hb + cl.pid, n * 4, h2d, c->cs));
+    CUDA_OK(cudaMemcpyAsync(p.sp, hb + cl.sp, n, h2d, c->cs));
+  }
+  // the blob's body is data from outside: species tags, positions and their order are checked before anything
+  // indexes by them (header and hash only vouch for the configuration)
+  c->launches += launch_state_validate(c->P, p, (unsigned)n, c->cs);
+  DevState hv;
+  BIT1_OK_OR_RETURN(read_state(c, &hv));
+  if (hv.load_error) return BIT1_ERR_CHECKPOINT;
   c->launches += launch_rebuild(c->P, c->buf[0], c->cs);
   CUDA_OK(cudaGetLastError());
   CUDA_OK(cudaStreamSynchronize(c->cs));
+  c->step_target = h.step; c->last_general_step = ~0ull; c->burst = 0;
   c->loaded = true;
   return BIT1_OK;
 }

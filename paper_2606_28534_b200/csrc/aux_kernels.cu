@@ -1,4 +1,5 @@
-// Kernels off the per-step path: load (validate, cell index, general stable sort by cell), moments.
+// Kernels off the per-step path: load (validate, cell index, general stable sort by cell), moments, export, and the
+// cell-index fill (the store's cell array is cell_of(x) by construction and only materialised when asked for).
 // The load-time sort is a multi-pass LSD radix sort (8-bit digits) on (cell, original index); it is the
 // general counterpart of the banded single-scatter sort of the step kernels and is not timed.
 #include "aux_kernels.h"
@@ -16,7 +17,6 @@ __global__ void __launch_bounds__(256) k_load_prepare(const __grid_constant__ Pa
     const int s = in.sp[i];
     if (!(x >= 0.0 && x < P.L) || s >= P.ns) bad = true;
     const int c = cell_of(P, x);
-    in.cell[i] = c;
     if (!have_pid) in.pid[i] = (unsigned)i;
     const unsigned pid = in.pid[i];
     maxpid = max(maxpid, pid + 1u);
@@ -26,6 +26,36 @@ __global__ void __launch_bounds__(256) k_load_prepare(const __grid_constant__ Pa
   for (int o = 16; o > 0; o >>= 1) maxpid = max(maxpid, __shfl_xor_sync(0xffffffffu, maxpid, o));
   if ((threadIdx.x & 31) == 0 && maxpid) atomicMax(&P.st->next_pid, maxpid);
   if (bad) atomicOr(&P.st->load_error, 1u);
+}
+
+// bit1_load_particles: every position inside [0, L), every species tag known -- checked before anything indexes by them
+__global__ void __launch_bounds__(256) k_load_validate(const __grid_constant__ Params P, Particles in, unsigned n) {
+  bool bad = false;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const double x = in.x[i];
+    if (!(x >= 0.0 && x < P.L) || (int)in.sp[i] >= P.ns) bad = true;
+  }
+  if (bad) atomicOr(&P.st->load_error, 1u);
+}
+int launch_load_validate(const Params& P, const Particles& in, unsigned n, cudaStream_t s) {
+  if (n == 0) return 0;
+  k_load_validate<<<148 * 8, 256, 0, s>>>(P, in, n);
+  return 1;
+}
+// bit1_restart: the same, and the positions must be in cell order (the blob's body is data from outside)
+__global__ void __launch_bounds__(256) k_state_validate(const __grid_constant__ Params P, Particles p, unsigned n) {
+  bool bad = false;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+    const double x = p.x[i];
+    if (!(x >= 0.0 && x < P.L) || (int)p.sp[i] >= P.ns) bad = true;
+    else if (i > 0 && cell_of(P, p.x[i - 1]) > cell_of(P, x)) bad = true;
+  }
+  if (bad) atomicOr(&P.st->load_error, 1u);
+}
+int launch_state_validate(const Params& P, const Particles& p, unsigned n, cudaStream_t s) {
+  if (n == 0) return 0;
+  k_state_validate<<<148 * 8, 256, 0, s>>>(P, p, n);
+  return 1;
 }
 
 constexpr int kRadixItems = 8;
@@ -142,7 +172,7 @@ __global__ void __launch_bounds__(1024) k_scan_chunks(unsigned* a, size_t n, con
   }
 }
 // tmp: (n / kScanChunk + 1) words
-static int launch_scan_u32(unsigned* a, size_t n, unsigned* tmp, cudaStream_t s) {
+int launch_scan_u32(unsigned* a, size_t n, unsigned* tmp, cudaStream_t s) {
   if (n <= (size_t)4 * kScanChunk) {
     k_scan_u32<<<1, 1024, 0, s>>>(a, n);
     return 1;
@@ -209,25 +239,23 @@ __global__ void __launch_bounds__(256) k_gather(Particles in, Particles out, con
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
     const unsigned j = perm[i];
     out.x[i] = in.x[j]; out.vx[i] = in.vx[j]; out.vy[i] = in.vy[j]; out.vz[i] = in.vz[j];
-    out.cell[i] = in.cell[j]; out.pid[i] = in.pid[j]; out.sp[i] = in.sp[j];
+    out.pid[i] = in.pid[j]; out.sp[i] = in.sp[j];
   }
 }
 
-int launch_load_sort(const Params& P, const Particles& in, const Particles& out, unsigned n, int have_pid,
-                     void* scratch, cudaStream_t s, cudaEvent_t before_gather) {
-  if (n == 0) return 0;
+// Stable LSD radix sort (8-bit digits over key bits [0, bits)) of n (key, value) pairs of 32-bit words.
+// scratch: [k0 | v0 | k1 | v1] of `stride` words each, then the per-block digit counts; the input pairs are in
+// (k0, v0); *keys / *vals say which pair of arrays holds the result.
+int launch_radix_sort_u32(unsigned n, unsigned stride, int bits, void* scratch, cudaStream_t s, unsigned** keys,
+                          unsigned** vals) {
+  unsigned* k0 = reinterpret_cast<unsigned*>(scratch);
+  unsigned* v0 = k0 + stride;
+  unsigned* k1 = v0 + stride;
+  unsigned* v1 = k1 + stride;
+  unsigned* bh = v1 + stride;
   int launches = 0;
   const unsigned nblocks = (n + kRadixChunk - 1) / kRadixChunk;
-  unsigned* k0 = reinterpret_cast<unsigned*>(scratch);
-  unsigned* v0 = k0 + P.capacity;
-  unsigned* k1 = v0 + P.capacity;
-  unsigned* v1 = k1 + P.capacity;
-  unsigned* bh = v1 + P.capacity;
-  k_load_prepare<<<148 * 8, 256, 0, s>>>(P, in, n, have_pid, k0, v0);
-  ++launches;
-  int bits = 0;
-  while ((1ll << bits) < (long long)P.nc) ++bits;
-  for (int shift = 0; shift < bits; shift += 8) {
+  for (int shift = 0; shift < bits && n > 0; shift += 8) {
     k_radix_hist<<<nblocks, 256, 0, s>>>(k0, n, shift, bh, nblocks);
     launches += launch_scan_u32(bh, (size_t)256 * nblocks, bh + (size_t)256 * nblocks, s);
     k_radix_scatter<<<nblocks, 256, 0, s>>>(k0, v0, n, shift, bh, nblocks, k1, v1);
@@ -235,8 +263,25 @@ int launch_load_sort(const Params& P, const Particles& in, const Particles& out,
     unsigned* t = k0; k0 = k1; k1 = t;
     t = v0; v0 = v1; v1 = t;
   }
+  *keys = k0;
+  *vals = v0;
+  return launches;
+}
+
+int launch_load_sort(const Params& P, const Particles& in, const Particles& out, unsigned n, int have_pid,
+                     void* scratch, cudaStream_t s, cudaEvent_t before_gather) {
+  if (n == 0) return 0;
+  int launches = 0;
+  unsigned* k0 = reinterpret_cast<unsigned*>(scratch);
+  unsigned* v0 = k0 + P.capacity;
+  k_load_prepare<<<148 * 8, 256, 0, s>>>(P, in, n, have_pid, k0, v0);
+  ++launches;
+  int bits = 0;
+  while ((1ll << bits) < (long long)P.nc) ++bits;
+  unsigned *ks = nullptr, *vs = nullptr;
+  launches += launch_radix_sort_u32(n, P.capacity, bits, scratch, s, &ks, &vs);
   if (before_gather) cudaStreamWaitEvent(s, before_gather, 0);   // the velocity arrays arrive on another stream
-  k_gather<<<148 * 8, 256, 0, s>>>(in, out, v0, n);
+  k_gather<<<148 * 8, 256, 0, s>>>(in, out, vs, n);
   return launches + 1;
 }
 
@@ -319,6 +364,17 @@ __global__ void __launch_bounds__(1024) k_moments_final(const __grid_constant__ 
   }
 }
 
+// cell[i] = cell_of(x[i]) for the live particles (bit1_get_particles; a step never reads or writes the cell array)
+__global__ void __launch_bounds__(256) k_fill_cells(const __grid_constant__ Params P, Particles cur) {
+  const unsigned n = P.st->n;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    cur.cell[i] = cell_of(P, cur.x[i]);
+}
+int launch_fill_cells(const Params& P, const Particles& cur, cudaStream_t s) {
+  k_fill_cells<<<148 * 8, 256, 0, s>>>(P, cur);
+  return 1;
+}
+
 int launch_moments(const Params& P, const Particles& cur, double* partial, double* out, cudaStream_t s) {
   k_moments_partial<<<kMomBlocks, 256, 0, s>>>(P, cur, partial);
   k_moments_final<<<1, 1024, 0, s>>>(P, partial, kMomBlocks, out);
@@ -348,7 +404,7 @@ __global__ void __launch_bounds__(256) k_export_count(const __grid_constant__ Pa
       const unsigned i = ch * kExpChunk + r * 256 + threadIdx.x;
       const bool hit = i < n && cur.sp[i] == (unsigned char)species;
       // neighbours mostly share the cell: one atomic per run of the warp
-      const unsigned key = hit ? (unsigned)cur.cell[i] : 0xffffffffu - (threadIdx.x & 31);
+      const unsigned key = hit ? (unsigned)cell_of(P, cur.x[i]) : 0xffffffffu - (threadIdx.x & 31);
       const unsigned m = __match_any_sync(0xffffffffu, key);
       if (hit) {
         mine++;

@@ -3,11 +3,22 @@
 #include "common.cuh"
 
 namespace bit1 {
+// sets DevState::load_error when a position is outside [0, L) or a species tag is unknown (load) / additionally when
+// the positions are not in cell order (restart)
+int launch_load_validate(const Params& P, const Particles& in, unsigned n, cudaStream_t s);
+int launch_state_validate(const Params& P, const Particles& p, unsigned n, cudaStream_t s);
 // validate + cell index + general stable sort by cell of `in` (n particles) into `out`
 // before_gather: NULL, or an event the final gather waits for (arrays other than x, sp, pid still being copied)
 int launch_load_sort(const Params& P, const Particles& in, const Particles& out, unsigned n, int have_pid,
                      void* scratch, cudaStream_t s, cudaEvent_t before_gather);
 size_t load_scratch_bytes(unsigned capacity);
+// exclusive scan of n words in place (tmp: n / 4096 + 2 words)
+int launch_scan_u32(unsigned* a, size_t n, unsigned* tmp, cudaStream_t s);
+// stable radix sort of n (key, value) word pairs laid out as load_scratch_bytes(stride) describes
+int launch_radix_sort_u32(unsigned n, unsigned stride, int bits, void* scratch, cudaStream_t s, unsigned** keys,
+                          unsigned** vals);
+// cell[i] = cell_of(x[i]) for the live particles
+int launch_fill_cells(const Params& P, const Particles& cur, cudaStream_t s);
 // out: [kMaxSpecies*3] = (count, sum v^2, sum vx) per species, then sum g_j E_j^2
 int launch_moments(const Params& P, const Particles& cur, double* partial, double* out, cudaStream_t s);
 size_t moments_scratch_bytes();

@@ -28,13 +28,13 @@ constexpr int kWCap = BIT1_WCAP;          // max cells in a tile's window (smem 
 constexpr int kWarps = kThreads / 32;
 static_assert(kWCap <= kThreads && (32 % kWarps == 0 || kWarps % 32 == 0), "pass geometry");
 
-// overflow ("far mover" / birth) key: cell(28) | cls(2) | ord(34)
-constexpr int kOrdBits = 34;
-constexpr int kClsShift = kOrdBits;
-constexpr int kCellShift = kOrdBits + 2;
+// side-list ("far mover" / birth) key: cell | cls(2) | ord(Params::ord_bits), packed so that the radix sort of a long
+// list only visits the bits in use (Params::key_bits)
 constexpr unsigned long long kInvalidKey = ~0ull;
+// sort-window radius: adaptive per step (DevState::R_cur) up to Params::R_max <= kMaxR
+constexpr int kMaxR = (BIT1_WCAP - 8) / 2;
 
-constexpr unsigned kFlagCapacity = 1u, kFlagEscape = 2u, kFlagOverflow = 4u;
+constexpr unsigned kFlagCapacity = 1u, kFlagEscape = 2u, kFlagPidWrap = 8u;
 constexpr unsigned kElastic = 1u, kIonise = 2u, kCx = 4u, kIonProduct = 8u, kElectronProduct = 16u,
                    kTargetMaxwellian = 32u;
 constexpr int kSrcNone = 0, kSrcSelf = 1, kSrcPair = 2;
@@ -78,6 +78,16 @@ struct DevState {
   unsigned freeze_field;
   unsigned load_error;
   unsigned ovf_valid; // side-list entries that k_mid placed (ovf_count minus dropped births)
+  // sort window (reading R-win): radius of this step, radius chosen for the next one
+  unsigned R_cur, R_next;
+  // 1: this step's side list did not fit (ovf_count > ovf_cap).  Nothing of the step is committed and every later
+  // kernel returns at once until the host has taken the step through the general path (api.cu settle())
+  unsigned stalled;
+  unsigned pad0_;
+  // excess[e]: particles whose new cell lies e cells outside their tile's old cell range (e >= 2; the last bin holds
+  // everything beyond kMaxR); filled by pass A, read and cleared by k_mid when it chooses R_next
+  unsigned long long excess[kMaxR + 2];
+  unsigned long long general_steps;   // steps that took the general path
   unsigned long long wall_count[2][kMaxSpecies];
   long long wall_charge[2];
   unsigned long long nu_overflow, dir_fallback, escape, births, reinject, recycled;
@@ -92,12 +102,14 @@ struct DevState {
 
 struct Params {
   int nc, bc, ng, ns;
-  int R;         // window radius in cells
+  int R_max;     // upper bound of the adaptive window radius (rows of the banded arrays are sized for it)
+  int R_fixed;   // >= 0: the radius is pinned to this value (tests); -1: adaptive
+  int ord_bits, cell_shift, key_bits;   // side-list key: cell << cell_shift | cls << ord_bits | ord
   int n_sig, n_norm;
   int sp_ep, sp_ip;
   int dep_u32;   // 1: every Q_s * kTile < 2^32, shared-memory deposit counters may be 32-bit
   unsigned seed_lo, seed_hi;
-  unsigned capacity, ovf_cap, ovf_pow2;
+  unsigned capacity, ovf_cap;
   int max_tiles;
   double inv_dx, L, dt, dx, area;
   double src_lo, src_span;
@@ -126,6 +138,8 @@ struct Params {
   void *coop_scratch;  // k_field: per-CTA partial sums (16-byte aligned)
   int *cell_base;   // nc: cell_start + far movers placed before the windowed particles
   int *ovf_before;  // nc
+  int *ovf_lb, *ovf_ub;  // nc: first / one-past-last sorted side-list position of a cell's group (long lists)
+  unsigned *radix_hist;  // 256 * (CTAs of k_mid): digit counts of the grid-wide radix sort
   // tiles
   unsigned *tile_hist;  // banded histogram rows: row t (one count per window cell) at tile_row_offset(clo_t, t, R)
   int *tile_base;       // same layout: destination of the tile's first particle of each window cell
@@ -133,12 +147,13 @@ struct Params {
                         // tile's particles for that cell held by earlier warps of the tile
   unsigned *evt;        // one bit per particle slot: pass B must take the slow path (wall hit / MC candidate)
   // overflow list
-  unsigned long long *ovf_key;  // ovf_pow2 (unsorted, then sorted in place)
-  unsigned *ovf_idx;            // ovf_pow2: record index of sorted position
-  OvfRec *ovf_rec;              // ovf_cap
-  int *ovf_dst;                 // ovf_pow2: destination slot of sorted position (-1: dropped)
-  unsigned long long *tmp_key;  // ovf_pow2 scratch (birth ordering)
-  unsigned *tmp_idx;            // ovf_pow2 scratch
+  // side list (far movers and births of the step), ovf_cap entries each
+  unsigned long long *ovf_key;  // unsorted, then sorted in place
+  unsigned *ovf_idx;            // record index of sorted position
+  OvfRec *ovf_rec;
+  int *ovf_dst;                 // destination slot of sorted position
+  unsigned long long *tmp_key, *tmp2_key;  // scratch: birth ordering, radix ping-pong
+  unsigned *tmp_idx, *tmp2_idx;
   SpeciesP sp[kMaxSpecies];
 };
 

@@ -1,5 +1,5 @@
-// Tile staging for the two particle passes: one tile (kTile particles, all seven SoA arrays, its event bits and
-// its window of E) is brought into shared memory by 1D bulk-async copies (TMA, SASS UBLKCP) that complete on an
+// Tile staging for the two particle passes: one tile (kTile particles: x, v, pid, species -- the cell index is
+// cell_of(x) by construction and is not fetched --, its event bits and its window of E) is brought into shared memory by 1D bulk-async copies (TMA, SASS UBLKCP) that complete on an
 // mbarrier, two stages deep, so that the next tile's 41 B x kTile are in flight while the current tile is computed.
 // bytes in flight per SM are decoupled from registers and occupancy.
 #pragma once
@@ -9,7 +9,6 @@ namespace bit1 {
 
 struct __align__(128) Stage {
   double x[kTile], vx[kTile], vy[kTile], vz[kTile];
-  int cell[kTile];
   unsigned pid[kTile];
   unsigned char sp[kTile];
   unsigned evt[kTile / 32];
@@ -58,23 +57,35 @@ __device__ __forceinline__ bool e_window(int clo, int chi, int& e0, int& ne) {
   return ne <= kWCap + 4;
 }
 
+// The sort window of a tile whose old cells are [clo, chi]: cells [wlo, wlo + W) with W <= kWCap.  The radius is the
+// step's R (DevState::R_cur), cut down symmetrically for tiles so sparse that the window would not fit.  Pass A,
+// k_mid and pass B all derive a tile's window through this one function.
+struct TileWin {
+  int clo, chi, wlo, W;
+};
+__device__ __forceinline__ TileWin make_window(int clo, int chi, int R) {
+  TileWin t;
+  const int span = chi - clo + 1;
+  if (span + 2 * R > kWCap) R = span < kWCap ? (kWCap - span) >> 1 : 0;
+  t.clo = clo; t.chi = chi; t.wlo = clo - R;
+  const int w = span + 2 * R;
+  t.W = w < kWCap ? w : kWCap;
+  return t;
+}
+
 // One elected thread: arm the stage's barrier and issue the copies of tile `tile` (always whole tiles: the
 // arrays are padded to a multiple of kTile, the tail of the last tile is never used).
 __device__ __forceinline__ void issue_tile(const Params& P, const Particles& cur, Stage* st, unsigned long long* bar,
-                                           int tile, int2 d, bool with_evt, bool with_E, bool with_rank,
-                                           bool with_cell) {
+                                           int tile, int2 d, int R, bool with_evt, bool with_E, bool with_rank) {
   const size_t base = (size_t)tile * kTile;
   int e0 = 0, ne = 0;
   const bool stage_E = with_E && e_window(d.x, d.y, e0, ne);
-  // the cell array is not fetched on the V2 path: cell == cell_of(x) by construction (load, pass B, side list)
   unsigned bytes = 4u * kTile * 8u + kTile * 4u + kTile;
-  if (with_cell) bytes += kTile * 4u;
   if (with_evt) bytes += kTile / 8;
   if (stage_E) bytes += (unsigned)ne * 8u;
   // window of the tile, rounded up to whole 16-byte units (the rows are padded, see tile_row_offset)
-  int w = d.y - d.x + 1 + 2 * P.R;
-  w = ((w < kWCap ? w : kWCap) + 3) & ~3;
-  const size_t row = tile_row_offset(d.x, tile, P.R);
+  const int w = (make_window(d.x, d.y, R).W + 3) & ~3;
+  const size_t row = tile_row_offset(d.x, tile, R);
   if (with_rank) bytes += (unsigned)w * 4u * (1u + (unsigned)kWarps);
   st->d = d;
   mbar_expect_tx(bar, bytes);
@@ -82,7 +93,6 @@ __device__ __forceinline__ void issue_tile(const Params& P, const Particles& cur
   bulk_g2s(st->vx, cur.vx + base, kTile * 8, bar);
   bulk_g2s(st->vy, cur.vy + base, kTile * 8, bar);
   bulk_g2s(st->vz, cur.vz + base, kTile * 8, bar);
-  if (with_cell) bulk_g2s(st->cell, cur.cell + base, kTile * 4, bar);
   bulk_g2s(st->pid, cur.pid + base, kTile * 4, bar);
   bulk_g2s(st->sp, cur.sp + base, kTile, bar);
   if (with_evt) bulk_g2s(st->evt, P.evt + base / 32, kTile / 8, bar);

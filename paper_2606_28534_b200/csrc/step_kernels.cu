@@ -7,7 +7,8 @@
 //              deposition fused                                    (rows a4-a5; PAPER.md:111 arrj/narrj)
 //   k_field    exact integer-scan Poisson solve -> phi, E          (row a6; PAPER.md:33 step (iii))
 // Both particle passes are persistent (kMinBlocks CTAs per SM) and read their tiles through the two-stage
-// bulk-async pipeline of pipeline.cuh.
+// bulk-async pipeline of pipeline.cuh.  The store's cell array is not touched by a step (cell == cell_of(x)); a step
+// whose side list does not fit stalls (DevState::stalled) and is taken by general_kernels.cu instead.
 #include <cooperative_groups.h>
 
 #include "advance.cuh"
@@ -18,18 +19,6 @@ namespace cg = cooperative_groups;
 namespace bit1 {
 
 // ---------------------------------------------------------------------------------------------
-// tile geometry shared by both passes
-struct TileWin {
-  int clo, chi, wlo, W;
-};
-__device__ __forceinline__ TileWin make_window(int clo, int chi, int R) {
-  TileWin t;
-  t.clo = clo; t.chi = chi; t.wlo = clo - R;
-  const int w = chi - clo + 1 + 2 * R;
-  t.W = w < kWCap ? w : kWCap;
-  return t;
-}
-
 __device__ __forceinline__ void load_species(const Params& P, SpeciesP* s_sp) {
   const int words = P.ns * (int)(sizeof(SpeciesP) / 8);
   const unsigned long long* src = reinterpret_cast<const unsigned long long*>(P.sp);
@@ -46,7 +35,8 @@ struct PassSmem {
   static constexpr size_t a_hist = stages;                                  // unsigned[2][kWCap][kWarps]
   static constexpr size_t a_sp = a_hist + 2 * (size_t)kWCap * kWarps * 4;   // SpeciesP[kMaxSpecies]
   static constexpr size_t a_bar = (a_sp + kMaxSpecies * sizeof(SpeciesP) + 15) & ~(size_t)15;  // 2 x u64
-  static constexpr size_t a_total = a_bar + 16;
+  static constexpr size_t a_exc = a_bar + 16;                               // unsigned[kMaxR + 2]
+  static constexpr size_t a_total = a_exc + (((size_t)(kMaxR + 2) * 4 + 15) & ~(size_t)15);
   static constexpr size_t b_wc = stages;                                    // unsigned[kWarps][kWCap]
   static constexpr size_t b_dens = b_wc + (size_t)kWCap * kWarps * 4;       // unsigned[2][kWCap + 1][kMaxSpecies]
   static constexpr size_t b_sp = b_dens + 2 * (size_t)kDensWords * 4;
@@ -54,12 +44,13 @@ struct PassSmem {
   static constexpr size_t b_total = b_bar + 16;
 };
 
-// (cell of the first particle, cell of the last particle) of tile t, read from the sorted cell array itself
-__device__ __forceinline__ int2 tile_cells(const Particles& cur, int t, unsigned n) {
+// (cell of the first particle, cell of the last particle) of tile t: the array is sorted by cell and
+// cell == cell_of(x) by construction (load, pass B, side list), so two positions tell
+__device__ __forceinline__ int2 tile_cells(const Params& P, const Particles& cur, int t, unsigned n) {
   const size_t first = (size_t)t * kTile;
   const size_t end = first + kTile;
   const size_t last = (end < (size_t)n ? end : (size_t)n) - 1;
-  return make_int2(cur.cell[first], cur.cell[last]);
+  return make_int2(cell_of(P, cur.x[first]), cell_of(P, cur.x[last]));
 }
 
 // first 52 bits of the two-word uniform of slot C0 as an integer: u52(a, b) = (w + 0.5) * 2^-52
@@ -68,23 +59,25 @@ __device__ __forceinline__ unsigned long long w52(unsigned a, unsigned b) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// Pass A.  VARIANT 1 writes the advanced state back in place; VARIANT 2 writes one event bit per particle.
+// Pass A writes nothing into the particle store: counts, one event bit per particle, the side list.
 // Per tile: phase 1 is straight-line arithmetic over the thread's kItems particles (no warp-wide operation in
 // it, so the compiler interleaves the independent dependency chains); phase 2 redoes the rare particles (wall
 // hit, periodic wrap, null-collision candidate, move beyond the window) through the full advance(); phase 3
 // builds the banded histogram.  One CTA barrier per tile: the histogram is double-buffered.
-template <int VARIANT>
 __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_constant__ Params P, Particles cur) {
   constexpr int kWarpSpan = 32 * kItems;
+  if (P.st->stalled) return;
   typedef PassSmem SM;
   extern __shared__ __align__(128) unsigned char smem[];
   Stage* stg = reinterpret_cast<Stage*>(smem);
   unsigned* s_hist2 = reinterpret_cast<unsigned*>(smem + SM::a_hist);
   SpeciesP* s_sp = reinterpret_cast<SpeciesP*>(smem + SM::a_sp);
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem + SM::a_bar);
+  unsigned* s_exc = reinterpret_cast<unsigned*>(smem + SM::a_exc);
 
   const unsigned n = P.st->n;
   const unsigned long long step = P.st->step;
+  const int R = (int)P.st->R_cur;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int ntiles = (int)((n + kTile - 1) / kTile);
   const int G = gridDim.x;
@@ -96,11 +89,12 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
     fence_proxy_async();
     for (int k = 0; k < 2; ++k) {
       const int t = blockIdx.x + k * G;
-      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, tile_cells(cur, t, n), false, true, false, false);
+      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, tile_cells(P, cur, t, n), R, false, true, false);
     }
   }
   load_species(P, s_sp);
   for (int k = threadIdx.x; k < 2 * kWCap * kWarps; k += kThreads) s_hist2[k] = 0;
+  if (threadIdx.x < kMaxR + 2) s_exc[threadIdx.x] = 0;
   // the deposition of this step accumulates into dens: clear it here (nobody reads it during pass A)
   {
     const size_t tot = (size_t)P.ns * (size_t)P.ng;
@@ -117,12 +111,12 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
     // cells of the tile after next (its load is issued at the end of this iteration)
     int2 dn = make_int2(0, 0);
     const int tnext = tile + 2 * G;
-    if (threadIdx.x == 0 && tnext < ntiles) dn = tile_cells(cur, tnext, n);
+    if (threadIdx.x == 0 && tnext < ntiles) dn = tile_cells(P, cur, tnext, n);
     mbar_wait(&bar[it & 1], (unsigned)(it >> 1) & 1u);
 
     const int clo = S->d.x, chi = S->d.y;
     if (threadIdx.x == 0) cur.desc[tile] = S->d;   // read by k_mid's column scan and by pass B's issuing thread
-    const TileWin tw = make_window(clo, chi, P.R);
+    const TileWin tw = make_window(clo, chi, R);
     int e0, ne;
     const double* Eptr = e_window(clo, chi, e0, ne) ? (S->E - e0) : P.E;
 
@@ -142,11 +136,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
       const bool inside = push_fast(P, s, Eptr, c, x[r], vx[r], vy[r], vz[r]);
       cn[r] = cell_of(P, x[r]);
       const int k = cn[r] - tw.wlo;
-#ifdef BIT1_EXPERIMENT_NOPUSH
-      thr[r] = 0ull;
-#else
       thr[r] = have ? s.pthr : 0ull;
-#endif
       if (have && !(inside && k >= 0 && k < tw.W)) evm |= 1u << r;
     }
     unsigned long long any = 0;
@@ -167,15 +157,15 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
         if ((evm >> r) & 1u) {
           const int off = warp * kWarpSpan + r * 32 + lane;
           const unsigned i = base + (unsigned)off;
-          const int c = slow_advance<true>(P, s_sp, step, Eptr, S, off, i);
+          const int c = slow_advance<SinkList>(P, s_sp, step, Eptr, S, off, i);
           cn[r] = c;
-          if (VARIANT == 1) { x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off]; }
           if (c >= 0) {
             const int k = c - tw.wlo;
             if (!(k >= 0 && k < tw.W)) {
-              emit_record(P, make_key(c, c < tw.wlo ? 1u : 0u, (unsigned long long)i), S->x[off], S->vx[off],
+              emit_record(P, make_key(P, c, c < tw.wlo ? 1u : 0u, (unsigned long long)i), S->x[off], S->vx[off],
                           S->vy[off], S->vz[off], S->pid[off], (int)S->sp[off]);
               cn[r] = -2;  // placed through the side list
+              atomicAdd(&s_exc[min(max(clo - c, c - chi), kMaxR + 1)], 1u);   // see phase 3
             }
           }
         }
@@ -187,15 +177,14 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
       const int off = warp * kWarpSpan + r * 32 + lane;
       const bool have = (unsigned)off < cnt;
       unsigned key = 0x80000000u | (unsigned)lane;  // unique: matches nobody
-      if (have) {
-        if (VARIANT == 1) {
-          const unsigned i = base + (unsigned)off;
-          cur.x[i] = x[r]; cur.vx[i] = vx[r]; cur.vy[i] = vy[r]; cur.vz[i] = vz[r];
-          cur.cell[i] = cn[r] == -2 ? -1 : cn[r];   // side-list particles are not placed by pass B's tile loop
-        }
-        if (cn[r] >= 0) key = (unsigned)(cn[r] - tw.wlo);
+      if (have && cn[r] >= 0) {
+        key = (unsigned)(cn[r] - tw.wlo);
+        // how far outside the tile's old cell range the particle lands: k_mid picks the next step's radius from
+        // these counts (never taken at radius 1: a windowed particle is then at most one cell outside)
+        const int ex = max(clo - cn[r], cn[r] - chi);
+        if (ex >= 2) atomicAdd(&s_exc[min(ex, kMaxR + 1)], 1u);
       }
-      if (VARIANT == 2) {
+      {
         const unsigned eb = __ballot_sync(0xffffffffu, (evm >> r) & 1u);
         if (lane == 0) P.evt[(base >> 5) + (unsigned)(warp * kItems + r)] = eb;
       }
@@ -207,7 +196,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
     __syncthreads();
     // per window cell: the warps' counts become exclusive prefixes (tile_pre, read back by pass B: this warp's
     // particles for that cell start that far into the tile's run), their sum is the tile's count
-    const size_t rowo = tile_row_offset(clo, tile, P.R);
+    const size_t rowo = tile_row_offset(clo, tile, R);
     for (int k = threadIdx.x; k < tw.W; k += kThreads) {
       unsigned run = 0;
       unsigned* pre = P.tile_pre + (rowo + (size_t)k) * kWarps;
@@ -222,14 +211,23 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
       const int c = tw.wlo + k;
       if (run && c >= 0 && c < P.nc) atomicAdd(&P.cell_count[c], (int)run);
     }
-    if (threadIdx.x == 0 && tnext < ntiles) issue_tile(P, cur, S, &bar[it & 1], tnext, dn, false, true, false, false);
+    if (threadIdx.x == 0 && tnext < ntiles) issue_tile(P, cur, S, &bar[it & 1], tnext, dn, R, false, true, false);
+  }
+  __syncthreads();
+  if (threadIdx.x < kMaxR + 2) {
+    const unsigned v = s_exc[threadIdx.x];
+    if (v) atomicAdd(&P.st->excess[threadIdx.x], (unsigned long long)v);
   }
 }
 
 // ---------------------------------------------------------------------------------------------
-// k_mid helpers: CTA-wide and grid-wide sorts, block scans.
+// k_mid helpers: sorts of the side list (CTA-wide bitonic in shared memory for short lists, radix over the whole
+// cooperative grid for long ones), block scans.
 constexpr int kMidThreads = 1024;
+constexpr int kMidWarps = kMidThreads / 32;
 constexpr int kSortSmem = 2048;
+constexpr int kMidRaw = 256 * kMidWarps * 4;   // bytes: radix counters [digit][warp]; the bitonic sort's keys + values alias them
+static_assert(kSortSmem * 12 <= kMidRaw, "k_mid shared memory");
 
 __device__ void cta_bitonic(unsigned long long* key, unsigned* val, unsigned n) {
   for (unsigned k = 2; k <= n; k <<= 1) {
@@ -265,87 +263,26 @@ __device__ __forceinline__ unsigned lower_bound_u64(const unsigned long long* a,
   return lo;
 }
 
-// sort (key, val) pairs of length P2 (power of two, padded with kInvalidKey) held in global memory
-__device__ void cta_sort(unsigned long long* gkey, unsigned* gval, unsigned P2, unsigned long long* s_key,
+// sort n <= kSortSmem (key, val) pairs held in global memory by one CTA; the sorted pairs stay in s_key / s_val
+// (padded with kInvalidKey up to the next power of two) for the caller's binary searches
+__device__ void cta_sort(unsigned long long* gkey, unsigned* gval, unsigned n, unsigned long long* s_key,
                          unsigned* s_val) {
-  if (P2 <= (unsigned)kSortSmem) {
-    for (unsigned i = threadIdx.x; i < P2; i += blockDim.x) { s_key[i] = gkey[i]; s_val[i] = gval[i]; }
-    __syncthreads();
-    cta_bitonic(s_key, s_val, P2);
-    for (unsigned i = threadIdx.x; i < P2; i += blockDim.x) { gkey[i] = s_key[i]; gval[i] = s_val[i]; }
-    __syncthreads();
-  } else {
-    __syncthreads();
-    cta_bitonic(gkey, gval, P2);  // robustness path: global memory, one CTA
+  const unsigned P2 = next_pow2(n > 1 ? n : 1);
+  for (unsigned i = threadIdx.x; i < P2; i += blockDim.x) {
+    s_key[i] = i < n ? gkey[i] : kInvalidKey;
+    s_val[i] = i < n ? gval[i] : 0u;
   }
-}
-
-// Side lists too long for one CTA's shared memory (a degenerate input: most particles leave their tile's window):
-// bitonic sort over the whole cooperative grid.  Chunks of kSortSmem elements are sorted in shared memory; the
-// exchanges at distance >= kSortSmem run in global memory with one grid barrier each.  The direction of a compare
-// is taken from the global index, so the network is the same as cta_bitonic's.
-__device__ void chunk_steps(unsigned long long* gkey, unsigned* gval, unsigned base, unsigned k_lo, unsigned k_hi,
-                            unsigned long long* s_key, unsigned* s_val) {
-  for (unsigned i = threadIdx.x; i < (unsigned)kSortSmem; i += blockDim.x) { s_key[i] = gkey[base + i]; s_val[i] = gval[base + i]; }
   __syncthreads();
-  for (unsigned k = k_lo; k <= k_hi; k <<= 1) {
-    unsigned j = k >> 1;
-    if (j > (unsigned)kSortSmem / 2) j = (unsigned)kSortSmem / 2;
-    for (; j > 0; j >>= 1) {
-      for (unsigned i = threadIdx.x; i < (unsigned)kSortSmem; i += blockDim.x) {
-        const unsigned ixj = i ^ j;
-        if (ixj > i) {
-          const unsigned long long a = s_key[i], b = s_key[ixj];
-          const bool asc = ((base + i) & k) == 0;
-          if ((a > b) == asc) {
-            s_key[i] = b; s_key[ixj] = a;
-            const unsigned t = s_val[i]; s_val[i] = s_val[ixj]; s_val[ixj] = t;
-          }
-        }
-      }
-      __syncthreads();
-    }
-  }
-  for (unsigned i = threadIdx.x; i < (unsigned)kSortSmem; i += blockDim.x) { gkey[base + i] = s_key[i]; gval[base + i] = s_val[i]; }
+  cta_bitonic(s_key, s_val, P2);
+  for (unsigned i = threadIdx.x; i < n; i += blockDim.x) { gkey[i] = s_key[i]; gval[i] = s_val[i]; }
   __syncthreads();
-}
-
-__device__ void grid_bitonic(cg::grid_group& grid, unsigned long long* gkey, unsigned* gval, unsigned P2,
-                             unsigned long long* s_key, unsigned* s_val) {
-  const unsigned nchunk = P2 / (unsigned)kSortSmem;   // P2 > kSortSmem, both powers of two
-  for (unsigned c = blockIdx.x; c < nchunk; c += gridDim.x)
-    chunk_steps(gkey, gval, c * (unsigned)kSortSmem, 2u, (unsigned)kSortSmem, s_key, s_val);
-  __threadfence();
-  grid.sync();
-  const size_t gtid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, gsz = (size_t)gridDim.x * blockDim.x;
-  for (unsigned k = 2u * (unsigned)kSortSmem; k <= P2 && k != 0; k <<= 1) {
-    for (unsigned j = k >> 1; j >= (unsigned)kSortSmem; j >>= 1) {
-      for (size_t i = gtid; i < (size_t)P2; i += gsz) {
-        const size_t ixj = i ^ (size_t)j;
-        if (ixj > i) {
-          const unsigned long long a = gkey[i], b = gkey[ixj];
-          const bool asc = (i & (size_t)k) == 0;
-          if ((a > b) == asc) {
-            gkey[i] = b; gkey[ixj] = a;
-            const unsigned t = gval[i]; gval[i] = gval[ixj]; gval[ixj] = t;
-          }
-        }
-      }
-      __threadfence();
-      grid.sync();
-    }
-    for (unsigned c = blockIdx.x; c < nchunk; c += gridDim.x)
-      chunk_steps(gkey, gval, c * (unsigned)kSortSmem, k, k, s_key, s_val);
-    __threadfence();
-    grid.sync();
-  }
 }
 
 // One-CTA cooperative grids (small workloads) need no grid-wide barrier: a CTA barrier orders the block's own global
 // writes for its own threads, and saves the round trip through the barrier word in global memory.
 __device__ __forceinline__ void grid_or_cta_sync(cg::grid_group& grid) {
   if (gridDim.x == 1) __syncthreads();
-  else grid.sync();
+  else { __threadfence(); grid.sync(); }
 }
 
 __device__ int block_exclusive_scan_int(int v, int* s_warp, int* total) {
@@ -396,50 +333,148 @@ __device__ int block_sum_int(int v, int* s_warp) {
   return t;
 }
 
+// Stable LSD radix sort (8-bit digits over key bits [0, nbits)) of n (key, val) pairs over the whole cooperative
+// grid; (k1, v1) is scratch of the same size; the result ends in (k0, v0).  Side lists of 1e5..1e7 entries (a hot
+// tail, a sheath start-up, a pinned small radius) cost a few passes over 12 B per entry instead of the
+// O(n log^2 n) exchanges and grid barriers of a bitonic network.  Every CTA owns a contiguous chunk of the array and
+// every warp a contiguous segment of the chunk, so "stable" is "in warp-segment order": per pass (a) per-(digit,
+// warp) counts, (b) after a grid barrier every CTA derives the start of each of its (digit, warp) runs from all
+// CTAs' digit totals, (c) the warps walk their segments again and scatter.
+__device__ void grid_radix_sort(cg::grid_group& grid, const Params& P, unsigned long long* k0, unsigned* v0,
+                                unsigned long long* k1, unsigned* v1, unsigned n, int nbits, unsigned* s_cnt,
+                                int* s_warp) {
+  const int G = gridDim.x, b = blockIdx.x;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned lt = (1u << lane) - 1u;
+  unsigned per = (n + (unsigned)G - 1u) / (unsigned)G;
+  per = (per + (unsigned)kMidThreads - 1u) & ~((unsigned)kMidThreads - 1u);      // whole 32-element rows per warp
+  const unsigned lo = min((unsigned)b * per, n), hi = min(lo + per, n);
+  const unsigned seg = per / (unsigned)kMidWarps;
+  const unsigned w_lo = min(lo + (unsigned)warp * seg, hi), w_hi = min(w_lo + seg, hi);
+  unsigned* ghist = P.radix_hist;   // [256][G]
+  int pass = 0;
+  for (int shift = 0; shift < nbits; shift += 8, ++pass) {
+    for (int k = threadIdx.x; k < 256 * kMidWarps; k += kMidThreads) s_cnt[k] = 0;
+    __syncthreads();
+    for (unsigned i0 = w_lo; i0 < w_hi; i0 += 32) {
+      const unsigned i = i0 + (unsigned)lane;
+      const unsigned d = i < w_hi ? (unsigned)((k0[i] >> shift) & 255ull) : (0x80000000u | (unsigned)lane);
+      const unsigned m = __match_any_sync(0xffffffffu, d);
+      if (i < w_hi && lane == __ffs(m) - 1) s_cnt[d * kMidWarps + warp] += (unsigned)__popc(m);
+      __syncwarp();
+    }
+    __syncthreads();
+    if (threadIdx.x < 256) {
+      unsigned t = 0;
+      for (int w = 0; w < kMidWarps; ++w) t += s_cnt[threadIdx.x * kMidWarps + w];
+      ghist[(size_t)threadIdx.x * G + b] = t;
+    }
+    grid_or_cta_sync(grid);
+    int tot = 0, mine = 0;
+    if (threadIdx.x < 256) {
+      for (int bb = 0; bb < G; ++bb) {
+        const int v = (int)ghist[(size_t)threadIdx.x * G + bb];
+        tot += v;
+        if (bb < b) mine += v;
+      }
+    }
+    int dummy;
+    const int ex = block_exclusive_scan_int(tot, s_warp, &dummy);   // entries with a smaller digit, all CTAs
+    if (threadIdx.x < 256) {
+      unsigned run = (unsigned)(ex + mine);
+      for (int w = 0; w < kMidWarps; ++w) {
+        const unsigned t = s_cnt[threadIdx.x * kMidWarps + w];
+        s_cnt[threadIdx.x * kMidWarps + w] = run;
+        run += t;
+      }
+    }
+    __syncthreads();
+    for (unsigned i0 = w_lo; i0 < w_hi; i0 += 32) {
+      const unsigned i = i0 + (unsigned)lane;
+      const bool have = i < w_hi;
+      const unsigned long long key = have ? k0[i] : 0ull;
+      const unsigned val = have ? v0[i] : 0u;
+      const unsigned d = have ? (unsigned)((key >> shift) & 255ull) : (0x80000000u | (unsigned)lane);
+      const unsigned m = __match_any_sync(0xffffffffu, d);
+      const int leader = __ffs(m) - 1;
+      unsigned old = 0;
+      if (have && lane == leader) {
+        old = s_cnt[d * kMidWarps + warp];
+        s_cnt[d * kMidWarps + warp] = old + (unsigned)__popc(m);
+      }
+      old = __shfl_sync(0xffffffffu, old, leader);
+      if (have) {
+        const unsigned dst = old + (unsigned)__popc(m & lt);
+        k1[dst] = key;
+        v1[dst] = val;
+      }
+      __syncwarp();
+    }
+    grid_or_cta_sync(grid);
+    { unsigned long long* t = k0; k0 = k1; k1 = t; }
+    { unsigned* t = v0; v0 = v1; v1 = t; }
+  }
+  if (pass & 1) {   // the result sits in the scratch pair: bring it home (k0 / k1 have swapped names)
+    for (unsigned i = lo + threadIdx.x; i < hi; i += kMidThreads) { k1[i] = k0[i]; v1[i] = v0[i]; }
+    grid_or_cta_sync(grid);
+  }
+}
+
 // k_mid: cooperative launch, one CTA per SM at most.
-//   phase 0 (CTA 0)  side list: births get their pids, the list is ordered by (cell, class, order), every group
-//                    joins its cell's count
+//   phase 0          side list: births get their pids in (parent, kind) order, the list is ordered by (cell, class,
+//                    order), every cell's group joins the cell's count.  Short lists: CTA 0, in shared memory; long
+//                    lists: the whole grid (radix sort).  A list beyond its capacity stalls the step (see DevState).
 //   phase 1          exclusive scan of the cell counts over all CTAs -> cell_start, cell_base; counts zeroed
 //   phase 2          destinations of the side-list entries; banded column scan (do_colscan): one thread per cell
 //                    walks, in tile order, the tiles whose window holds the cell and hands each its destination
 //                    base = cell_base[c] + what the earlier tiles send to c.  Those tiles are the ones that hold
-//                    old cells c-R .. c+R, found from the previous step's cell_start.
+//                    old cells c-R .. c+R, found from the previous step's cell_start.  Last, the next step's window
+//                    radius is chosen from pass A's excess counts.
 __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Params P, Particles cur, int do_colscan) {
-  __shared__ unsigned long long s_key[kSortSmem];
-  __shared__ unsigned s_val[kSortSmem];
+  __shared__ __align__(16) unsigned char s_raw[kMidRaw];
   __shared__ int s_warp[33];
   __shared__ unsigned s_cnt;
+  unsigned long long* s_key = reinterpret_cast<unsigned long long*>(s_raw);
+  unsigned* s_val = reinterpret_cast<unsigned*>(s_raw + kSortSmem * 8);
+  unsigned* s_radix = reinterpret_cast<unsigned*>(s_raw);
   cg::grid_group grid = cg::this_grid();
   DevState* st = P.st;
+  if (st->stalled) return;
   const unsigned n = st->n;
   const int G = gridDim.x, b = blockIdx.x;
-  unsigned M = st->ovf_count;
-  if (M > P.ovf_cap) M = P.ovf_cap;
+  const unsigned M = st->ovf_count;
+  if (M > P.ovf_cap) {
+    // the side list did not fit: nothing of this step is committed (pass A has only counted); the host takes the
+    // step through the general path.  Every CTA sees the same count, so the whole grid leaves here.
+    if (b == 0 && threadIdx.x == 0) st->stalled = 1u;
+    return;
+  }
+  const unsigned long long ord_mask = (1ull << P.ord_bits) - 1ull;
+  const int cshift = P.cell_shift, oshift = P.ord_bits;
+  const size_t gt = (size_t)b * kMidThreads + threadIdx.x, gs = (size_t)G * kMidThreads;
 
-  const unsigned P2 = next_pow2(M > 1 ? M : 1);
-  const bool big = P2 > (unsigned)kSortSmem;   // uniform over the grid
+  const bool big = M > (unsigned)kSortSmem;   // uniform over the grid
   if (big) {
-    // the same three steps as below, spread over the grid (grid_bitonic); births are counted in scan_part[0]
-    const size_t gt = (size_t)b * kMidThreads + threadIdx.x, gs = (size_t)G * kMidThreads;
+    // (a) births, compacted into (tmp_key = order, tmp_idx = record), ordered, numbered
     if (gt == 0) P.scan_part[0] = 0;
-    __threadfence();
-    grid.sync();
-    unsigned nb_local = 0;
-    for (size_t i = gt; i < (size_t)P2; i += gs) {
-      unsigned long long bk = kInvalidKey;
-      if (i < M) {
-        const unsigned long long key = P.ovf_key[i];
-        if (((key >> kClsShift) & 3ull) == 2ull) { bk = key & ((1ull << kOrdBits) - 1ull); nb_local++; }
+    grid_or_cta_sync(grid);
+    for (size_t i = gt; i < (size_t)M; i += gs) {
+      const unsigned long long key = P.ovf_key[i];
+      if (((key >> oshift) & 3ull) == 2ull) {
+        const int j = atomicAdd(&P.scan_part[0], 1);
+        P.tmp_key[j] = key & ord_mask;
+        P.tmp_idx[j] = (unsigned)i;
       }
-      P.tmp_key[i] = bk;
-      P.tmp_idx[i] = (unsigned)i;
     }
-    if (nb_local) atomicAdd(&P.scan_part[0], (int)nb_local);
-    __threadfence();
-    grid.sync();
+    grid_or_cta_sync(grid);
     const unsigned B = (unsigned)P.scan_part[0];
     if (B > 0) {
-      grid_bitonic(grid, P.tmp_key, P.tmp_idx, P2, s_key, s_val);
+      if (B <= (unsigned)kSortSmem) {
+        if (b == 0) cta_sort(P.tmp_key, P.tmp_idx, B, s_key, s_val);
+        grid_or_cta_sync(grid);
+      } else {
+        grid_radix_sort(grid, P, P.tmp_key, P.tmp_idx, P.tmp2_key, P.tmp2_idx, B, P.ord_bits, s_radix, s_warp);
+      }
       const unsigned room = P.capacity > n ? P.capacity - n : 0u;
       const unsigned next_pid = st->next_pid;
       for (size_t r = gt; r < (size_t)B; r += gs) {
@@ -447,35 +482,45 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
         if (r < room) P.ovf_rec[rec].pid = next_pid + (unsigned)r;
         else P.ovf_key[rec] = kInvalidKey;
       }
-      __threadfence();
-      grid.sync();
+      grid_or_cta_sync(grid);
       if (gt == 0) {
         const unsigned created = B < room ? B : room;
+        if (next_pid + created < next_pid) st->flags |= kFlagPidWrap;
         st->next_pid = next_pid + created;
         st->births += created;
         if (B > room) st->flags |= kFlagCapacity;
       }
     }
-    for (size_t i = gt; i < (size_t)P2; i += gs) {
-      if (i >= M) P.ovf_key[i] = kInvalidKey;
-      P.ovf_idx[i] = (unsigned)i;
-    }
-    __threadfence();
-    grid.sync();
-    grid_bitonic(grid, P.ovf_key, P.ovf_idx, P2, s_key, s_val);
-    const unsigned Mv = lower_bound_u64(P.ovf_key, P2, kInvalidKey);
+    // (b) the whole list by (cell, class, order); dropped births (kInvalidKey) sort behind everything
+    for (size_t i = gt; i < (size_t)M; i += gs) P.ovf_idx[i] = (unsigned)i;
+    grid_or_cta_sync(grid);
+    grid_radix_sort(grid, P, P.ovf_key, P.ovf_idx, P.tmp_key, P.tmp_idx, M, P.key_bits, s_radix, s_warp);
+    const unsigned Mv = lower_bound_u64(P.ovf_key, M, kInvalidKey);
+    // (c) groups per cell: the first and last entry of every group publish its bounds ...
     for (size_t p = gt; p < (size_t)Mv; p += gs) {
       const unsigned long long key = P.ovf_key[p];
-      const unsigned long long c = key >> kCellShift;
-      const unsigned lb = lower_bound_u64(P.ovf_key, Mv, c << kCellShift);
-      const unsigned ub = lower_bound_u64(P.ovf_key, Mv, (c + 1ull) << kCellShift);
-      const unsigned cls = (unsigned)((key >> kClsShift) & 3ull);
-      if (p == lb) {
-        const unsigned ub0 = lower_bound_u64(P.ovf_key, Mv, (c << kCellShift) | (1ull << kClsShift));
-        P.cell_count[c] += (int)(ub - lb);
-        P.ovf_before[c] = (int)(ub0 - lb);
+      const unsigned long long c = key >> cshift;
+      const unsigned cls = (unsigned)((key >> oshift) & 3ull);
+      const bool first = p == 0 || (P.ovf_key[p - 1] >> cshift) != c;
+      unsigned long long nk = 0;
+      const bool last = p + 1 == (size_t)Mv || ((nk = P.ovf_key[p + 1]) >> cshift) != c;
+      if (first) P.ovf_lb[c] = (int)p;
+      if (last) P.ovf_ub[c] = (int)p + 1;
+      if (cls == 0 && (last || ((nk >> oshift) & 3ull) != 0ull)) P.ovf_before[c] = (int)p + 1;   // made relative below
+    }
+    grid_or_cta_sync(grid);
+    // ... then every entry takes its rank from them: class 0 counts from the cell's start, classes 1-2 from its end
+    for (size_t p = gt; p < (size_t)Mv; p += gs) {
+      const unsigned long long key = P.ovf_key[p];
+      const int c = (int)(key >> cshift);
+      const unsigned cls = (unsigned)((key >> oshift) & 3ull);
+      const int lb = P.ovf_lb[c], ub = P.ovf_ub[c];
+      if ((int)p == lb) {
+        P.cell_count[c] += ub - lb;
+        const int ub0 = P.ovf_before[c];
+        P.ovf_before[c] = ub0 > lb ? ub0 - lb : 0;   // class-0 entries open the group, so ub0 > lb iff there are any
       }
-      P.ovf_dst[p] = cls == 0 ? (int)(p - lb) : (int)(p - lb) - (int)(ub - lb);
+      P.ovf_dst[p] = cls == 0 ? (int)p - lb : (int)p - ub;
     }
     if (gt == 0) {
       st->ovf_valid = Mv;
@@ -486,59 +531,54 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
     unsigned Mv = 0;
     if (M > 0) {
       // (a) births: order by (parent index, kind), assign pid = next_pid + r, drop those beyond capacity
-      unsigned nb_local = 0;
-      for (unsigned i = threadIdx.x; i < P2; i += blockDim.x) {
-        unsigned long long bk = kInvalidKey;
-        if (i < M) {
-          const unsigned long long key = P.ovf_key[i];
-          if (((key >> kClsShift) & 3ull) == 2ull) { bk = key & ((1ull << kOrdBits) - 1ull); nb_local++; }
-        }
-        P.tmp_key[i] = bk;
-        P.tmp_idx[i] = i;
-      }
       if (threadIdx.x == 0) s_cnt = 0;
       __syncthreads();
-      if (nb_local) atomicAdd(&s_cnt, nb_local);
+      for (unsigned i = threadIdx.x; i < M; i += blockDim.x) {
+        const unsigned long long key = P.ovf_key[i];
+        if (((key >> oshift) & 3ull) == 2ull) {
+          const unsigned j = atomicAdd(&s_cnt, 1u);
+          P.tmp_key[j] = key & ord_mask;
+          P.tmp_idx[j] = i;
+        }
+      }
       __syncthreads();
       const unsigned B = s_cnt;
       __syncthreads();
       if (B > 0) {
-        cta_sort(P.tmp_key, P.tmp_idx, P2, s_key, s_val);
+        cta_sort(P.tmp_key, P.tmp_idx, B, s_key, s_val);
         const unsigned room = P.capacity > n ? P.capacity - n : 0u;
         const unsigned next_pid = st->next_pid;
         for (unsigned r = threadIdx.x; r < B; r += blockDim.x) {
-          const unsigned rec = P.tmp_idx[r];
+          const unsigned rec = s_val[r];
           if (r < room) P.ovf_rec[rec].pid = next_pid + r;
           else P.ovf_key[rec] = kInvalidKey;
         }
         __syncthreads();
         if (threadIdx.x == 0) {
           const unsigned created = B < room ? B : room;
+          if (next_pid + created < next_pid) st->flags |= kFlagPidWrap;
           st->next_pid = next_pid + created;
           st->births += created;
           if (B > room) st->flags |= kFlagCapacity;
         }
       }
       // (b) order the whole list by (cell, class, order)
-      for (unsigned i = threadIdx.x; i < P2; i += blockDim.x) {
-        if (i >= M) P.ovf_key[i] = kInvalidKey;
-        P.ovf_idx[i] = i;
-      }
+      for (unsigned i = threadIdx.x; i < M; i += blockDim.x) P.ovf_idx[i] = i;
       __syncthreads();
-      cta_sort(P.ovf_key, P.ovf_idx, P2, s_key, s_val);
-      // the sorted keys are still in shared memory (P2 <= kSortSmem here): the binary searches below are chains of
-      // dependent loads, a few dozen ns each there against most of a microsecond each in global memory
+      cta_sort(P.ovf_key, P.ovf_idx, M, s_key, s_val);
+      // the sorted keys are still in shared memory: the binary searches below are chains of dependent loads, a few
+      // dozen ns each there against most of a microsecond each in global memory
       const unsigned long long* K = s_key;
-      Mv = lower_bound_u64(K, P2, kInvalidKey);
+      Mv = lower_bound_u64(K, M, kInvalidKey);
       // (c) groups per cell: rank inside the group, group size joins the cell count
       for (unsigned p = threadIdx.x; p < Mv; p += blockDim.x) {
         const unsigned long long key = K[p];
-        const unsigned long long c = key >> kCellShift;
-        const unsigned lb = lower_bound_u64(K, Mv, c << kCellShift);
-        const unsigned ub = lower_bound_u64(K, Mv, (c + 1ull) << kCellShift);
-        const unsigned cls = (unsigned)((key >> kClsShift) & 3ull);
+        const unsigned long long c = key >> cshift;
+        const unsigned lb = lower_bound_u64(K, Mv, c << cshift);
+        const unsigned ub = lower_bound_u64(K, Mv, (c + 1ull) << cshift);
+        const unsigned cls = (unsigned)((key >> oshift) & 3ull);
         if (p == lb) {
-          const unsigned ub0 = lower_bound_u64(K, Mv, (c << kCellShift) | (1ull << kClsShift));
+          const unsigned ub0 = lower_bound_u64(K, Mv, (c << cshift) | (1ull << oshift));
           P.cell_count[c] += (int)(ub - lb);
           P.ovf_before[c] = (int)(ub0 - lb);
         }
@@ -552,7 +592,6 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
       if (M > st->max_far_movers) st->max_far_movers = M;
     }
   }
-  __threadfence();
   grid_or_cta_sync(grid);
 
   // phase 1: scan of the cell counts.  CTA b owns cells [c_lo, c_hi).
@@ -566,7 +605,6 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
     sum = block_sum_int(sum, s_warp);
     if (threadIdx.x == 0) P.scan_part[b] = sum;
   }
-  __threadfence();
   grid_or_cta_sync(grid);
   int carry, total;
   {
@@ -607,23 +645,21 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
     P.cell_start[nc] = total;
     st->n_next = (unsigned)total;
   }
-  __threadfence();
   grid_or_cta_sync(grid);
 
   // phase 2
   const unsigned Mv = st->ovf_valid;
-  const size_t gtid = (size_t)b * kMidThreads + threadIdx.x, gsz = (size_t)G * kMidThreads;
-  for (size_t p = gtid; p < Mv; p += gsz) {
+  for (size_t p = gt; p < Mv; p += gs) {
     const unsigned long long key = P.ovf_key[p];
-    const int c = (int)(key >> kCellShift);
-    const unsigned cls = (unsigned)((key >> kClsShift) & 3ull);
+    const int c = (int)(key >> cshift);
+    const unsigned cls = (unsigned)((key >> oshift) & 3ull);
     const int rel = P.ovf_dst[p];
     P.ovf_dst[p] = (cls == 0 ? P.cell_start[c] : P.cell_start[c + 1]) + rel;
   }
   if (do_colscan && n > 0) {
-    const int R = P.R;
+    const int R = (int)st->R_cur;
     const int* cso = P.cell_start_old;
-    for (size_t cc = gtid; cc < (size_t)nc; cc += gsz) {
+    for (size_t cc = gt; cc < (size_t)nc; cc += gs) {
       const int c = (int)cc;
       const int lo = cso[max(c - R, 0)];              // first old particle with cell >= c - R
       const int hi = cso[min(c + R + 1, nc)] - 1;     // last old particle with cell <= c + R
@@ -657,6 +693,28 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
       }
     }
   }
+  // the next step's window radius (reading R-win): the smallest radius that leaves no more than one far mover per
+  // four tiles among the particles that stay inside the domain -- a wider window costs every tile two more row
+  // entries per cell of radius, a far mover costs a side-list record, a sort key and a scattered placement
+  if (gt == 0) {
+    int Rn = 1;
+    if (P.R_fixed >= 0) {
+      Rn = P.R_fixed;
+    } else {
+      // beyond = particles landing r+1 .. R_max cells outside their tile's old range (farther ones are far movers
+      // under every radius and do not bear on the choice)
+      const unsigned long long thr = (unsigned long long)(n >> 12);
+      unsigned long long beyond = 0;
+      Rn = P.R_max;
+      for (int r = P.R_max - 1; r >= 1; --r) {
+        beyond += st->excess[r + 1];
+        if (beyond > thr) break;
+        Rn = r;
+      }
+    }
+    st->R_next = (unsigned)Rn;
+    for (int e = 0; e < kMaxR + 2; ++e) st->excess[e] = 0;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -666,10 +724,10 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
 // phase 1 recomputes the push (V2) as straight-line arithmetic, phase 1b redoes the particles pass A flagged
 // through the full advance(), phase 2 ranks inside (warp, cell), deposits and scatters.  One CTA barrier per
 // tile (it frees the stage); the tile's deposit is double-buffered and flushed after it.
-template <int VARIANT>
 __global__ void __launch_bounds__(kThreads, kMinBlocks)
 k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
   constexpr int kWarpSpan = 32 * kItems;
+  if (P.st->stalled) return;
   typedef PassSmem SM;
   extern __shared__ __align__(128) unsigned char smem[];
   Stage* stg = reinterpret_cast<Stage*>(smem);
@@ -677,10 +735,10 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
   unsigned* s_dens2 = reinterpret_cast<unsigned*>(smem + SM::b_dens);   // [2][kWCap + 1][ns]
   SpeciesP* s_sp = reinterpret_cast<SpeciesP*>(smem + SM::b_sp);
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(smem + SM::b_bar);
-  constexpr bool kRecompute = VARIANT == 2;   // V2: the tile carries the old state and the event bits
 
   const unsigned n = P.st->n;
   const unsigned long long step = P.st->step;
+  const int R = (int)P.st->R_cur;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned lt = (1u << lane) - 1u;   // lanes below this one (cheaper to rematerialise than S2R SR_LTMASK)
   const int ntiles = (int)((n + kTile - 1) / kTile);
@@ -695,7 +753,7 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     fence_proxy_async();
     for (int k = 0; k < 2; ++k) {
       const int t = blockIdx.x + k * G;
-      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, cur.desc[t], kRecompute, kRecompute, true, VARIANT == 1);
+      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, cur.desc[t], R, true, true, true);
     }
   }
   load_species(P, s_sp);
@@ -714,7 +772,7 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     mbar_wait(&bar[it & 1], (unsigned)(it >> 1) & 1u);
     // the stage's descriptor is only valid once its barrier has completed
     const int2 d = S->d;
-    const TileWin tw = make_window(d.x, d.y, P.R);
+    const TileWin tw = make_window(d.x, d.y, R);
 
     // destination of this warp's first particle of every window cell
     for (int k = lane; k < tw.W; k += 32) wc[k] = (unsigned)S->tb[k] + S->pre[k * kWarps + warp];
@@ -732,24 +790,21 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
       const int off = warp * kWarpSpan + r * 32 + lane;
       const bool have = (unsigned)off < cnt;
       x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off];
-      int c = d.x;
-      if (have) c = kRecompute ? cell_of(P, x[r]) : S->cell[off];
-      if (kRecompute) {
-        const int sp = have ? (int)S->sp[off] : 0;
-        if (have && ((S->evt[warp * kItems + r] >> lane) & 1u)) evm |= 1u << r;
-        push_fast(P, s_sp[sp], Eptr, c, x[r], vx[r], vy[r], vz[r]);
-        c = cell_of(P, x[r]);
-      }
+      int c = have ? cell_of(P, x[r]) : d.x;
+      const int sp = have ? (int)S->sp[off] : 0;
+      if (have && ((S->evt[warp * kItems + r] >> lane) & 1u)) evm |= 1u << r;
+      push_fast(P, s_sp[sp], Eptr, c, x[r], vx[r], vy[r], vz[r]);
+      c = cell_of(P, x[r]);
       const int k = c - tw.wlo;
       key[r] = (have && c >= 0 && k >= 0 && k < tw.W) ? k : -1;
     }
-    // phase 1b (V2): the particles pass A flagged take the full step again, side effects off
-    if (kRecompute && evm) {
+    // phase 1b: the particles pass A flagged take the full step again, side effects off
+    if (evm) {
 #pragma unroll
       for (int r = 0; r < kItems; ++r) {
         if ((evm >> r) & 1u) {
           const int off = warp * kWarpSpan + r * 32 + lane;
-          const int c = slow_advance<false>(P, s_sp, step, Eptr, S, off, base + (unsigned)off);
+          const int c = slow_advance<SinkNone>(P, s_sp, step, Eptr, S, off, base + (unsigned)off);
           x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off];
           const int k = c - tw.wlo;
           key[r] = (c >= 0 && k >= 0 && k < tw.W) ? k : -1;
@@ -810,13 +865,13 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
         const int off = warp * kWarpSpan + r * 32 + lane;
         const unsigned dst = o + (unsigned)__popc(m[r] & lt);
         nxt.x[dst] = x[r]; nxt.vx[dst] = vx[r]; nxt.vy[dst] = vy[r]; nxt.vz[dst] = vz[r];
-        nxt.cell[dst] = tw.wlo + key[r]; nxt.pid[dst] = S->pid[off]; nxt.sp[dst] = (unsigned char)sp[r];
+        nxt.pid[dst] = S->pid[off]; nxt.sp[dst] = (unsigned char)sp[r];
       }
     }
     if (evm) fence_proxy_async();   // only the slow path writes into the stage (generic proxy) before its reload
     __syncthreads();  // the stage may be overwritten; the tile's deposit is complete
     if (threadIdx.x == 0 && tnext < ntiles)
-      issue_tile(P, cur, S, &bar[it & 1], tnext, dn, kRecompute, kRecompute, true, VARIANT == 1);
+      issue_tile(P, cur, S, &bar[it & 1], tnext, dn, R, true, true, true);
     if (P.dep_u32) {
       for (int k = threadIdx.x; k < ns * (tw.W + 1); k += kThreads) {
         const unsigned v = s_dens[k];
@@ -836,9 +891,9 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
   for (unsigned p = blockIdx.x * kThreads + threadIdx.x; p < Mv; p += G * kThreads) {
     const int dst = P.ovf_dst[p];
     const OvfRec rec = P.ovf_rec[P.ovf_idx[p]];
-    const int c = (int)(P.ovf_key[p] >> kCellShift);
+    const int c = (int)(P.ovf_key[p] >> P.cell_shift);
     nxt.x[dst] = rec.x; nxt.vx[dst] = rec.vx; nxt.vy[dst] = rec.vy; nxt.vz[dst] = rec.vz;
-    nxt.cell[dst] = c; nxt.pid[dst] = rec.pid; nxt.sp[dst] = (unsigned char)rec.sp;
+    nxt.pid[dst] = rec.pid; nxt.sp[dst] = (unsigned char)rec.sp;
     const unsigned Q = (unsigned)s_sp[rec.sp].Q;
     const unsigned a = deposit_a(rec.x, c, P.inv_dx, Q);
     int j1 = c + 1;
@@ -849,17 +904,22 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// Standalone deposit (load / restart; also SURVEY 8(a) row a5 as its own kernel).
-__global__ void __launch_bounds__(kAuxThreads) k_deposit(const __grid_constant__ Params P, Particles cur) {
-  const unsigned n = P.st->n;
-  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-    const int c = cur.cell[i], s = cur.sp[i];
+// Standalone deposit (load / restart / general path; also SURVEY 8(a) row a5 as its own kernel).  *n_ptr particles.
+__global__ void __launch_bounds__(kAuxThreads) k_deposit(const __grid_constant__ Params P, Particles cur,
+                                                         const unsigned* n_ptr) {
+  const unsigned n = *n_ptr;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  // whole warps iterate together (the match below is warp-wide)
+  for (size_t i0 = (size_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u); i0 < n; i0 += stride) {
+    const size_t i = i0 + (threadIdx.x & 31u);
+    const bool have = i < n;
+    const double x = have ? cur.x[i] : 0.0;
+    const int c = cell_of(P, x), s = have ? (int)cur.sp[i] : 0;
     const unsigned Q = (unsigned)P.sp[s].Q;
-    const unsigned a = deposit_a(cur.x[i], c, P.inv_dx, Q);
+    const unsigned a = deposit_a(x, c, P.inv_dx, Q);
     // neighbours in the sorted array mostly share (cell, species): one atomic per run inside the warp
-    const unsigned gk = (unsigned)c * kMaxSpecies + (unsigned)s;
-    const unsigned act = __activemask();
-    const unsigned m = __match_any_sync(act, gk);
+    const unsigned gk = have ? (unsigned)c * kMaxSpecies + (unsigned)s : (0x80000000u | (threadIdx.x & 31u));
+    const unsigned m = __match_any_sync(0xffffffffu, gk);
     unsigned long long lo = Q - a, hi = a;
     // segmented sum over the match group (small groups: loop over members)
     unsigned long long slo = 0, shi = 0;
@@ -868,7 +928,7 @@ __global__ void __launch_bounds__(kAuxThreads) k_deposit(const __grid_constant__
       slo += __shfl_sync(m, lo, src);
       shi += __shfl_sync(m, hi, src);
     }
-    if ((int)(threadIdx.x & 31) == __ffs(m) - 1) {
+    if (have && (int)(threadIdx.x & 31) == __ffs(m) - 1) {
       int j1 = c + 1;
       if (!P.bc && j1 == P.nc) j1 = 0;
       atomicAdd((unsigned long long*)&P.dens[(size_t)s * P.ng + c], slo);
@@ -1017,6 +1077,7 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
   const int nc = P.nc, ng = P.ng, bc = P.bc;
   const int G = gridDim.x, b = blockIdx.x;
   DevState* st = P.st;
+  if (st->stalled) return;
   i128* part = reinterpret_cast<i128*>(P.coop_scratch);  // [4][G]: tot, wsum, A, C
   // phase A: rho, then (NEXT-1, reading N1-a) `smooth` passes of the exact-integer 1-2-1 filter, then the two
   // plain reductions over the array the solve uses
@@ -1129,6 +1190,8 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
     if (commit_step) st->step += 1ull;
     st->ovf_count = 0;
     st->ovf_valid = 0;
+    const unsigned Rn = P.R_fixed >= 0 ? (unsigned)P.R_fixed : st->R_next;
+    st->R_cur = Rn < 1u && P.R_fixed < 0 ? 1u : Rn;
   }
 }
 
@@ -1138,6 +1201,7 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
 // running sums when r > interval - window; at r == interval the sums are latched and cleared.
 __global__ void __launch_bounds__(kAuxThreads) k_average(const __grid_constant__ Params P) {
   DevState* st = P.st;
+  if (st->stalled) return;   // the step did not happen
   const unsigned long long I = (unsigned long long)P.avg_interval, W = (unsigned long long)P.avg_window;
   unsigned long long r = st->step % I;
   if (r == 0) r = I;
@@ -1185,14 +1249,9 @@ static int particle_grid(const Params& P) {
 
 cudaError_t configure_kernels() {
   typedef PassSmem SM;
-  cudaError_t e;
-  e = cudaFuncSetAttribute(k_pass_a<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::a_total);
+  cudaError_t e = cudaFuncSetAttribute(k_pass_a, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::a_total);
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_pass_a<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::a_total);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_pass_b<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::b_total);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(k_pass_b<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::b_total);
+  return cudaFuncSetAttribute(k_pass_b, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::b_total);
 }
 
 static int coop_grid(int work_items, int per_cta) {
@@ -1202,50 +1261,58 @@ static int coop_grid(int work_items, int per_cta) {
   return g < cap ? g : cap;
 }
 
-static void launch_mid(const Params& P, const Particles& cur, int do_colscan, cudaStream_t s) {
+int launch_mid(const Params& P, const Particles& cur, int do_colscan, cudaStream_t s) {
   Params Pc = P;
   Particles pc = cur;
   int dc = do_colscan;
   void* args[] = {&Pc, &pc, &dc};
   cudaLaunchCooperativeKernel((const void*)k_mid, dim3(coop_grid(P.nc, kMidThreads)), dim3(kMidThreads), args, 0, s);
+  return 1;
 }
 
-static void launch_field(const Params& P, int commit_step, cudaStream_t s) {
+int launch_field(const Params& P, int commit_step, cudaStream_t s) {
   Params Pc = P;
   int cs = commit_step;
   void* args[] = {&Pc, &cs};
   cudaLaunchCooperativeKernel((const void*)k_field, dim3(coop_grid(P.ng, kFieldThreads * kFieldItems)),
                               dim3(kFieldThreads), args, 0, s);
+  return 1;
 }
 
-int launch_step(const Params& P, const Particles& cur, const Particles& nxt, int variant, cudaStream_t s,
-                cudaEvent_t* ev) {
+// time-averaged diagnostics of the step just taken (NEXT-1), when armed
+int launch_average(const Params& P, cudaStream_t s) {
+  if (P.avg_window <= 0) return 0;
+  k_average<<<sm_count(), kAuxThreads, 0, s>>>(P);
+  return 1;
+}
+
+int launch_step(const Params& P, const Particles& cur, const Particles& nxt, cudaStream_t s, cudaEvent_t* ev) {
   typedef PassSmem SM;
   const int g = particle_grid(P);
   if (ev) cudaEventRecord(ev[0], s);
-  if (variant == 2) k_pass_a<2><<<g, kThreads, SM::a_total, s>>>(P, cur);
-  else k_pass_a<1><<<g, kThreads, SM::a_total, s>>>(P, cur);
+  k_pass_a<<<g, kThreads, SM::a_total, s>>>(P, cur);
   if (ev) cudaEventRecord(ev[1], s);
   launch_mid(P, cur, 1, s);
   if (ev) cudaEventRecord(ev[2], s);
-  if (variant == 2) k_pass_b<2><<<g, kThreads, SM::b_total, s>>>(P, cur, nxt);
-  else k_pass_b<1><<<g, kThreads, SM::b_total, s>>>(P, cur, nxt);
+  k_pass_b<<<g, kThreads, SM::b_total, s>>>(P, cur, nxt);
   if (ev) cudaEventRecord(ev[3], s);
   launch_field(P, 1, s);
   if (ev) cudaEventRecord(ev[4], s);
-  if (P.avg_window > 0) {
-    k_average<<<sm_count(), kAuxThreads, 0, s>>>(P);
-    return 5;
-  }
-  return 4;
+  return 4 + launch_average(P, s);
 }
 
 // load / restart: counts -> cell_start, deposit, field (no push).  cur must be sorted by cell.  (The tile
-// descriptors are not part of the state: pass A reads them off the sorted cell array.)
+// descriptors are not part of the state: pass A reads them off the sorted positions.)
 __global__ void __launch_bounds__(kAuxThreads) k_count_cells(const __grid_constant__ Params P, Particles cur) {
   const unsigned n = P.st->n;
-  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
-    atomicAdd(&P.cell_count[cur.cell[i]], 1);
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i0 = (size_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u); i0 < n; i0 += stride) {
+    const size_t i = i0 + (threadIdx.x & 31u);
+    const bool have = i < n;
+    const unsigned c = have ? (unsigned)cell_of(P, cur.x[i]) : (0x80000000u | (threadIdx.x & 31u));
+    const unsigned m = __match_any_sync(0xffffffffu, c);
+    if (have && (int)(threadIdx.x & 31u) == __ffs(m) - 1) atomicAdd(&P.cell_count[c], __popc(m));
+  }
 }
 __global__ void k_clear_grids(const __grid_constant__ Params P) {
   const size_t tot = (size_t)P.ns * (size_t)P.ng;
@@ -1257,12 +1324,21 @@ __global__ void k_clear_grids(const __grid_constant__ Params P) {
   }
 }
 
+int launch_clear_grids(const Params& P, cudaStream_t s) {
+  k_clear_grids<<<sm_count() * 4, 256, 0, s>>>(P);
+  return 1;
+}
+
+int launch_deposit(const Params& P, const Particles& cur, const unsigned* n_ptr, cudaStream_t s) {
+  k_deposit<<<sm_count() * 4, kAuxThreads, 0, s>>>(P, cur, n_ptr);
+  return 1;
+}
+
 int launch_rebuild(const Params& P, const Particles& cur, cudaStream_t s) {
-  const int g = sm_count() * 4;
-  k_clear_grids<<<g, 256, 0, s>>>(P);
-  k_count_cells<<<g, kAuxThreads, 0, s>>>(P, cur);
+  launch_clear_grids(P, s);
+  k_count_cells<<<sm_count() * 4, kAuxThreads, 0, s>>>(P, cur);
   launch_mid(P, cur, 0, s);   // ovf_count == 0: plain scan; n_next = n; no column scan (no tile rows yet)
-  k_deposit<<<g, kAuxThreads, 0, s>>>(P, cur);
+  launch_deposit(P, cur, &P.st->n, s);
   launch_field(P, 0, s);  // commits n = n_next, leaves the step counter alone
   return 5;
 }

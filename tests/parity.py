@@ -2,12 +2,12 @@
 import numpy as np
 
 
-def run_pair(w, nsteps, *, variant=0, checkpoint_staging=False, chunk=None):
+def run_pair(w, nsteps, *, checkpoint_staging=False, chunk=None, **bit1_kw):
     """Run the CUDA path and the oracle side by side; returns (gpu, oracle)."""
     from oracle.oracle import Oracle
     from paper_2606_28534_b200.binding import Bit1
 
-    g = Bit1(w, variant=variant, checkpoint_staging=checkpoint_staging)
+    g = Bit1(w, checkpoint_staging=checkpoint_staging, **bit1_kw)
     g.load()
     o = Oracle(w)
     if nsteps:

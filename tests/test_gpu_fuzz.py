@@ -1,5 +1,6 @@
 """Randomised parity: seeded random combinations of workload, size, collision rate, sources, recycling, neutral target,
-smoothing, averaging, window radius, velocity scale and step chunking, CUDA path vs oracle, every element compared.
+smoothing, averaging, window radius (adaptive or pinned) and its bound, side-list capacity (small ones force the general
+path), launch mode, velocity scale and step chunking, CUDA path vs oracle, every element compared, no case skipped.
 BIT1_FUZZ_CASES (default 24) sets how many cases run; BIT1_FUZZ_SEED shifts the sequence; BIT1_FUZZ_BIG=1 draws 4e5 to
 2.5e6 particles per case instead of 7e2 to 7e4."""
 import os
@@ -32,13 +33,19 @@ def _case(seed):
         kw["pair_source"] = bool(rng.integers(0, 2))
         kw["recycle"] = bool(rng.integers(0, 2))
     opts = dict(passes=int(rng.choice([0, 0, 1, 3])), window=0, interval=0,
-                boost=float(rng.choice([1.0, 1.0, 6.0, 40.0])), R=int(rng.choice([1, 1, 0, 2, 4])),
+                boost=float(rng.choice([1.0, 1.0, 6.0, 40.0])), R=int(rng.choice([-1, -1, 1, 0, 2, 4])),
                 chunks=[int(c) for c in rng.integers(1, 14, size=int(rng.integers(1, 5)))],
                 target=bool(cfg >= 4 and rng.integers(0, 2)), gen_seed=int(rng.integers(1, 2**31)),
                 lib_seed=int(rng.integers(1, 2**62)), restart=bool(rng.integers(0, 3) == 0), thin=thin)
     if rng.integers(0, 2):
         opts["interval"] = int(rng.integers(1, 7))
         opts["window"] = int(rng.integers(1, opts["interval"] + 1))
+    # arranger internals (none changes a result): window radius adaptive (-1) or pinned, its upper bound, the side-list
+    # capacity (small ones send steps through the general path), direct launches instead of graph replay
+    b1 = dict(window_radius=None if opts["R"] < 0 else opts["R"], window_radius_max=int(rng.choice([0, 0, 1, 4, 60])),
+              side_list_capacity=int(rng.choice([0, 0, 0, 16, 300, 5000])), direct_launch=bool(rng.integers(0, 4) == 0),
+              checkpoint_staging=bool(rng.integers(0, 2)))
+    opts["bit1"] = b1
     return cfg, kw, opts
 
 
@@ -58,11 +65,7 @@ def test_random_case_matches_oracle(seed):
         setattr(w, k, np.ascontiguousarray(getattr(w, k) * op["boost"]))
     if op["target"]:
         w.target_species = 2
-    os.environ["BIT1_WINDOW_R"] = str(op["R"])
-    try:
-        g = Bit1(w)
-    finally:
-        del os.environ["BIT1_WINDOW_R"]
+    g = Bit1(w, **op["bit1"])
     o = Oracle(w, load=False)
     for side in (g, o):
         side.set_smoothing(op["passes"])
@@ -78,17 +81,10 @@ def test_random_case_matches_oracle(seed):
             g.checkpoint(blob)
             g.checkpoint_wait()
             g.close()
-            os.environ["BIT1_WINDOW_R"] = str(op["R"])
-            try:
-                g = Bit1(w)
-            finally:
-                del os.environ["BIT1_WINDOW_R"]
+            g = Bit1(w, **op["bit1"])
             g.restart(blob)
     g.sync(check_flags=False)
-    m = g.get_moments()
-    if m["flags"] & 4:      # side list beyond its capacity (reading R-side): the CUDA path reports it, nothing to compare
-        pytest.skip("side-list capacity exceeded: " + where)
-    assert assert_state_equal(g, o, where=where)
+    assert assert_state_equal(g, o, where=where)   # whatever path the steps took (fast, side list, general): same bits
     dg, fg, cg, sg = g.get_average()
     do, fo, co, so = o.average()
     assert (cg, sg) == (co, so) and np.array_equal(dg, do) and np.array_equal(fg, fo), where

@@ -9,19 +9,21 @@ from parity import run_pair, assert_state_equal, assert_moments_close
 pytestmark = pytest.mark.gpu
 
 
+MODES = {"default": {}, "direct": dict(direct_launch=True), "general": dict(side_list_capacity=16, window_radius=0)}
+
+
 def small(cfg, scale, **kw):
     w = W.make_config(cfg, scale=scale, **kw)
     return w
 
 
-@pytest.mark.parametrize("variant", [1, 2])
-def test_load_state_matches_oracle(variant):
+def test_load_state_matches_oracle():
     w = small(2, 1 / 64)
-    g, o = run_pair(w, 0, variant=variant)
+    g, o = run_pair(w, 0)
     assert assert_state_equal(g, o, where="load")
 
 
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("mode", ["default", "direct", "general"])
 @pytest.mark.parametrize("cfg,scale,kw", [
     (1, 1 / 16, {}),
     (2, 1 / 64, {}),
@@ -31,14 +33,16 @@ def test_load_state_matches_oracle(variant):
     (4, 1 / 4096, dict(n0_scale=300.0)),
     (5, 1 / 16384, dict(n0_scale=300.0)),
 ])
-def test_one_step_state_matches_oracle(cfg, scale, kw, variant):
+def test_one_step_state_matches_oracle(cfg, scale, kw, mode):
+    """default: the fast path; direct: without CUDA graphs; general: a side list of 16 entries, so that steps with
+    more far movers and births than that stall and are taken by the general path (same bits)."""
     w = small(cfg, scale, **kw)
-    g, o = run_pair(w, 1, variant=variant)
+    g, o = run_pair(w, 1, **MODES[mode])
     exact = assert_state_equal(g, o, where=f"c{cfg} 1 step")
     assert exact, "fp64 state is within tolerance but not bit-identical"
 
 
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("mode", ["default", "general"])
 @pytest.mark.parametrize("cfg,scale,kw,steps", [
     (1, 1.0, {}, 100),
     (2, 1 / 16, {}, 100),
@@ -47,9 +51,9 @@ def test_one_step_state_matches_oracle(cfg, scale, kw, variant):
     (4, 1 / 1024, dict(n0_scale=100.0), 100),
     (5, 1 / 4096, dict(n0_scale=100.0), 100),
 ])
-def test_hundred_steps_match_oracle(cfg, scale, kw, steps, variant):
+def test_hundred_steps_match_oracle(cfg, scale, kw, steps, mode):
     w = small(cfg, scale, **kw)
-    g, o = run_pair(w, steps, variant=variant)
+    g, o = run_pair(w, steps, **MODES[mode])
     assert_state_equal(g, o, where=f"c{cfg} {steps} steps")
     assert_moments_close(g, o, tol=1e-9)
 
