@@ -58,7 +58,7 @@ struct Particles {
   int *cell;
   unsigned *pid;
   unsigned char *sp;
-  int2 *desc;  // per tile of this buffer: (cell of its first particle, cell of its last particle)
+  int2 *desc;  // per tile of this buffer: (cell of its first particle, cell of its last particle), written by k_mid
 };
 
 struct OvfRec {  // one far mover or birth, full state (48 B)

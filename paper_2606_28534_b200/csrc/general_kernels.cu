@@ -210,7 +210,7 @@ int launch_general_step(const Params& P, const Particles& cur, const Particles& 
   launches += launch_clear_grids(P, s);
   k_gen_count_cells<<<g, kGenThreads, 0, s>>>(P, ks);
   launches += 1;
-  launches += launch_mid(P, cur, 0, s);   // scan of the counts -> cell_start, n_next (no side list, no column scan)
+  launches += launch_mid(P, cur, nxt.desc, 0, s);   // scan of the counts -> cell_start, n_next, tile descriptors
   k_gen_gather<<<g, kGenThreads, 0, s>>>(P, cur, nxt, vs);
   launches += 1;
   launches += launch_deposit(P, nxt, &P.st->n_next, s);

@@ -44,15 +44,6 @@ struct PassSmem {
   static constexpr size_t b_total = b_bar + 16;
 };
 
-// (cell of the first particle, cell of the last particle) of tile t: the array is sorted by cell and
-// cell == cell_of(x) by construction (load, pass B, side list), so two positions tell
-__device__ __forceinline__ int2 tile_cells(const Params& P, const Particles& cur, int t, unsigned n) {
-  const size_t first = (size_t)t * kTile;
-  const size_t end = first + kTile;
-  const size_t last = (end < (size_t)n ? end : (size_t)n) - 1;
-  return make_int2(cell_of(P, cur.x[first]), cell_of(P, cur.x[last]));
-}
-
 // first 52 bits of the two-word uniform of slot C0 as an integer: u52(a, b) = (w + 0.5) * 2^-52
 __device__ __forceinline__ unsigned long long w52(unsigned a, unsigned b) {
   return (((unsigned long long)a << 32) | (unsigned long long)b) >> 12;
@@ -89,7 +80,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
     fence_proxy_async();
     for (int k = 0; k < 2; ++k) {
       const int t = blockIdx.x + k * G;
-      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, tile_cells(P, cur, t, n), R, false, true, false);
+      if (t < ntiles) issue_tile(P, cur, &stg[k], &bar[k], t, cur.desc[t], R, false, true, false);
     }
   }
   load_species(P, s_sp);
@@ -111,11 +102,10 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
     // cells of the tile after next (its load is issued at the end of this iteration)
     int2 dn = make_int2(0, 0);
     const int tnext = tile + 2 * G;
-    if (threadIdx.x == 0 && tnext < ntiles) dn = tile_cells(P, cur, tnext, n);
+    if (threadIdx.x == 0 && tnext < ntiles) dn = cur.desc[tnext];
     mbar_wait(&bar[it & 1], (unsigned)(it >> 1) & 1u);
 
     const int clo = S->d.x, chi = S->d.y;
-    if (threadIdx.x == 0) cur.desc[tile] = S->d;   // read by k_mid's column scan and by pass B's issuing thread
     const TileWin tw = make_window(clo, chi, R);
     int e0, ne;
     const double* Eptr = e_window(clo, chi, e0, ne) ? (S->E - e0) : P.E;
@@ -165,7 +155,9 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
               emit_record(P, make_key(P, c, c < tw.wlo ? 1u : 0u, (unsigned long long)i), S->x[off], S->vx[off],
                           S->vy[off], S->vz[off], S->pid[off], (int)S->sp[off]);
               cn[r] = -2;  // placed through the side list
-              atomicAdd(&s_exc[min(max(clo - c, c - chi), kMaxR + 1)], 1u);   // see phase 3
+              // see phase 3 (a tile too sparse for its window sends cells of its own old range here: no excess)
+              const int ex = max(clo - c, c - chi);
+              if (ex >= 2) atomicAdd(&s_exc[min(ex, kMaxR + 1)], 1u);
             }
           }
         }
@@ -177,13 +169,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
       const int off = warp * kWarpSpan + r * 32 + lane;
       const bool have = (unsigned)off < cnt;
       unsigned key = 0x80000000u | (unsigned)lane;  // unique: matches nobody
-      if (have && cn[r] >= 0) {
-        key = (unsigned)(cn[r] - tw.wlo);
-        // how far outside the tile's old cell range the particle lands: k_mid picks the next step's radius from
-        // these counts (never taken at radius 1: a windowed particle is then at most one cell outside)
-        const int ex = max(clo - cn[r], cn[r] - chi);
-        if (ex >= 2) atomicAdd(&s_exc[min(ex, kMaxR + 1)], 1u);
-      }
+      if (have && cn[r] >= 0) key = (unsigned)(cn[r] - tw.wlo);
       {
         const unsigned eb = __ballot_sync(0xffffffffu, (evm >> r) & 1u);
         if (lane == 0) P.evt[(base >> 5) + (unsigned)(warp * kItems + r)] = eb;
@@ -191,6 +177,17 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
       const unsigned m = __match_any_sync(0xffffffffu, key);
       if (!(key & 0x80000000u) && lane == __ffs(m) - 1) s_hist[key * kWarps + warp] += (unsigned)__popc(m);
       __syncwarp();
+    }
+    // how far outside the tile's old cell range the windowed particles land: k_mid picks the next step's radius from
+    // these counts and the far movers' (phase 2).  At radius 1 a windowed particle is at most one cell outside and
+    // there is nothing to count; the loop is kept out of the phases above, whose instruction count bounds the pass.
+    if (R > 1) {
+#pragma unroll
+      for (int r = 0; r < kItems; ++r) {
+        const bool have = (unsigned)(warp * kWarpSpan + r * 32 + lane) < cnt;
+        const int ex = max(clo - cn[r], cn[r] - chi);
+        if (have && cn[r] >= 0 && ex >= 2) atomicAdd(&s_exc[min(ex, kMaxR + 1)], 1u);
+      }
     }
     if (evm) fence_proxy_async();   // only the slow path writes into the stage (generic proxy) before its reload
     __syncthreads();
@@ -424,13 +421,15 @@ __device__ void grid_radix_sort(cg::grid_group& grid, const Params& P, unsigned 
 //   phase 0          side list: births get their pids in (parent, kind) order, the list is ordered by (cell, class,
 //                    order), every cell's group joins the cell's count.  Short lists: CTA 0, in shared memory; long
 //                    lists: the whole grid (radix sort).  A list beyond its capacity stalls the step (see DevState).
-//   phase 1          exclusive scan of the cell counts over all CTAs -> cell_start, cell_base; counts zeroed
+//   phase 1          exclusive scan of the cell counts over all CTAs -> cell_start, cell_base; counts zeroed; the
+//                    (first cell, last cell) descriptor of every tile of the new arrangement (desc_out)
 //   phase 2          destinations of the side-list entries; banded column scan (do_colscan): one thread per cell
 //                    walks, in tile order, the tiles whose window holds the cell and hands each its destination
 //                    base = cell_base[c] + what the earlier tiles send to c.  Those tiles are the ones that hold
 //                    old cells c-R .. c+R, found from the previous step's cell_start.  Last, the next step's window
 //                    radius is chosen from pass A's excess counts.
-__global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Params P, Particles cur, int do_colscan) {
+__global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Params P, Particles cur, int2* desc_out,
+                                                     int do_colscan) {
   __shared__ __align__(16) unsigned char s_raw[kMidRaw];
   __shared__ int s_warp[33];
   __shared__ unsigned s_cnt;
@@ -636,6 +635,16 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
         P.cell_base[c + k] = ex + bf[k];
         P.cell_count[c + k] = 0;
         P.ovf_before[c + k] = 0;
+        // descriptors of the new arrangement's tiles (first, last cell): the tiles that slots [ex, ex + v) touch
+        // take this cell as their first cell if their first slot lies in it, as their last if their last slot does
+        if (v[k] > 0) {
+          const int end = ex + v[k];
+          for (int t = ex / kTile; t * kTile < end; ++t) {
+            const int last = min(t * kTile + kTile, total) - 1;
+            if (t * kTile >= ex) desc_out[t].x = c + k;
+            if (last < end) desc_out[t].y = c + k;
+          }
+        }
       }
       ex += v[k];
     }
@@ -1261,11 +1270,12 @@ static int coop_grid(int work_items, int per_cta) {
   return g < cap ? g : cap;
 }
 
-int launch_mid(const Params& P, const Particles& cur, int do_colscan, cudaStream_t s) {
+int launch_mid(const Params& P, const Particles& cur, int2* desc_out, int do_colscan, cudaStream_t s) {
   Params Pc = P;
   Particles pc = cur;
+  int2* dout = desc_out;
   int dc = do_colscan;
-  void* args[] = {&Pc, &pc, &dc};
+  void* args[] = {&Pc, &pc, &dout, &dc};
   cudaLaunchCooperativeKernel((const void*)k_mid, dim3(coop_grid(P.nc, kMidThreads)), dim3(kMidThreads), args, 0, s);
   return 1;
 }
@@ -1292,7 +1302,7 @@ int launch_step(const Params& P, const Particles& cur, const Particles& nxt, cud
   if (ev) cudaEventRecord(ev[0], s);
   k_pass_a<<<g, kThreads, SM::a_total, s>>>(P, cur);
   if (ev) cudaEventRecord(ev[1], s);
-  launch_mid(P, cur, 1, s);
+  launch_mid(P, cur, nxt.desc, 1, s);
   if (ev) cudaEventRecord(ev[2], s);
   k_pass_b<<<g, kThreads, SM::b_total, s>>>(P, cur, nxt);
   if (ev) cudaEventRecord(ev[3], s);
@@ -1301,8 +1311,7 @@ int launch_step(const Params& P, const Particles& cur, const Particles& nxt, cud
   return 4 + launch_average(P, s);
 }
 
-// load / restart: counts -> cell_start, deposit, field (no push).  cur must be sorted by cell.  (The tile
-// descriptors are not part of the state: pass A reads them off the sorted positions.)
+// load / restart: counts -> cell_start and tile descriptors, deposit, field (no push).  cur must be sorted by cell.
 __global__ void __launch_bounds__(kAuxThreads) k_count_cells(const __grid_constant__ Params P, Particles cur) {
   const unsigned n = P.st->n;
   const size_t stride = (size_t)gridDim.x * blockDim.x;
@@ -1337,7 +1346,7 @@ int launch_deposit(const Params& P, const Particles& cur, const unsigned* n_ptr,
 int launch_rebuild(const Params& P, const Particles& cur, cudaStream_t s) {
   launch_clear_grids(P, s);
   k_count_cells<<<sm_count() * 4, kAuxThreads, 0, s>>>(P, cur);
-  launch_mid(P, cur, 0, s);   // ovf_count == 0: plain scan; n_next = n; no column scan (no tile rows yet)
+  launch_mid(P, cur, cur.desc, 0, s);   // ovf_count == 0: plain scan; n_next = n; no column scan (no tile rows yet)
   launch_deposit(P, cur, &P.st->n, s);
   launch_field(P, 0, s);  // commits n = n_next, leaves the step counter alone
   return 5;

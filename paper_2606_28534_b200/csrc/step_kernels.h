@@ -11,7 +11,8 @@ int launch_step(const Params& P, const Particles& cur, const Particles& nxt, cud
 int launch_rebuild(const Params& P, const Particles& cur, cudaStream_t s);
 // pieces of the above that the general path reuses
 int launch_clear_grids(const Params& P, cudaStream_t s);
-int launch_mid(const Params& P, const Particles& cur, int do_colscan, cudaStream_t s);
+// desc_out: tile descriptors of the arrangement the scan describes (the store half it lives in)
+int launch_mid(const Params& P, const Particles& cur, int2* desc_out, int do_colscan, cudaStream_t s);
 int launch_deposit(const Params& P, const Particles& cur, const unsigned* n_ptr, cudaStream_t s);
 int launch_field(const Params& P, int commit_step, cudaStream_t s);
 int launch_average(const Params& P, cudaStream_t s);

@@ -79,6 +79,7 @@ class Workload:
     inv_norm: np.ndarray
     steps: int
     target_species: int = -1   # NEXT-2: species whose particle density is the collision target (-1: uniform n0)
+    n_per: int = 0             # particles per loaded species of the recipe (also set when the arrays are skipped)
     x: np.ndarray = field(repr=False, default=None)
     vx: np.ndarray = field(repr=False, default=None)
     vy: np.ndarray = field(repr=False, default=None)
@@ -189,7 +190,8 @@ _CFG = {
 
 def make_config(cfg: int, scale: float = 1.0, *, n0_scale: float = 1.0, pair_source: bool = False, recycle: bool = False,
                 gen_seed: Optional[int] = None, lib_seed: Optional[int] = None,
-                capacity_factor: float = 1.02, particles: bool = True) -> Workload:
+                capacity_factor: float = 1.02, particles: bool = True, ppc_scale: float = 1.0,
+                quiet: bool = True) -> Workload:
     """Build configuration `cfg` (1..5) of BASELINE.json.
 
     scale       shrinks N and nc together (same particles per cell, same profile shape).
@@ -199,11 +201,16 @@ def make_config(cfg: int, scale: float = 1.0, *, n0_scale: float = 1.0, pair_sou
     recycle     NEXT-2: absorbed D+ ions leave a D neutral at the wall; configs without a neutral
                 species get an (initially empty) one.
     particles   False skips the particle arrays (only parameters and tables).
+    ppc_scale   multiplies the particles per cell at unchanged nc (the weight follows, so the physical density stays):
+                e.g. configs[4]'s 1 048 576 cells with 16 instead of 954 particles per cell.
+    quiet       True (default): every D+ ion is loaded on its electron (rho == 0 at step 0); False: the charged
+                species are loaded independently -- the stress variant with a sqrt(N) charge imbalance, strong
+                Langmuir oscillations and orders of magnitude more far movers.
     """
     c = _CFG[cfg]
     nc = max(8, int(round(c["nc"] * scale)))
     ns = c["ns"]
-    n_per = max(1, int(round(c["N"] * scale)) // ns)
+    n_per = max(1, int(round(c["N"] * scale * ppc_scale)) // ns)
     lam, wpe = _plasma_scales(c["n_ref"], c["T"])
     dx = 0.5 * lam
     dt = 0.1 / wpe
@@ -242,12 +249,13 @@ def make_config(cfg: int, scale: float = 1.0, *, n0_scale: float = 1.0, pair_sou
     n_total = n_per * ns
     cap = int(math.ceil(n_total * capacity_factor)) + 1024
     w = Workload(
-        name=f"c{cfg}" + ("P" if pair_source else "") + (f"@{scale:g}" if scale != 1.0 else ""),
+        name=f"c{cfg}" + ("P" if pair_source else "") + (f"@{scale:g}" if scale != 1.0 else "") +
+        (f"x{ppc_scale:g}ppc" if ppc_scale != 1.0 else "") + ("" if quiet else "-noisy"),
         nc=nc, dx=dx, bc=c["bc"], area=area, B=B, dt=dt, species=sp,
         seed=(lib_seed if lib_seed is not None else 2606285340000 + cfg),
         capacity=cap, src_lo=0.25 * L, src_hi=0.75 * L, n0=n0, vth_n=_vth(T0, M_D),
         E_ion=E_ION, m_n=M_D, sig_el=tabs[0], sig_ion=tabs[1], sig_cx=tabs[2], dE_eV=DE_EV,
-        inv_norm=inv_norm_table(), steps=c["steps"],
+        inv_norm=inv_norm_table(), steps=c["steps"], n_per=n_per,
         note=f"BASELINE.json configs[{cfg - 1}], scale {scale:g}",
     )
     if not particles:
@@ -258,7 +266,7 @@ def make_config(cfg: int, scale: float = 1.0, *, n0_scale: float = 1.0, pair_sou
     for k, s in enumerate(sp[:ns]):   # a neutral species added for recycling starts empty
         Tk = T0 if s.name == "D" else T
         x, vx, vy, vz = _species_arrays(gseed, k, n_per, L, c["profile"], _vth(Tk, s.m))
-        if k == 1:
+        if k == 1 and quiet:
             # quiet, quasi-neutral start: every ion is loaded on its electron, rho == 0 at step 0 (SURVEY 8(d) for
             # config 1; extended to every config -- DESIGN.md "Input recipe": independent random loads leave a
             # sqrt(N) charge imbalance over 1e4..5e5 Debye lengths, i.e. Langmuir oscillations of many thermal
@@ -274,6 +282,54 @@ def make_config(cfg: int, scale: float = 1.0, *, n0_scale: float = 1.0, pair_sou
     w.vz = np.ascontiguousarray(np.concatenate(vzs))
     w.sp = np.ascontiguousarray(np.concatenate(tags))
     return w
+
+
+def device_particles(w: Workload, cfg: int, device, gen_seed: Optional[int] = None):
+    """The particle arrays of make_config(cfg, particles=False) generated on the GPU by torch's own seeded generator
+    (same profile, temperatures, equal thirds/halves per species, quiet start), as CUDA tensors (x, vx, vy, vz, sp) for
+    bit1_load_particles(..., ptrs_on_device=1).  For the 1e9-particle configs[4] in bench.py: generating and pinning
+    33 GB on the host would take minutes; nothing is compared with the oracle on these arrays (full-size parity runs
+    use make_config's host arrays)."""
+    import torch
+
+    c = _CFG[cfg]
+    ns = c["ns"]
+    n_per = w.n_per
+    n = n_per * ns
+    g = torch.Generator(device=device)
+    g.manual_seed((gen_seed if gen_seed is not None else 2606285340 + cfg) & (2**63 - 1))
+    x = torch.empty(n, dtype=torch.float64, device=device)
+    v = [torch.empty(n, dtype=torch.float64, device=device) for _ in range(3)]
+    sp = torch.empty(n, dtype=torch.uint8, device=device)
+    L = w.L
+    step = 1 << 25
+    for k in range(ns):
+        Tk = 1.0 if w.species[k].name == "D" else c["T"]
+        vth = _vth(Tk, w.species[k].m)
+        lo = k * n_per
+        sp[lo:lo + n_per] = k
+        for a in range(0, n_per, step):
+            m = min(step, n_per - a)
+            sl = slice(lo + a, lo + a + m)
+            if k == 1:
+                x[sl] = x[a:a + m]          # quiet start: every ion on its electron
+            else:
+                u = torch.rand(m, dtype=torch.float64, device=device, generator=g)
+                if c["profile"] == "uniform":
+                    xs = u * L
+                elif c["profile"] == "exp":
+                    Ls = 0.1 * L
+                    side = torch.rand(m, dtype=torch.float64, device=device, generator=g) < 0.5
+                    d = -Ls * torch.log1p(-u * (-math.expm1(-0.5 * L / Ls)))
+                    xs = torch.where(side, 0.5 * L + d, 0.5 * L - d)
+                else:
+                    plo = 0.5 * (1.0 + math.erf(-2.5 / math.sqrt(2.0)))
+                    phi = 0.5 * (1.0 + math.erf(2.5 / math.sqrt(2.0)))
+                    xs = 0.5 * L + 0.2 * L * math.sqrt(2.0) * torch.special.erfinv(2.0 * (plo + u * (phi - plo)) - 1.0)
+                x[sl] = torch.clamp(xs, 0.0, float(np.nextafter(L, 0.0)))
+            for comp in v:
+                comp[sl] = vth * torch.randn(m, dtype=torch.float64, device=device, generator=g)
+    return x, v[0], v[1], v[2], sp
 
 
 _CHUNK = 1 << 21
