@@ -254,6 +254,7 @@ def _measure(sim, steps: int, warmup: int, peak: float, barrier=None, sampler_in
     ms = ev0.elapsed_time(ev1)
     launches = sim.launch_count() - launches0
     sim.sync()
+    ms_settled = 1e3 * (time.perf_counter() - t_wall0)   # wall clock incl. any step redone by the general path
     n_end = sim.n_live()
     units = 0.5 * (n_start + n_end) * steps
     psteps_want = min(steps, 50)
@@ -265,8 +266,8 @@ def _measure(sim, steps: int, warmup: int, peak: float, barrier=None, sampler_in
     n_prof = 0.5 * (n_end + sim.n_live())
     mom = sim.get_moments()
     kern = {k: v / max(psteps, 1) for k, v in prof.items()}
-    return dict(ms=ms, units=units, launches=int(launches), clocks=clocks, n_end=n_end, n_prof=n_prof, kern=kern,
-                psteps=int(psteps), mom=mom)
+    return dict(ms=ms, ms_settled=ms_settled, units=units, launches=int(launches), clocks=clocks, n_end=n_end,
+                n_prof=n_prof, kern=kern, psteps=int(psteps), mom=mom)
 
 
 def _summary(r, steps: int, peak: float, n0: int):
@@ -471,6 +472,46 @@ def run_cuda(args):
     print(json.dumps(line))
 
 
+def run_sweep(args):
+    """profiles/r2_far_mover_sweep.md: ms/step of one configuration against the fraction of particles that leave their
+    tile's sort window, made by scaling the loaded velocities with the window radius pinned (the side list takes the
+    far movers, the general path takes over beyond its capacity) and adaptive (the window widens instead).  Prints one
+    JSON line per point."""
+    import numpy as np
+    import torch
+
+    from paper_2606_28534_b200.binding import Bit1
+
+    torch.cuda.set_device(0)
+    peak, _ = _peaks()
+    w, wname = _workload(args.config, args.scale, 0, quiet=not args.noisy)
+    base = {k: getattr(w, k).copy() for k in ("vx", "vy", "vz")}
+    for radius in (1, None):
+        for vs in (1.0, 1.5, 2.0, 2.5, 3.0, 4.0, 6.0, 10.0, 40.0):
+            for k in base:
+                setattr(w, k, np.ascontiguousarray(base[k] * vs))
+            kw = dict(window_radius_max=args.radius_max or 40)
+            if radius is not None:
+                kw["window_radius"] = radius
+            sim = Bit1(w, device="cuda:0", **kw)
+            sim.load()
+            steps = args.steps
+            r = _measure(sim, steps, args.warmup, peak)
+            m = r["mom"]
+            # steps redone by the general path run when the host next waits: their time is in the wall clock only
+            ms = r["ms_settled"] if m["general_steps"] else r["ms"]
+            print(json.dumps({"workload": wname + ("" if not args.noisy else " (independent load)"), "vscale": vs,
+                              "radius": "adaptive" if radius is None else radius, "ms_per_step": round(ms / steps, 3),
+                              "timed": "wall clock incl. settle" if m["general_steps"] else "CUDA events",
+                              "far_mover_fraction": m["far_movers"] / max(m["step"], 1) / max(r["n_end"], 1),
+                              "max_far_movers_per_step": m["max_far_movers_per_step"], "window_radius": m["window_radius"],
+                              "general_steps": m["general_steps"], "steps_total": m["step"], "flags": m["flags"],
+                              "kernel_ms_per_step": {k: round(v, 3) for k, v in r["kern"].items()}}), flush=True)
+            sim.close()
+            del sim
+            torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -488,10 +529,13 @@ def main():
     ap.add_argument("--radius", type=int, default=None, help="pin the sort-window radius (default: adaptive)")
     ap.add_argument("--radius-max", type=int, default=0)
     ap.add_argument("--side-list", type=int, default=0, help="side-list capacity (entries)")
+    ap.add_argument("--sweep", default=None, choices=["far-movers"], help="print the far-mover sweep instead of the bench line")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_cuda(args)

@@ -240,6 +240,41 @@ bit1_status bit1_export_species(bit1_ctx *ctx, int species, uint64_t capacity_ou
                                 int64_t *counts_per_cell, double *x, double *vx, double *vy, double *vz,
                                 uint32_t *pid_or_null);
 
+/* Streaming checkpoints: the in-memory hand-off of the paper's openPMD/ADIOS2 "SST" engine ("SST for
+ * in-memory streaming"; record order of PAPER.md:57; an in-situ consumer reads the
+ * checkpoints "without interrupting execution"); SURVEY 8(f) NEXT-4.  No openPMD/ADIOS2 here: the transport is a ring
+ * of 2..8 slots in caller-owned PINNED HOST memory (nslots * slot_bytes, 256-byte aligned; bit1_stream_slot_size() is
+ * the worst case for this context) and a sequence number.
+ *   Producer (the thread that drives the context): bit1_stream_publish waits for the steps enqueued so far, compacts
+ * every species on the device into the paper's record layout -- counts per cell, then x, vx, vy, vz (and the particle
+ * id) in cell order --, copies the slot out on the side stream and returns; bit1_step calls that follow overlap the
+ * copy.  When the copy has landed a host function on the side stream writes the slot's sequence number.  It fills a
+ * free slot, else overwrites the oldest unread one; BIT1_ERR_CAPACITY if the consumer holds every slot or a slot is
+ * too small.  Needs checkpoint_staging = 1 and a side stream (BIT1_ERR_STATE otherwise).
+ *   Consumer (any thread of the process): bit1_stream_acquire hands out the newest complete slot with a sequence
+ * number > after_seq (BIT1_ERR_STATE if there is none yet; it never blocks) and keeps the producer off it until
+ * bit1_stream_release(seq).  The slot starts with a bit1_stream_header; offsets are bytes from the slot's start.
+ * A reader in another process that maps the same memory follows the seqlock: a slot is complete iff
+ * seq == seq_begin != 0, before and after it has copied what it needs. */
+#define BIT1_STREAM_MAX_SLOTS 8
+typedef struct {
+  char magic[8];                       /* "BIT1STRM" */
+  uint64_t seq_begin;                  /* sequence number of the snapshot being written / held by this slot */
+  uint64_t seq;                        /* == seq_begin once the slot is complete */
+  uint64_t step, n_total, bytes;       /* step counter of the snapshot, live particles, bytes used in the slot */
+  int32_t nc, ns, bc, _pad;
+  uint64_t count[BIT1_MAX_SPECIES];    /* particles of species s */
+  uint64_t off_counts[BIT1_MAX_SPECIES]; /* int32[nc]: particles of species s per cell */
+  uint64_t off_x[BIT1_MAX_SPECIES], off_vx[BIT1_MAX_SPECIES], off_vy[BIT1_MAX_SPECIES], off_vz[BIT1_MAX_SPECIES]; /* fp64[count] */
+  uint64_t off_pid[BIT1_MAX_SPECIES];  /* uint32[count] */
+} bit1_stream_header;
+size_t bit1_stream_slot_size(bit1_ctx *ctx);
+bit1_status bit1_stream_open(bit1_ctx *ctx, void *ring_pinned_host, size_t slot_bytes, int nslots);
+bit1_status bit1_stream_publish(bit1_ctx *ctx, uint64_t *seq_or_null);
+bit1_status bit1_stream_acquire(bit1_ctx *ctx, uint64_t after_seq, const void **slot, uint64_t *seq);
+bit1_status bit1_stream_release(bit1_ctx *ctx, uint64_t seq);
+bit1_status bit1_stream_close(bit1_ctx *ctx);
+
 void bit1_destroy(bit1_ctx *ctx);
 const char *bit1_error_string(bit1_status s);
 /* Per-kernel device timing for the roofline report.  While enabled, bit1_step

@@ -55,6 +55,15 @@ class bit1_moments(C.Structure):
                 ("window_radius", C.c_uint32), ("_pad", C.c_uint32), ("density", c_f64p * MAX_SPECIES)]
 
 
+class bit1_stream_header(C.Structure):
+    _fields_ = [("magic", C.c_char * 8), ("seq_begin", C.c_uint64), ("seq", C.c_uint64), ("step", C.c_uint64),
+                ("n_total", C.c_uint64), ("bytes", C.c_uint64), ("nc", C.c_int32), ("ns", C.c_int32), ("bc", C.c_int32),
+                ("_pad", C.c_int32), ("count", C.c_uint64 * MAX_SPECIES), ("off_counts", C.c_uint64 * MAX_SPECIES),
+                ("off_x", C.c_uint64 * MAX_SPECIES), ("off_vx", C.c_uint64 * MAX_SPECIES),
+                ("off_vy", C.c_uint64 * MAX_SPECIES), ("off_vz", C.c_uint64 * MAX_SPECIES),
+                ("off_pid", C.c_uint64 * MAX_SPECIES)]
+
+
 _lib = None
 
 
@@ -117,6 +126,18 @@ def load_library(path: Optional[str] = None):
     L.bit1_restart.argtypes = [vp, vp, C.c_size_t]
     L.bit1_export_species.restype = C.c_int
     L.bit1_export_species.argtypes = [vp, C.c_int, C.c_uint64, C.POINTER(C.c_uint64), vp, vp, vp, vp, vp, vp]
+    L.bit1_stream_slot_size.restype = C.c_size_t
+    L.bit1_stream_slot_size.argtypes = [vp]
+    L.bit1_stream_open.restype = C.c_int
+    L.bit1_stream_open.argtypes = [vp, vp, C.c_size_t, C.c_int]
+    L.bit1_stream_publish.restype = C.c_int
+    L.bit1_stream_publish.argtypes = [vp, C.POINTER(C.c_uint64)]
+    L.bit1_stream_acquire.restype = C.c_int
+    L.bit1_stream_acquire.argtypes = [vp, C.c_uint64, C.POINTER(vp), C.POINTER(C.c_uint64)]
+    L.bit1_stream_release.restype = C.c_int
+    L.bit1_stream_release.argtypes = [vp, C.c_uint64]
+    L.bit1_stream_close.restype = C.c_int
+    L.bit1_stream_close.argtypes = [vp]
     L.bit1_destroy.restype = None
     L.bit1_destroy.argtypes = [vp]
     L.bit1_error_string.restype = C.c_char_p
@@ -393,6 +414,52 @@ class Bit1:
                                             d["pid"].ctypes.data), "bit1_export_species")
         d["counts"] = counts
         return d
+
+    # -- streaming checkpoints (NEXT-4) ------------------------------------------------------------
+    def stream_slot_size(self) -> int:
+        return int(self.lib.bit1_stream_slot_size(self.h))
+
+    def stream_open(self, ring, nslots: int):
+        """ring: pinned torch uint8 CPU tensor of nslots equal slots (256-byte aligned, slot size a multiple of 256)."""
+        self._ring = ring
+        self._slot_bytes = ring.numel() // nslots
+        _check(self.lib.bit1_stream_open(self.h, ring.data_ptr(), self._slot_bytes, int(nslots)), "bit1_stream_open")
+
+    def stream_publish(self) -> int:
+        seq = C.c_uint64()
+        _check(self.lib.bit1_stream_publish(self.h, C.byref(seq)), "bit1_stream_publish")
+        return int(seq.value)
+
+    def stream_acquire(self, after_seq: int = 0):
+        """Newest complete snapshot with a sequence number > after_seq, or None.  Returns (seq, snapshot): step,
+        n_total and per species a dict(counts[nc] int32, x, vx, vy, vz, pid) of numpy VIEWS of the pinned slot, valid
+        until stream_release(seq)."""
+        slot, seq = C.c_void_p(), C.c_uint64()
+        st = self.lib.bit1_stream_acquire(self.h, int(after_seq), C.byref(slot), C.byref(seq))
+        if st == ERR_STATE:
+            return None
+        _check(st, "bit1_stream_acquire")
+        hd = bit1_stream_header.from_address(slot.value)
+        assert hd.magic == b"BIT1STRM" and hd.seq == hd.seq_begin == seq.value
+
+        def view(off, n, dt):
+            nbytes = n * np.dtype(dt).itemsize
+            buf = (C.c_char * nbytes).from_address(slot.value + off)
+            return np.frombuffer(buf, dtype=dt, count=n)
+
+        sp = []
+        for s in range(hd.ns):
+            n = int(hd.count[s])
+            sp.append(dict(counts=view(hd.off_counts[s], hd.nc, np.int32), x=view(hd.off_x[s], n, np.float64),
+                           vx=view(hd.off_vx[s], n, np.float64), vy=view(hd.off_vy[s], n, np.float64),
+                           vz=view(hd.off_vz[s], n, np.float64), pid=view(hd.off_pid[s], n, np.uint32)))
+        return int(seq.value), dict(step=int(hd.step), n_total=int(hd.n_total), bytes=int(hd.bytes), species=sp)
+
+    def stream_release(self, seq: int):
+        _check(self.lib.bit1_stream_release(self.h, int(seq)), "bit1_stream_release")
+
+    def stream_close(self):
+        _check(self.lib.bit1_stream_close(self.h), "bit1_stream_close")
 
     def profile(self, enable: bool = True):
         _check(self.lib.bit1_profile(self.h, int(enable)), "bit1_profile")

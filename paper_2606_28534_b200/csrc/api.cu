@@ -6,6 +6,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <atomic>
 #include <new>
 #include <vector>
 
@@ -114,9 +115,16 @@ CkptLayout ckpt_layout(int nc, int ng, int ns, size_t n) {
   return c;
 }
 
+// Streamed snapshot (bit1_stream_publish): per species the counts per cell (int32[nc]) and the x, vx, vy, vz (fp64)
+// and id (uint32) records in cell order, every array 256-byte aligned; worst case over how n splits among species
+size_t stream_payload_bytes(int nc, int ns, size_t n) {
+  return (size_t)ns * (align_up((size_t)nc * 4) + 5 * kAlign) + 4 * align_up(n * 8) + align_up(n * 4) +
+         (size_t)ns * 5 * kAlign;
+}
+
 struct Layout {
   size_t st, tables, dens, dens_old, rho, rho_s, rho_t, avg, phi, E, cell_count, cell_start, cell_start_old, scan_part, coop_scratch, cell_base, ovf_before, ovf_lb, ovf_ub, radix_hist, tile_hist, tile_base, tile_pre, evt,
-      ovf_key, ovf_idx, ovf_dst, tmp_key, tmp_idx, tmp2_key, tmp2_idx, ovf_rec, part[2], scratch, small, mom, total;
+      ovf_key, ovf_idx, ovf_dst, tmp_key, tmp_idx, tmp2_key, tmp2_idx, ovf_rec, part[2], scratch, small, exp, mom, total;
   unsigned ovf_cap;
   int max_tiles, ng;
   size_t scratch_bytes;
@@ -169,12 +177,14 @@ Layout make_layout(int nc, int bc, int ns, const Shape& sh) {
   // one scratch area for the calls that never overlap one another: load-time sort, general-path step, export, and
   // the device snapshot of an overlapped checkpoint (a general-path step first waits for a pending checkpoint)
   l.scratch_bytes = general_scratch_bytes((unsigned)cap);
-  if (export_scratch_bytes(nc, (unsigned)cap) > l.scratch_bytes) l.scratch_bytes = export_scratch_bytes(nc, (unsigned)cap);
   if (sh.staging) {
-    const size_t cb = ckpt_layout(nc, l.ng, ns, cap).bytes;
+    size_t cb = ckpt_layout(nc, l.ng, ns, cap).bytes;
+    const size_t sb = stream_payload_bytes(nc, ns, cap);   // bit1_stream_publish stages its records there too
+    if (sb > cb) cb = sb;
     if (cb > l.scratch_bytes) l.scratch_bytes = cb;
   }
   l.scratch = take(l.scratch_bytes);
+  l.exp = take(export_scratch_bytes(nc, (unsigned)cap));
   l.small = take(ckpt_layout(nc, l.ng, ns, 0).bytes);   // DevState + averaging sums of a checkpoint without staging
   l.mom = take(moments_scratch_bytes());
   l.total = o;
@@ -231,7 +241,16 @@ struct bit1_ctx {
   uint64_t last_general_step;   // step index the general path last took
   unsigned burst;               // steps to take by the general path outright after the next stall
   uint64_t general_steps_host;
+  // streaming checkpoints (bit1_stream_*): ring of caller-owned pinned slots, states shared with the consumer thread
+  char* ring;
+  size_t slot_bytes;
+  int nslots;
+  uint64_t next_seq;
+  std::atomic<int> slot_state[BIT1_STREAM_MAX_SLOTS];        // kSlotFree / Filling / Ready / Held
+  std::atomic<uint64_t> slot_seq[BIT1_STREAM_MAX_SLOTS];
+  struct StreamDone { bit1_ctx* c; int slot; uint64_t seq; } done_arg[BIT1_STREAM_MAX_SLOTS];
 };
+enum { kSlotFree = 0, kSlotFilling = 1, kSlotReady = 2, kSlotHeld = 3 };
 constexpr size_t kMaxProfSteps = 4096;
 
 #define CUDA_OK(call)                              \
@@ -337,6 +356,8 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   c->graph[0] = c->graph[1] = nullptr;
   c->use_graph = o->launch_mode == 0;
   c->step_target = 0; c->last_general_step = ~0ull; c->burst = 0; c->general_steps_host = 0;
+  c->ring = nullptr; c->slot_bytes = 0; c->nslots = 0; c->next_seq = 1;
+  for (int k = 0; k < BIT1_STREAM_MAX_SLOTS; ++k) { c->slot_state[k].store(kSlotFree); c->slot_seq[k].store(0); }
 
   Params& P = c->P;
   P.nc = g->nc; P.bc = g->bc; P.ng = lay.ng; P.ns = ns;
@@ -964,9 +985,9 @@ bit1_status bit1_export_species(bit1_ctx* c, int species, uint64_t capacity_out,
   if (!c || species < 0 || species >= c->P.ns || !n_out) return BIT1_ERR_INVALID_ARG;
   if (!c->loaded) return BIT1_ERR_STATE;
   BIT1_OK_OR_RETURN(settle(c, nullptr));
-  // staging area = scratch; the idle half of the store is also about to be written
+  // a checkpoint without staging may still be reading the store; the idle half is about to be written
   if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; c->ckpt_reads_live = false; }
-  char* sc = c->ws + c->lay.scratch;
+  char* sc = c->ws + c->lay.exp;
   c->launches += launch_export_count(c->P, c->buf[c->cur], species, c->P.capacity, sc, c->cs);
   unsigned long long total = 0;
   CUDA_OK(cudaMemcpyAsync(&total, sc, 8, cudaMemcpyDeviceToHost, c->cs));
@@ -1154,6 +1175,161 @@ bit1_status bit1_restart(bit1_ctx* c, const void* blob, size_t bytes) {
   c->step_target = h.step; c->last_general_step = ~0ull; c->burst = 0;
   c->loaded = true;
   return BIT1_OK;
+}
+
+// ---- streaming checkpoints (second half) -------------------------------------------------
+static void CUDART_CB stream_done_cb(void* p) {
+  // runs on a CUDA-internal thread once the side-stream copy into the slot has landed: publish the sequence number
+  bit1_ctx::StreamDone* d = static_cast<bit1_ctx::StreamDone*>(p);
+  bit1_ctx* c = d->c;
+  bit1_stream_header* hd = reinterpret_cast<bit1_stream_header*>(c->ring + (size_t)d->slot * c->slot_bytes);
+  std::atomic_thread_fence(std::memory_order_release);
+  reinterpret_cast<std::atomic<uint64_t>*>(&hd->seq)->store(d->seq, std::memory_order_release);
+  c->slot_seq[d->slot].store(d->seq, std::memory_order_release);
+  c->slot_state[d->slot].store(kSlotReady, std::memory_order_release);
+}
+
+size_t bit1_stream_slot_size(bit1_ctx* c) {
+  if (!c) return 0;
+  return sizeof(bit1_stream_header) + stream_payload_bytes(c->P.nc, c->P.ns, c->P.capacity);
+}
+
+bit1_status bit1_stream_open(bit1_ctx* c, void* ring, size_t slot_bytes, int nslots) {
+  if (!c || !ring || nslots < 2 || nslots > BIT1_STREAM_MAX_SLOTS || (slot_bytes & (kAlign - 1)) ||
+      (reinterpret_cast<uintptr_t>(ring) & (kAlign - 1)))
+    return BIT1_ERR_INVALID_ARG;
+  if (!c->staging || c->ss == c->cs) return BIT1_ERR_STATE;   // needs the device snapshot area and a side stream
+  if (c->ring) return BIT1_ERR_STATE;
+  if (slot_bytes < sizeof(bit1_stream_header) + 5 * kAlign) return BIT1_ERR_CAPACITY;
+  c->ring = static_cast<char*>(ring);
+  c->slot_bytes = slot_bytes;
+  c->nslots = nslots;
+  for (int k = 0; k < nslots; ++k) {
+    c->slot_state[k].store(kSlotFree);
+    c->slot_seq[k].store(0);
+    memset(c->ring + (size_t)k * slot_bytes, 0, sizeof(bit1_stream_header));
+  }
+  return BIT1_OK;
+}
+
+bit1_status bit1_stream_close(bit1_ctx* c) {
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; c->ckpt_reads_live = false; }
+  if (c->ss != c->cs) CUDA_OK(cudaStreamSynchronize(c->ss));   // the host function has run
+  c->ring = nullptr; c->nslots = 0;
+  return BIT1_OK;
+}
+
+bit1_status bit1_stream_publish(bit1_ctx* c, uint64_t* seq_out) {
+  NvtxRange nvtx_("bit1_stream_publish");
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  if (!c->loaded || !c->ring) return BIT1_ERR_STATE;
+  // one snapshot in flight at a time: the device staging area is shared with bit1_checkpoint
+  if (c->ckpt_pending) { CUDA_OK(cudaEventSynchronize(c->ev_done)); c->ckpt_pending = false; c->ckpt_reads_live = false; }
+  DevState h;
+  BIT1_OK_OR_RETURN(settle(c, &h));
+  // a slot the consumer does not hold: a free one, else the oldest unread one (it is dropped, as a bounded SST queue does)
+  int slot = -1;
+  uint64_t oldest = ~0ull;
+  for (int k = 0; k < c->nslots && slot < 0; ++k)
+    if (c->slot_state[k].load(std::memory_order_acquire) == kSlotFree) slot = k;
+  if (slot < 0) {
+    for (int k = 0; k < c->nslots; ++k)
+      if (c->slot_state[k].load(std::memory_order_acquire) == kSlotReady && c->slot_seq[k].load() < oldest) {
+        oldest = c->slot_seq[k].load();
+        slot = k;
+      }
+    if (slot >= 0) {
+      int expect = kSlotReady;   // the consumer may grab it at this very moment: then it is held, look no further
+      if (!c->slot_state[slot].compare_exchange_strong(expect, kSlotFilling)) slot = -1;
+    }
+  } else {
+    c->slot_state[slot].store(kSlotFilling, std::memory_order_release);
+  }
+  if (slot < 0) return BIT1_ERR_CAPACITY;   // every slot is held by the consumer
+  const Params& P = c->P;
+  const int nc = P.nc, ns = P.ns;
+  char* sg = c->ws + c->lay.scratch;   // device staging, payload layout (offsets relative to the end of the header)
+  char* ex = c->ws + c->lay.exp;
+  bit1_stream_header hd;
+  memset(&hd, 0, sizeof(hd));
+  memcpy(hd.magic, "BIT1STRM", 8);
+  const uint64_t seq = c->next_seq++;
+  hd.seq_begin = seq; hd.seq = 0; hd.step = h.step; hd.n_total = h.n; hd.nc = nc; hd.ns = ns; hd.bc = P.bc;
+  size_t o = 0;
+  const size_t hsz = sizeof(bit1_stream_header);
+  for (int s = 0; s < ns; ++s) {
+    // counts per cell and the species' total ("the vector of particle counts per cell", then the records)
+    c->launches += launch_export_count(P, c->buf[c->cur], s, P.capacity, ex, c->cs);
+    unsigned long long total = 0;
+    CUDA_OK(cudaMemcpyAsync(&total, ex, 8, cudaMemcpyDeviceToHost, c->cs));
+    CUDA_OK(cudaStreamSynchronize(c->cs));
+    const size_t n = (size_t)total;
+    hd.count[s] = total;
+    hd.off_counts[s] = hsz + o; o += align_up((size_t)nc * 4);
+    hd.off_x[s] = hsz + o; o += align_up(n * 8);
+    hd.off_vx[s] = hsz + o; o += align_up(n * 8);
+    hd.off_vy[s] = hsz + o; o += align_up(n * 8);
+    hd.off_vz[s] = hsz + o; o += align_up(n * 8);
+    hd.off_pid[s] = hsz + o; o += align_up(n * 4);
+    if (hsz + o > c->slot_bytes) { c->slot_state[slot].store(kSlotFree); return BIT1_ERR_CAPACITY; }
+    CUDA_OK(cudaMemcpyAsync(sg + (hd.off_counts[s] - hsz), ex + 256, (size_t)nc * 4, cudaMemcpyDeviceToDevice, c->cs));
+    Particles out;
+    memset(&out, 0, sizeof(out));
+    out.x = reinterpret_cast<double*>(sg + (hd.off_x[s] - hsz));
+    out.vx = reinterpret_cast<double*>(sg + (hd.off_vx[s] - hsz));
+    out.vy = reinterpret_cast<double*>(sg + (hd.off_vy[s] - hsz));
+    out.vz = reinterpret_cast<double*>(sg + (hd.off_vz[s] - hsz));
+    out.pid = reinterpret_cast<unsigned*>(sg + (hd.off_pid[s] - hsz));
+    if (n) c->launches += launch_export_scatter(P, c->buf[c->cur], out, s, ex, c->cs);
+  }
+  hd.bytes = hsz + o;
+  char* hs = c->ring + (size_t)slot * c->slot_bytes;
+  // a reader in another process sees seq != seq_begin while the slot is being filled
+  memcpy(hs, &hd, sizeof(hd));
+  std::atomic_thread_fence(std::memory_order_release);
+  CUDA_OK(cudaEventRecord(c->ev_snap, c->cs));
+  CUDA_OK(cudaStreamWaitEvent(c->ss, c->ev_snap, 0));
+  if (o) CUDA_OK(cudaMemcpyAsync(hs + hsz, sg, o, cudaMemcpyDeviceToHost, c->ss));
+  c->done_arg[slot].c = c; c->done_arg[slot].slot = slot; c->done_arg[slot].seq = seq;
+  CUDA_OK(cudaLaunchHostFunc(c->ss, stream_done_cb, &c->done_arg[slot]));
+  CUDA_OK(cudaEventRecord(c->ev_done, c->ss));
+  c->ckpt_pending = true;
+  if (seq_out) *seq_out = seq;
+  return BIT1_OK;
+}
+
+bit1_status bit1_stream_acquire(bit1_ctx* c, uint64_t after_seq, const void** slot_out, uint64_t* seq_out) {
+  if (!c || !slot_out || !seq_out) return BIT1_ERR_INVALID_ARG;
+  if (!c->ring) return BIT1_ERR_STATE;
+  for (;;) {
+    int best = -1;
+    uint64_t bs = after_seq;
+    for (int k = 0; k < c->nslots; ++k) {
+      if (c->slot_state[k].load(std::memory_order_acquire) != kSlotReady) continue;
+      const uint64_t q = c->slot_seq[k].load(std::memory_order_acquire);
+      if (q > bs) { bs = q; best = k; }
+    }
+    if (best < 0) return BIT1_ERR_STATE;   // nothing newer than after_seq yet
+    int expect = kSlotReady;
+    if (c->slot_state[best].compare_exchange_strong(expect, kSlotHeld, std::memory_order_acq_rel)) {
+      *slot_out = c->ring + (size_t)best * c->slot_bytes;
+      *seq_out = bs;
+      return BIT1_OK;
+    }
+    // the producer took it back for the next snapshot in the meantime: look again
+  }
+}
+
+bit1_status bit1_stream_release(bit1_ctx* c, uint64_t seq) {
+  if (!c) return BIT1_ERR_INVALID_ARG;
+  if (!c->ring) return BIT1_ERR_STATE;
+  for (int k = 0; k < c->nslots; ++k)
+    if (c->slot_state[k].load(std::memory_order_acquire) == kSlotHeld && c->slot_seq[k].load() == seq) {
+      c->slot_state[k].store(kSlotFree, std::memory_order_release);
+      return BIT1_OK;
+    }
+  return BIT1_ERR_INVALID_ARG;
 }
 
 }  // extern "C"

@@ -37,7 +37,6 @@ __global__ void k_gen_begin(const __grid_constant__ Params P, unsigned* hdr) {
   st->ovf_count = 0u;
   st->ovf_valid = 0u;
   st->general_steps += 1ull;
-  for (int e = 0; e < kMaxR + 2; ++e) st->excess[e] = 0ull;
   hdr[kGenTotal] = 0u;
 }
 

@@ -417,6 +417,28 @@ __device__ void grid_radix_sort(cg::grid_group& grid, const Params& P, unsigned 
   }
 }
 
+// The next step's window radius (reading R-win), from pass A's excess counts: the smallest radius that leaves no more
+// than one far mover per four tiles among the particles landing within R_max cells of their tile's old range -- a
+// wider window costs every tile two more row entries per cell of radius, a far mover costs a side-list record, a
+// sort key and a scattered placement.  Farther ones are far movers under every radius and do not bear on the choice.
+__device__ void choose_radius(const Params& P, DevState* st, unsigned n) {
+  int Rn = 1;
+  if (P.R_fixed >= 0) {
+    Rn = P.R_fixed;
+  } else {
+    const unsigned long long thr = (unsigned long long)(n >> 12);
+    unsigned long long beyond = 0;   // particles landing r+1 .. R_max cells outside
+    Rn = P.R_max;
+    for (int r = P.R_max - 1; r >= 1; --r) {
+      beyond += st->excess[r + 1];
+      if (beyond > thr) break;
+      Rn = r;
+    }
+  }
+  st->R_next = (unsigned)Rn;
+  for (int e = 0; e < kMaxR + 2; ++e) st->excess[e] = 0;
+}
+
 // k_mid: cooperative launch, one CTA per SM at most.
 //   phase 0          side list: births get their pids in (parent, kind) order, the list is ordered by (cell, class,
 //                    order), every cell's group joins the cell's count.  Short lists: CTA 0, in shared memory; long
@@ -445,7 +467,10 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
   if (M > P.ovf_cap) {
     // the side list did not fit: nothing of this step is committed (pass A has only counted); the host takes the
     // step through the general path.  Every CTA sees the same count, so the whole grid leaves here.
-    if (b == 0 && threadIdx.x == 0) st->stalled = 1u;
+    if (b == 0 && threadIdx.x == 0) {
+      st->stalled = 1u;
+      choose_radius(P, st, n);   // pass A's counts are complete: the step after the general one gets a fitting window
+    }
     return;
   }
   const unsigned long long ord_mask = (1ull << P.ord_bits) - 1ull;
@@ -702,28 +727,8 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
       }
     }
   }
-  // the next step's window radius (reading R-win): the smallest radius that leaves no more than one far mover per
-  // four tiles among the particles that stay inside the domain -- a wider window costs every tile two more row
-  // entries per cell of radius, a far mover costs a side-list record, a sort key and a scattered placement
-  if (gt == 0) {
-    int Rn = 1;
-    if (P.R_fixed >= 0) {
-      Rn = P.R_fixed;
-    } else {
-      // beyond = particles landing r+1 .. R_max cells outside their tile's old range (farther ones are far movers
-      // under every radius and do not bear on the choice)
-      const unsigned long long thr = (unsigned long long)(n >> 12);
-      unsigned long long beyond = 0;
-      Rn = P.R_max;
-      for (int r = P.R_max - 1; r >= 1; --r) {
-        beyond += st->excess[r + 1];
-        if (beyond > thr) break;
-        Rn = r;
-      }
-    }
-    st->R_next = (unsigned)Rn;
-    for (int e = 0; e < kMaxR + 2; ++e) st->excess[e] = 0;
-  }
+  // (a scan on behalf of load, restart or the general path has no excess counts to go by: the radius stays)
+  if (gt == 0 && do_colscan) choose_radius(P, st, n);
 }
 
 // ---------------------------------------------------------------------------------------------
