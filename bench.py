@@ -512,6 +512,89 @@ def run_sweep(args):
             torch.cuda.empty_cache()
 
 
+def run_stream_overlap(args):
+    """profiles/r2_stream_overlap.md: ms/step of the configuration alone, with bit1_checkpoint (staged) every K steps and
+    with bit1_stream_publish every K steps while a consumer thread drains the ring; CUDA events around the whole leg."""
+    import threading
+
+    import torch
+
+    from paper_2606_28534_b200.binding import Bit1
+
+    torch.cuda.set_device(0)
+    w, wname = _workload(args.config, args.scale, 0)
+    sim = Bit1(w, device="cuda:0", checkpoint_staging=True)
+    sim.load()
+    sim.step(args.warmup)
+    sim.sync()
+    total = args.steps
+
+    def timed(every, what):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        with torch.cuda.stream(sim.compute_stream):
+            ev0.record(sim.compute_stream)
+            done = 0
+            while done < total:
+                k = min(every or total, total - done)
+                sim.step(k)
+                done += k
+                if every and what == "checkpoint":
+                    sim.checkpoint(blob)
+                elif every and what == "stream":
+                    sim.stream_publish()
+            ev1.record(sim.compute_stream)
+        sim.sync()
+        wall = time.perf_counter() - t0
+        sim.checkpoint_wait()
+        return ev0.elapsed_time(ev1) / total, 1e3 * wall / total
+
+    base_ev, base_wall = timed(0, None)
+    print(json.dumps({"workload": wname, "leg": "steps only", "steps": total, "ms_per_step_events": round(base_ev, 4),
+                      "ms_per_step_wall": round(base_wall, 4)}), flush=True)
+    blob = torch.empty(sim.checkpoint_size(), dtype=torch.uint8).pin_memory()
+    for every in args.every:
+        ev, wall = timed(every, "checkpoint")
+        print(json.dumps({"workload": wname, "leg": f"bit1_checkpoint (staged) every {every} steps", "steps": total,
+                          "snapshot_GB": round(sim.checkpoint_size() / 1e9, 2), "ms_per_step_events": round(ev, 4),
+                          "ms_per_step_wall": round(wall, 4), "overhead_wall_pct": round(100 * (wall / base_wall - 1), 2)}),
+              flush=True)
+    del blob
+    slot = (sim.stream_slot_size() + 255) // 256 * 256
+    ring = torch.empty(2 * slot, dtype=torch.uint8).pin_memory()
+    sim.stream_open(ring, 2)
+    seen, stop = [], threading.Event()
+
+    def consumer():
+        last = 0
+        while True:
+            got = sim.stream_acquire(last)
+            if got is None:
+                if stop.is_set():
+                    return
+                time.sleep(0.001)
+                continue
+            last, snap = got
+            # a consumer in the paper's sense: per-species density profile from the counts per cell
+            seen.append((snap["step"], [int(r["counts"].sum()) for r in snap["species"]]))
+            sim.stream_release(last)
+
+    t = threading.Thread(target=consumer)
+    t.start()
+    for every in args.every:
+        n_seen = len(seen)
+        ev, wall = timed(every, "stream")
+        print(json.dumps({"workload": wname, "leg": f"bit1_stream_publish every {every} steps + consumer thread",
+                          "steps": total, "slot_GB": round(slot / 1e9, 2), "ms_per_step_events": round(ev, 4),
+                          "ms_per_step_wall": round(wall, 4), "overhead_wall_pct": round(100 * (wall / base_wall - 1), 2),
+                          "snapshots_consumed": len(seen) - n_seen}), flush=True)
+    stop.set()
+    t.join()
+    sim.stream_close()
+    sim.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -529,11 +612,15 @@ def main():
     ap.add_argument("--radius", type=int, default=None, help="pin the sort-window radius (default: adaptive)")
     ap.add_argument("--radius-max", type=int, default=0)
     ap.add_argument("--side-list", type=int, default=0, help="side-list capacity (entries)")
-    ap.add_argument("--sweep", default=None, choices=["far-movers"], help="print the far-mover sweep instead of the bench line")
+    ap.add_argument("--sweep", default=None, choices=["far-movers", "stream"],
+                    help="print the far-mover sweep / the checkpoint-overlap table instead of the bench line")
+    ap.add_argument("--every", type=int, nargs="+", default=[200, 100, 50], help="--sweep stream: snapshot intervals")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3
-    if args.sweep:
+    if args.sweep == "stream":
+        run_stream_overlap(args)
+    elif args.sweep:
         run_sweep(args)
     elif args.impl == "reference":
         run_reference(args)

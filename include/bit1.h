@@ -58,6 +58,7 @@ typedef enum {
 /* sticky device flag bits (bit1_moments.flags) */
 #define BIT1_FLAG_CAPACITY 1u  /* births beyond capacity were dropped (SURVEY 8(c) "A") */
 #define BIT1_FLAG_ESCAPE 2u    /* a particle crossed more than one domain length (reading A21) */
+#define BIT1_FLAG_CHECK 16u    /* checked build (libbit1_checked.so): an index check in a kernel failed; see bit1_moments */
 #define BIT1_FLAG_PID_WRAP 8u  /* the 32-bit particle-id counter wrapped: newborn particles share random streams with old ones */
 
 /* species process flags */
@@ -134,7 +135,9 @@ typedef struct {
   uint64_t recycled;                  /* wall-recycling events (NEXT-2) */
   uint64_t general_steps;             /* steps that took the general path (side list beyond its capacity) */
   uint32_t window_radius;             /* sort-window radius, in cells, that the next step will use */
-  uint32_t _pad;
+  uint32_t check_failures;            /* checked builds only: index checks that failed (flag BIT1_FLAG_CHECK) ... */
+  uint32_t check_line, _pad;          /* ... source line of the first one in its kernel file ... */
+  int64_t check_index, check_limit;   /* ... and the index and bound it saw */
   double *density[BIT1_MAX_SPECIES];  /* HOST, optional (NULL to skip), ng entries each, m^-3 */
 } bit1_moments;
 
@@ -286,6 +289,12 @@ bit1_status bit1_profile(bit1_ctx *ctx, int enable);
 bit1_status bit1_get_profile(bit1_ctx *ctx, double ms[4], uint64_t *steps);
 /* Kernels launched by this context since create (bench.py's gpu_launches). */
 uint64_t bit1_launch_count(bit1_ctx *ctx);
+/* 1 for libbit1_checked.so (the same sources built with -DBIT1_CHECKED: every index the step kernels compute from
+ * particle data is compared with its bound before use; profiles/r2_sanitizer.md), 0 for the shipped library. */
+int bit1_build_is_checked(void);
+/* Checked build: runs one deliberately out-of-range index through the check on the device and returns BIT1_OK iff it
+ * was caught and recorded (the record is cleared again).  BIT1_ERR_STATE in the shipped library. */
+bit1_status bit1_check_selftest(bit1_ctx *ctx);
 
 #ifdef __cplusplus
 }

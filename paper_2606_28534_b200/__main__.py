@@ -12,7 +12,28 @@ from __future__ import annotations
 
 import argparse
 import json
+import os
 import time
+
+
+def plan_stops(step: int, last: int, dmpstep: int = 0, report: int = 0, mvstep: int = 0):
+    """The step counts at which the run has to come back to the host: the multiples of every interval that lie in
+    (step, last], and `last` itself.  Sorted, each once."""
+    stops = {last} if last > step else set()
+    for every in (dmpstep, report, mvstep):
+        if every > 0:
+            stops.update(range((step // every + 1) * every, last + 1, every))
+    return sorted(s for s in stops if s > step)
+
+
+def write_atomic(path: str, data) -> None:
+    """Write the checkpoint next to `path` and rename it over it: a crash in mid-write leaves the previous file."""
+    tmp = path + ".part"
+    with open(tmp, "wb") as f:
+        f.write(memoryview(data))
+        f.flush()
+        os.fsync(f.fileno())
+    os.replace(tmp, path)
 
 
 def main():
@@ -49,41 +70,44 @@ def main():
     sim.set_smoothing(args.smooth)
     if args.mvflag > 0:
         sim.set_averaging(args.mvflag, max(args.mvstep, args.mvflag))
-    blob = torch.empty(sim.checkpoint_size(), dtype=torch.uint8).pin_memory() if (args.dmpstep > 0 or args.restart) else None
+    blob = torch.empty(sim.checkpoint_size(), dtype=torch.uint8).pin_memory() if args.dmpstep > 0 else None
     if args.restart:
-        blob.copy_(torch.from_numpy(np.fromfile(args.restart, dtype=np.uint8)))
-        sim.restart(blob)
+        sim.restart(torch.from_numpy(np.fromfile(args.restart, dtype=np.uint8)))
     else:
         sim.load()
     step = sim.get_moments()["step"]
-    stops = set([last])
-    for every in (args.dmpstep, args.report, args.mvstep if args.mvflag > 0 else 0):
-        if every > 0:
-            stops.update(range((step // every + 1) * every, last + 1, every))
     t0 = time.perf_counter()
     units = 0
-    for stop in sorted(s for s in stops if s > step):
-        n_before = sim.n_live()
-        sim.step(stop - step)
-        units += n_before * (stop - step)
-        step = stop
-        if args.dmpstep > 0 and step % args.dmpstep == 0:
-            sim.checkpoint_wait()           # the previous blob must be on disk before it is overwritten
-            sim.checkpoint(blob)            # snapshot now, copy to the host while the next steps run
+    pending = 0   # bytes of a checkpoint whose copy to the host is still in flight
+
+    def finish_checkpoint():
+        nonlocal pending
+        if pending:
             sim.checkpoint_wait()
             if args.dump:
-                blob.numpy().tofile(args.dump)
+                write_atomic(args.dump, blob.numpy()[:pending])
+            pending = 0
+
+    for stop in plan_stops(step, last, args.dmpstep, args.report, args.mvstep if args.mvflag > 0 else 0):
+        n_before = sim.n_live()
+        sim.step(stop - step)               # enqueued; returns at once
+        units += n_before * (stop - step)
+        step = stop
+        finish_checkpoint()                 # the previous snapshot lands and goes to disk while these steps run
+        if args.dmpstep > 0 and step % args.dmpstep == 0:
+            pending = sim.checkpoint(blob)  # snapshot on the device now, copy out behind the steps that follow
         if args.report > 0 and step % args.report == 0 or step == last:
             m = sim.get_moments()
             print(json.dumps({"step": m["step"], "n_live": m["n_live"], "count": m["count"].tolist(),
                               "kinetic_J": m["kinetic_J"].tolist(), "field_J": m["field_J"],
                               "wall_count": m["wall_count"].tolist(), "births": m["births"],
-                              "recycled": m["recycled"], "flags": m["flags"]}))
+                              "recycled": m["recycled"], "general_steps": m["general_steps"], "flags": m["flags"]}))
         if args.mvflag > 0 and args.mvstep > 0 and step % args.mvstep == 0:
             d, f, cnt, at = sim.get_average()
             if cnt:
                 print(json.dumps({"average_over_steps": cnt, "latched_at": at, "phi_mid_V": float(f[len(f) // 2] / cnt),
                                   "mean_deposit_per_species": (d.sum(axis=1) / cnt).tolist()}))
+    finish_checkpoint()
     sim.sync(check_flags=False)
     dt = time.perf_counter() - t0
     print(json.dumps({"workload": w.name, "steps_run": step, "wall_s": dt,

@@ -52,7 +52,9 @@ class bit1_moments(C.Structure):
                 ("births", C.c_uint64), ("reinject", C.c_uint64), ("candidates", C.c_uint64 * MAX_SPECIES),
                 ("events", (C.c_uint64 * 3) * MAX_SPECIES), ("far_movers", C.c_uint64),
                 ("max_far_movers_per_step", C.c_uint64), ("recycled", C.c_uint64), ("general_steps", C.c_uint64),
-                ("window_radius", C.c_uint32), ("_pad", C.c_uint32), ("density", c_f64p * MAX_SPECIES)]
+                ("window_radius", C.c_uint32), ("check_failures", C.c_uint32), ("check_line", C.c_uint32),
+                ("_pad", C.c_uint32), ("check_index", C.c_int64), ("check_limit", C.c_int64),
+                ("density", c_f64p * MAX_SPECIES)]
 
 
 class bit1_stream_header(C.Structure):
@@ -148,6 +150,10 @@ def load_library(path: Optional[str] = None):
     L.bit1_get_profile.argtypes = [vp, C.POINTER(C.c_double * 4), C.POINTER(C.c_uint64)]
     L.bit1_launch_count.restype = C.c_uint64
     L.bit1_launch_count.argtypes = [vp]
+    L.bit1_build_is_checked.restype = C.c_int
+    L.bit1_build_is_checked.argtypes = []
+    L.bit1_check_selftest.restype = C.c_int
+    L.bit1_check_selftest.argtypes = [vp]
     if path is None:
         _lib = L
     return L
@@ -183,14 +189,15 @@ class Bit1:
 
     def __init__(self, w, *, checkpoint_staging: bool = False, device: str = "cuda:0", side_stream: bool = True,
                  direct_launch: bool = False, window_radius_max: int = 0, window_radius: Optional[int] = None,
-                 side_list_capacity: int = 0):
-        """window_radius: None = adaptive (default), k = pinned to k cells; the other keywords are bit1_options fields."""
+                 side_list_capacity: int = 0, lib=None):
+        """window_radius: None = adaptive (default), k = pinned to k cells; the other keywords are bit1_options fields.
+        lib: a library from load_library(path), e.g. the checked build (default: the shipped libbit1.so)."""
         import torch
 
         if not torch.cuda.is_available():
             raise RuntimeError("libbit1 needs a CUDA device (no CPU fallback)")
         self._torch = torch
-        self.lib = load_library()
+        self.lib = lib if lib is not None else load_library()
         self.w = w
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
@@ -331,7 +338,9 @@ class Bit1:
                    reinject=int(m.reinject), candidates=np.array(m.candidates[:ns], np.uint64),
                    events=np.array([list(m.events[k][:]) for k in range(ns)], np.uint64),
                    far_movers=int(m.far_movers), max_far_movers_per_step=int(m.max_far_movers_per_step),
-                   recycled=int(m.recycled), general_steps=int(m.general_steps), window_radius=int(m.window_radius))
+                   recycled=int(m.recycled), general_steps=int(m.general_steps), window_radius=int(m.window_radius),
+                   check_failures=int(m.check_failures), check_line=int(m.check_line),
+                   check_index=int(m.check_index), check_limit=int(m.check_limit))
         if density:
             out["density"] = dens
         return out
@@ -469,6 +478,9 @@ class Bit1:
         steps = C.c_uint64()
         _check(self.lib.bit1_get_profile(self.h, C.byref(ms), C.byref(steps)), "bit1_get_profile")
         return dict(zip(("pass_a", "mid", "pass_b", "field"), [float(v) for v in ms])), int(steps.value)
+
+    def check_selftest(self):
+        _check(self.lib.bit1_check_selftest(self.h), "bit1_check_selftest")
 
     def launch_count(self) -> int:
         return int(self.lib.bit1_launch_count(self.h))

@@ -23,7 +23,7 @@ static __device__ __noinline__ void emit_record(const Params& P, unsigned long l
                                          double vz, unsigned pid, int sp) {
   const unsigned slot = atomicAdd(&P.st->ovf_count, 1u);
   if (slot >= P.ovf_cap) return;   // k_mid sees ovf_count > ovf_cap and stalls the step: the general path takes it
-  P.ovf_key[slot] = key;
+  P.ovf_key[BIT1_CHECK(P.st, slot, P.ovf_cap)] = key;
   OvfRec r;
   r.x = x; r.vx = vx; r.vy = vy; r.vz = vz; r.pid = pid; r.sp = (unsigned)sp;
   P.ovf_rec[slot] = r;

@@ -515,6 +515,32 @@ void bit1_destroy(bit1_ctx* c) {
 
 uint64_t bit1_launch_count(bit1_ctx* c) { return c ? c->launches : 0; }
 
+int bit1_build_is_checked(void) {
+#ifdef BIT1_CHECKED
+  return 1;
+#else
+  return 0;
+#endif
+}
+
+bit1_status bit1_check_selftest(bit1_ctx* c) {
+  if (!c) return BIT1_ERR_INVALID_ARG;
+#ifdef BIT1_CHECKED
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  DevState before, after;
+  CUDA_OK(cudaMemcpy(&before, c->P.st, sizeof(DevState), cudaMemcpyDeviceToHost));
+  launch_check_selftest(c->P, c->cs);
+  CUDA_OK(cudaStreamSynchronize(c->cs));
+  CUDA_OK(cudaMemcpy(&after, c->P.st, sizeof(DevState), cudaMemcpyDeviceToHost));
+  const bool caught = after.check_count == before.check_count + 1 && (after.flags & kFlagCheck) &&
+                      (before.check_count != 0 || (after.check_idx == 5 && after.check_limit == 3));
+  CUDA_OK(cudaMemcpy(c->P.st, &before, sizeof(DevState), cudaMemcpyHostToDevice));   // clear the record again
+  return caught ? BIT1_OK : BIT1_ERR_CUDA;
+#else
+  return BIT1_ERR_STATE;
+#endif
+}
+
 bit1_status bit1_profile(bit1_ctx* c, int enable) {
   if (!c) return BIT1_ERR_INVALID_ARG;
   c->profiling = enable != 0;
@@ -920,6 +946,8 @@ bit1_status bit1_get_moments(bit1_ctx* c, bit1_moments* out) {
   out->births = h.births; out->reinject = h.reinject; out->recycled = h.recycled;
   out->far_movers = h.far_movers; out->max_far_movers_per_step = h.max_far_movers;
   out->general_steps = h.general_steps; out->window_radius = h.R_cur;
+  out->check_failures = h.check_count; out->check_line = h.check_line; out->_pad = 0;
+  out->check_index = h.check_idx; out->check_limit = h.check_limit;
   bool any = false;
   for (int k = 0; k < P.ns; ++k) any = any || dens_out[k];
   if (any) {

@@ -375,6 +375,14 @@ int launch_fill_cells(const Params& P, const Particles& cur, cudaStream_t s) {
   return 1;
 }
 
+#ifdef BIT1_CHECKED
+__global__ void k_check_selftest(const __grid_constant__ Params P, int* sink) {
+  int table[3] = {1, 2, 3};
+  sink[0] = table[BIT1_CHECK(P.st, 5 + (int)threadIdx.x, 3)];   // out of range: caught, redirected to entry 0
+}
+void launch_check_selftest(const Params& P, cudaStream_t s) { k_check_selftest<<<1, 1, 0, s>>>(P, P.scan_part); }
+#endif
+
 int launch_moments(const Params& P, const Particles& cur, double* partial, double* out, cudaStream_t s) {
   k_moments_partial<<<kMomBlocks, 256, 0, s>>>(P, cur, partial);
   k_moments_final<<<1, 1024, 0, s>>>(P, partial, kMomBlocks, out);

@@ -17,6 +17,9 @@ int launch_scan_u32(unsigned* a, size_t n, unsigned* tmp, cudaStream_t s);
 // stable radix sort of n (key, value) word pairs laid out as load_scratch_bytes(stride) describes
 int launch_radix_sort_u32(unsigned n, unsigned stride, int bits, void* scratch, cudaStream_t s, unsigned** keys,
                           unsigned** vals);
+#ifdef BIT1_CHECKED
+void launch_check_selftest(const Params& P, cudaStream_t s);
+#endif
 // cell[i] = cell_of(x[i]) for the live particles
 int launch_fill_cells(const Params& P, const Particles& cur, cudaStream_t s);
 // out: [kMaxSpecies*3] = (count, sum v^2, sum vx) per species, then sum g_j E_j^2

@@ -34,7 +34,7 @@ constexpr unsigned long long kInvalidKey = ~0ull;
 // sort-window radius: adaptive per step (DevState::R_cur) up to Params::R_max <= kMaxR
 constexpr int kMaxR = (BIT1_WCAP - 8) / 2;
 
-constexpr unsigned kFlagCapacity = 1u, kFlagEscape = 2u, kFlagPidWrap = 8u;
+constexpr unsigned kFlagCapacity = 1u, kFlagEscape = 2u, kFlagPidWrap = 8u, kFlagCheck = 16u;
 constexpr unsigned kElastic = 1u, kIonise = 2u, kCx = 4u, kIonProduct = 8u, kElectronProduct = 16u,
                    kTargetMaxwellian = 32u;
 constexpr int kSrcNone = 0, kSrcSelf = 1, kSrcPair = 2;
@@ -88,6 +88,9 @@ struct DevState {
   // everything beyond kMaxR); filled by pass A, read and cleared by k_mid when it chooses R_next
   unsigned long long excess[kMaxR + 2];
   unsigned long long general_steps;   // steps that took the general path
+  // checked builds (-DBIT1_CHECKED, see BIT1_CHECK below): the first failed index check and how many failed
+  unsigned check_count, check_line;
+  long long check_idx, check_limit;
   unsigned long long wall_count[2][kMaxSpecies];
   long long wall_charge[2];
   unsigned long long nu_overflow, dir_fallback, escape, births, reinject, recycled;
@@ -156,6 +159,31 @@ struct Params {
   unsigned *tmp_idx, *tmp2_idx;
   SpeciesP sp[kMaxSpecies];
 };
+
+// Checked build (build.py --checked -> libbit1_checked.so; profiles/r2_sanitizer.md): every index the step kernels
+// compute from particle data -- shared-memory histogram, window, deposit and counter slots, scatter destinations,
+// side-list slots, banded-row offsets, cell indices, radix destinations -- is compared with its bound before use.  A
+// failure is recorded (first site and value, count), raises the sticky flag kFlagCheck and the access is redirected to
+// index 0 instead of corrupting memory.  The shipped library compiles the checks away.
+#ifdef BIT1_CHECKED
+__device__ __noinline__ inline void check_fail(DevState* st, int line, long long idx, long long limit) {
+  if (atomicAdd(&st->check_count, 1u) == 0u) {
+    st->check_line = (unsigned)line;
+    st->check_idx = idx;
+    st->check_limit = limit;
+  }
+  atomicOr(&st->flags, kFlagCheck);
+}
+template <class T, class U>
+__device__ __forceinline__ T checked_index(DevState* st, int line, T idx, U limit) {
+  if ((unsigned long long)(long long)idx < (unsigned long long)(long long)limit) return idx;
+  check_fail(st, line, (long long)idx, (long long)limit);
+  return (T)0;
+}
+#define BIT1_CHECK(st, idx, limit) checked_index((st), __LINE__, (idx), (limit))
+#else
+#define BIT1_CHECK(st, idx, limit) (idx)
+#endif
 
 // Rows never overlap: clo is monotone in the tile index and a row holds chi - clo + 1 + 2R <= the distance to the
 // next row's start.  Offsets are multiples of 4 words so that a row can be fetched by a 16-byte bulk copy.

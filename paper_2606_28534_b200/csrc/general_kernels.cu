@@ -114,7 +114,7 @@ __global__ void __launch_bounds__(kGenThreads) k_gen_push(const __grid_constant_
       for (int kind = 0; kind < 4; ++kind) {
         if (!((sink.mask >> kind) & 1u)) continue;
         if (r < room) {   // reading R-W: the first capacity - N births in (parent, kind) order exist, the rest do not
-          const unsigned slot = n + r;
+          const unsigned slot = BIT1_CHECK(st, n + r, P.capacity);
           const BirthRec& b = sink.rec[kind];
           cur.x[slot] = b.x; cur.vx[slot] = b.vx; cur.vy[slot] = b.vy; cur.vz[slot] = b.vz;
           cur.pid[slot] = next_pid + r;
@@ -166,7 +166,7 @@ __global__ void __launch_bounds__(kGenThreads) k_gen_gather(const __grid_constan
                                                             Particles nxt, const unsigned* perm) {
   const unsigned n = P.st->n_next;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-    const unsigned j = perm[i];
+    const unsigned j = BIT1_CHECK(P.st, perm[i], P.capacity);
     nxt.x[i] = cur.x[j]; nxt.vx[i] = cur.vx[j]; nxt.vy[i] = cur.vy[j]; nxt.vz[i] = cur.vz[j];
     nxt.pid[i] = cur.pid[j]; nxt.sp[i] = cur.sp[j];
   }

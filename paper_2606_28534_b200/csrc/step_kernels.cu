@@ -157,7 +157,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
               cn[r] = -2;  // placed through the side list
               // see phase 3 (a tile too sparse for its window sends cells of its own old range here: no excess)
               const int ex = max(clo - c, c - chi);
-              if (ex >= 2) atomicAdd(&s_exc[min(ex, kMaxR + 1)], 1u);
+              if (ex >= 2) atomicAdd(&s_exc[BIT1_CHECK(P.st, min(ex, kMaxR + 1), kMaxR + 2)], 1u);
             }
           }
         }
@@ -172,10 +172,11 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
       if (have && cn[r] >= 0) key = (unsigned)(cn[r] - tw.wlo);
       {
         const unsigned eb = __ballot_sync(0xffffffffu, (evm >> r) & 1u);
-        if (lane == 0) P.evt[(base >> 5) + (unsigned)(warp * kItems + r)] = eb;
+        if (lane == 0) P.evt[BIT1_CHECK(P.st, (base >> 5) + (unsigned)(warp * kItems + r), (unsigned)(P.max_tiles + 1) * (kTile / 32))] = eb;
       }
       const unsigned m = __match_any_sync(0xffffffffu, key);
-      if (!(key & 0x80000000u) && lane == __ffs(m) - 1) s_hist[key * kWarps + warp] += (unsigned)__popc(m);
+      if (!(key & 0x80000000u) && lane == __ffs(m) - 1)
+        s_hist[BIT1_CHECK(P.st, key, (unsigned)tw.W) * kWarps + warp] += (unsigned)__popc(m);
       __syncwarp();
     }
     // how far outside the tile's old cell range the windowed particles land: k_mid picks the next step's radius from
@@ -186,7 +187,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
       for (int r = 0; r < kItems; ++r) {
         const bool have = (unsigned)(warp * kWarpSpan + r * 32 + lane) < cnt;
         const int ex = max(clo - cn[r], cn[r] - chi);
-        if (have && cn[r] >= 0 && ex >= 2) atomicAdd(&s_exc[min(ex, kMaxR + 1)], 1u);
+        if (have && cn[r] >= 0 && ex >= 2) atomicAdd(&s_exc[BIT1_CHECK(P.st, min(ex, kMaxR + 1), kMaxR + 2)], 1u);
       }
     }
     if (evm) fence_proxy_async();   // only the slow path writes into the stage (generic proxy) before its reload
@@ -196,7 +197,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
     const size_t rowo = tile_row_offset(clo, tile, R);
     for (int k = threadIdx.x; k < tw.W; k += kThreads) {
       unsigned run = 0;
-      unsigned* pre = P.tile_pre + (rowo + (size_t)k) * kWarps;
+      unsigned* pre = P.tile_pre + BIT1_CHECK(P.st, rowo + (size_t)k, tile_row_words(P.nc, P.max_tiles, P.R_max)) * kWarps;
 #pragma unroll
       for (int w = 0; w < kWarps; ++w) {
         const unsigned t = s_hist[k * kWarps + w];
@@ -402,8 +403,8 @@ __device__ void grid_radix_sort(cg::grid_group& grid, const Params& P, unsigned 
       old = __shfl_sync(0xffffffffu, old, leader);
       if (have) {
         const unsigned dst = old + (unsigned)__popc(m & lt);
-        k1[dst] = key;
-        v1[dst] = val;
+        k1[BIT1_CHECK(P.st, dst, n)] = key;
+        v1[dst < n ? dst : 0u] = val;
       }
       __syncwarp();
     }
@@ -528,8 +529,8 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
       const bool first = p == 0 || (P.ovf_key[p - 1] >> cshift) != c;
       unsigned long long nk = 0;
       const bool last = p + 1 == (size_t)Mv || ((nk = P.ovf_key[p + 1]) >> cshift) != c;
-      if (first) P.ovf_lb[c] = (int)p;
-      if (last) P.ovf_ub[c] = (int)p + 1;
+      if (first) P.ovf_lb[BIT1_CHECK(st, c, (unsigned long long)P.nc)] = (int)p;
+      if (last) P.ovf_ub[BIT1_CHECK(st, c, (unsigned long long)P.nc)] = (int)p + 1;
       if (cls == 0 && (last || ((nk >> oshift) & 3ull) != 0ull)) P.ovf_before[c] = (int)p + 1;   // made relative below
     }
     grid_or_cta_sync(grid);
@@ -688,7 +689,7 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
     const int c = (int)(key >> cshift);
     const unsigned cls = (unsigned)((key >> oshift) & 3ull);
     const int rel = P.ovf_dst[p];
-    P.ovf_dst[p] = (cls == 0 ? P.cell_start[c] : P.cell_start[c + 1]) + rel;
+    P.ovf_dst[p] = (cls == 0 ? P.cell_start[BIT1_CHECK(st, c, P.nc)] : P.cell_start[BIT1_CHECK(st, c, P.nc) + 1]) + rel;
   }
   if (do_colscan && n > 0) {
     const int R = (int)st->R_cur;
@@ -715,7 +716,7 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
           const int k = c - tw.wlo;
           in[q] = tb4 + q <= t1 && k >= 0 && k < tw.W;
           off[q] = tile_row_offset(d[q].x, min(tb4 + q, t1), R) + (size_t)(in[q] ? k : 0);
-          cnt[q] = in[q] ? P.tile_hist[off[q]] : 0u;
+          cnt[q] = in[q] ? P.tile_hist[BIT1_CHECK(st, off[q], tile_row_words(nc, P.max_tiles, P.R_max))] : 0u;
         }
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
@@ -842,7 +843,8 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
       old[r] = 0;
-      if (key[r] >= 0 && lane == __ffs(m[r]) - 1) old[r] = atomicAdd(&wc[key[r]], (unsigned)__popc(m[r]));
+      if (key[r] >= 0 && lane == __ffs(m[r]) - 1)
+        old[r] = atomicAdd(&wc[BIT1_CHECK(P.st, key[r], tw.W)], (unsigned)__popc(m[r]));
       __syncwarp();
     }
     // deposit (SURVEY 8(c) "D"): one shared-memory atomic pair per (cell, species) run of the warp
@@ -855,8 +857,9 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
         const unsigned m2 = __match_any_sync(0xffffffffu, mk2);
         const unsigned sa = __reduce_add_sync(m2, a[r]);
         if (valid && lane == __ffs(m2) - 1) {
-          atomicAdd(&s_dens[key[r] * ns + sp[r]], (unsigned)__popc(m2) * (unsigned)s_sp[sp[r]].Q - sa);
-          atomicAdd(&s_dens[(key[r] + 1) * ns + sp[r]], sa);
+          atomicAdd(&s_dens[BIT1_CHECK(P.st, key[r] * ns + sp[r], kDensWords)],
+                    (unsigned)__popc(m2) * (unsigned)s_sp[sp[r]].Q - sa);
+          atomicAdd(&s_dens[BIT1_CHECK(P.st, (key[r] + 1) * ns + sp[r], kDensWords)], sa);
         }
       }
     } else {
@@ -877,7 +880,7 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
       const unsigned o = __shfl_sync(0xffffffffu, old[r], __ffs(m[r]) - 1);
       if (key[r] >= 0) {
         const int off = warp * kWarpSpan + r * 32 + lane;
-        const unsigned dst = o + (unsigned)__popc(m[r] & lt);
+        const unsigned dst = BIT1_CHECK(P.st, o + (unsigned)__popc(m[r] & lt), P.st->n_next);
         nxt.x[dst] = x[r]; nxt.vx[dst] = vx[r]; nxt.vy[dst] = vy[r]; nxt.vz[dst] = vz[r];
         nxt.pid[dst] = S->pid[off]; nxt.sp[dst] = (unsigned char)sp[r];
       }
@@ -903,8 +906,8 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
   // side list: far movers and births go to the slots k_mid computed for them
   const unsigned Mv = P.st->ovf_valid;
   for (unsigned p = blockIdx.x * kThreads + threadIdx.x; p < Mv; p += G * kThreads) {
-    const int dst = P.ovf_dst[p];
-    const OvfRec rec = P.ovf_rec[P.ovf_idx[p]];
+    const int dst = BIT1_CHECK(P.st, P.ovf_dst[p], P.st->n_next);
+    const OvfRec rec = P.ovf_rec[BIT1_CHECK(P.st, P.ovf_idx[p], P.ovf_cap)];
     const int c = (int)(P.ovf_key[p] >> P.cell_shift);
     nxt.x[dst] = rec.x; nxt.vx[dst] = rec.vx; nxt.vy[dst] = rec.vy; nxt.vz[dst] = rec.vz;
     nxt.pid[dst] = rec.pid; nxt.sp[dst] = (unsigned char)rec.sp;

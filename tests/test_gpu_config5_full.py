@@ -180,8 +180,9 @@ def test_config5_full_size_checkpoint_every_50_steps_and_bit_identical_restart()
               "far_movers_per_step": far, "n_final": want["n"], "bit_identical": got == want,
               "sampled_particles_bit_identical_to_oracle": n_sampled,
               "all_elements_bit_identical_to_oracle_after_2_steps": True, "oracle_load_and_2_steps_s": t_oracle}
-    os.makedirs("gpurun_out", exist_ok=True)
-    with open("gpurun_out/config5_full.json", "w") as f:
-        json.dump(report, f, indent=1)
+    if os.environ.get("BIT1_REPORT_DIR"):   # where to leave the figures (profiles/r1e_config5_full.md was made from them)
+        os.makedirs(os.environ["BIT1_REPORT_DIR"], exist_ok=True)
+        with open(os.path.join(os.environ["BIT1_REPORT_DIR"], "config5_full.json"), "w") as f:
+            json.dump(report, f, indent=1)
     print(json.dumps(report))
     assert got == want, "restarted run differs from the uninterrupted one"

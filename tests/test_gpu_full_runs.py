@@ -19,8 +19,11 @@ REPORT = {}
 
 
 def _save():
-    os.makedirs("gpurun_out", exist_ok=True)
-    with open("gpurun_out/full_runs.json", "w") as f:
+    out = os.environ.get("BIT1_REPORT_DIR")   # where to leave the figures; nothing is written without it
+    if not out:
+        return
+    os.makedirs(out, exist_ok=True)
+    with open(os.path.join(out, "full_runs.json"), "w") as f:
         json.dump(REPORT, f, indent=1)
 
 
