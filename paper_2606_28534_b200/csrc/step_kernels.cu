@@ -11,6 +11,8 @@
 // whose side list does not fit stalls (DevState::stalled) and is taken by general_kernels.cu instead.
 #include <cooperative_groups.h>
 
+#include <type_traits>
+
 #include "advance.cuh"
 #include "step_kernels.h"
 
@@ -110,6 +112,10 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
     int e0, ne;
     const double* Eptr = e_window(clo, chi, e0, ne) ? (S->E - e0) : P.E;
 
+    // The tile body, compiled twice: for whole tiles (every tile but the store's last) without the per-particle
+    // "is this slot live" predicates, and for the ragged last tile with them.
+    auto tile_body = [&](auto full_c) {
+    constexpr bool kFull = decltype(full_c)::value;
     // phase 1
     int cn[kItems];
     double x[kItems], vx[kItems], vy[kItems], vz[kItems];
@@ -118,7 +124,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
       const int off = warp * kWarpSpan + r * 32 + lane;
-      const bool have = (unsigned)off < cnt;
+      const bool have = kFull || (unsigned)off < cnt;
       const int sp = have ? (int)S->sp[off] : 0;
       const SpeciesP& s = s_sp[sp];
       x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off];
@@ -167,7 +173,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
       const int off = warp * kWarpSpan + r * 32 + lane;
-      const bool have = (unsigned)off < cnt;
+      const bool have = kFull || (unsigned)off < cnt;
       unsigned key = 0x80000000u | (unsigned)lane;  // unique: matches nobody
       if (have && cn[r] >= 0) key = (unsigned)(cn[r] - tw.wlo);
       {
@@ -185,12 +191,15 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
     if (R > 1) {
 #pragma unroll
       for (int r = 0; r < kItems; ++r) {
-        const bool have = (unsigned)(warp * kWarpSpan + r * 32 + lane) < cnt;
+        const bool have = kFull || (unsigned)(warp * kWarpSpan + r * 32 + lane) < cnt;
         const int ex = max(clo - cn[r], cn[r] - chi);
         if (have && cn[r] >= 0 && ex >= 2) atomicAdd(&s_exc[BIT1_CHECK(P.st, min(ex, kMaxR + 1), kMaxR + 2)], 1u);
       }
     }
     if (evm) fence_proxy_async();   // only the slow path writes into the stage (generic proxy) before its reload
+    };   // tile_body
+    if (cnt == (unsigned)kTile) tile_body(std::true_type{});
+    else tile_body(std::false_type{});
     __syncthreads();
     // per window cell: the warps' counts become exclusive prefixes (tile_pre, read back by pass B: this warp's
     // particles for that cell start that far into the tile's run), their sum is the tile's count
@@ -796,22 +805,37 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     int e0, ne;
     const double* Eptr = e_window(d.x, d.y, e0, ne) ? (S->E - e0) : P.E;
 
+    // The tile body, compiled twice: for whole tiles (every tile but the store's last) without the per-particle
+    // "is this slot live" predicates, and for the ragged last tile with them.
+    auto tile_body = [&](auto full_c) {
+    constexpr bool kFull = decltype(full_c)::value;
     // phase 1: new state of every particle of the tile
     double x[kItems], vx[kItems], vy[kItems], vz[kItems];
     int key[kItems];        // window-relative new cell, or -1 when the particle is not placed by this tile
     unsigned evm = 0;
+    unsigned spk = 0;       // the kItems species tags, one byte each
+    // pass A's event bits of this warp's kItems rows (set for live slots only)
+    unsigned evw[kItems];
+    if constexpr (kItems == 4) {
+      const uint4 e4 = *reinterpret_cast<const uint4*>(&S->evt[warp * kItems]);
+      evw[0] = e4.x; evw[1] = e4.y; evw[2] = e4.z; evw[3] = e4.w;
+    } else {
+#pragma unroll
+      for (int r = 0; r < kItems; ++r) evw[r] = S->evt[warp * kItems + r];
+    }
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
       const int off = warp * kWarpSpan + r * 32 + lane;
-      const bool have = (unsigned)off < cnt;
+      const bool have = kFull || (unsigned)off < cnt;
       x[r] = S->x[off]; vx[r] = S->vx[off]; vy[r] = S->vy[off]; vz[r] = S->vz[off];
       int c = have ? cell_of(P, x[r]) : d.x;
       const int sp = have ? (int)S->sp[off] : 0;
-      if (have && ((S->evt[warp * kItems + r] >> lane) & 1u)) evm |= 1u << r;
+      spk |= (unsigned)sp << (8 * r);
+      evm |= ((evw[r] >> lane) & 1u) << r;
       push_fast(P, s_sp[sp], Eptr, c, x[r], vx[r], vy[r], vz[r]);
       c = cell_of(P, x[r]);
       const int k = c - tw.wlo;
-      key[r] = (have && c >= 0 && k >= 0 && k < tw.W) ? k : -1;
+      key[r] = (have && k >= 0 && k < tw.W) ? k : -1;
     }
     // phase 1b: the particles pass A flagged take the full step again, side effects off
     if (evm) {
@@ -833,18 +857,25 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     unsigned m[kItems], a[kItems], old[kItems];
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
-      const int off = warp * kWarpSpan + r * 32 + lane;
       const bool valid = key[r] >= 0;
-      sp[r] = valid ? (int)S->sp[off] : 0;
+      sp[r] = (int)((spk >> (8 * r)) & 0xffu);
       m[r] = __match_any_sync(0xffffffffu, valid ? (unsigned)key[r] : (0x80000000u | (unsigned)lane));
       a[r] = valid ? deposit_a(x[r], tw.wlo + key[r], P.inv_dx, (unsigned)s_sp[sp[r]].Q) : 0u;
     }
-    // the leader of every (item, cell) group reserves the group's destinations; items in order (stability)
+    // the leader of every (item, cell) group reserves the group's destinations; items in order (stability).  The
+    // counters are this warp's own: plain loads and stores, ordered by the warp barrier
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
       old[r] = 0;
-      if (key[r] >= 0 && lane == __ffs(m[r]) - 1)
-        old[r] = atomicAdd(&wc[BIT1_CHECK(P.st, key[r], tw.W)], (unsigned)__popc(m[r]));
+      if (key[r] >= 0 && lane == __ffs(m[r]) - 1) {
+        unsigned* slot = &wc[BIT1_CHECK(P.st, key[r], tw.W)];
+#ifdef BIT1_EXP_ATOMIC_WC
+        old[r] = atomicAdd(slot, (unsigned)__popc(m[r]));
+#else
+        old[r] = *slot;
+        *slot = old[r] + (unsigned)__popc(m[r]);
+#endif
+      }
       __syncwarp();
     }
     // deposit (SURVEY 8(c) "D"): one shared-memory atomic pair per (cell, species) run of the warp
@@ -886,6 +917,9 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
       }
     }
     if (evm) fence_proxy_async();   // only the slow path writes into the stage (generic proxy) before its reload
+    };   // tile_body
+    if (cnt == (unsigned)kTile) tile_body(std::true_type{});
+    else tile_body(std::false_type{});
     __syncthreads();  // the stage may be overwritten; the tile's deposit is complete
     if (threadIdx.x == 0 && tnext < ntiles)
       issue_tile(P, cur, S, &bar[it & 1], tnext, dn, R, true, true, true);

@@ -170,6 +170,45 @@ def test_all_particles_in_one_cell_and_sparse_cells():
     g.close()
 
 
+@pytest.mark.parametrize("bc_cfg", [1, 2])
+def test_deposit_at_nodes_cell_edges_and_the_last_representable_position(bc_cfg):
+    """The CIC split at its edges (SURVEY 8(c) "D": F = 0 for f <= 0, 2^32 - 1 for f >= 1, else trunc(f 2^32)): particles
+    exactly on nodes, one ulp either side of them, at 0, and at the last doubles below L, where x * inv_dx rounds up to nc,
+    the cell clamps to nc - 1 and f becomes 1.  Cold particles in a field-free box: the load-time deposit and the fused
+    deposit of the following steps see the same positions.  The CUDA path takes F with one saturating conversion."""
+    w = W.make_config(bc_cfg, scale=1 / 16)
+    # a cell size for which the last double below L times fl(1/dx) rounds up to nc: the clamp edge f = 1 exists
+    for f in np.random.default_rng(3).random(2000):
+        d = w.dx * (1.0 + 0.5 * f)
+        if np.nextafter(w.nc * d, -np.inf) * (1.0 / d) >= w.nc:
+            w.dx = float(d)
+            break
+    L = w.nc * w.dx
+    assert np.nextafter(L, -np.inf) * (1.0 / w.dx) - (w.nc - 1) >= 1.0, "no clamp edge for this dx"
+    if w.bc:
+        w.src_lo, w.src_hi = 0.25 * L, 0.75 * L
+    nodes = np.arange(w.nc, dtype=np.float64) * w.dx
+    xs = [nodes, np.nextafter(nodes, np.inf), np.nextafter(nodes[1:], -np.inf), nodes + 0.5 * w.dx,
+          nodes + w.dx * 2.0 ** -33, nodes + w.dx * (1.0 - 2.0 ** -33)]
+    top = [L]
+    for _ in range(64):
+        top.append(np.nextafter(top[-1], -np.inf))
+    xs.append(np.array(top[1:]))
+    x = np.concatenate(xs)
+    x = x[(x >= 0.0) & (x < L)]
+    rng = np.random.default_rng(5)
+    x = np.ascontiguousarray(rng.permutation(x))
+    n = x.shape[0]
+    w.x = x
+    w.sp = np.ascontiguousarray((np.arange(n) % len(w.species)).astype(np.uint8))
+    for k in ("vx", "vy", "vz"):
+        setattr(w, k, np.zeros(n))
+    for steps in (0, 2):
+        g, o = run_pair(w, steps)
+        assert assert_state_equal(g, o, where=f"deposit edges, bc {w.bc}, {steps} steps")
+        g.close()
+
+
 @pytest.mark.parametrize("cfg,scale,kw", [(1, 1 / 4, {}), (3, 1 / 256, dict(n0_scale=300.0, pair_source=True))])
 def test_side_list_longer_than_one_cta_sorts_over_the_grid(cfg, scale, kw):
     """A plasma 40 times hotter than the grid was sized for: nearly every particle leaves its tile's window, so the
