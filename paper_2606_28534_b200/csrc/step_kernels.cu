@@ -745,7 +745,7 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
 // Pass B.  A tile arrives with its particles, its window of E, its row of tile_base (destination of the tile's
 // first particle of every window cell, from k_mid) and its row of tile_pre (how many of those belong to
 // earlier warps, from pass A).  So every warp knows where its own particles of each cell start and works alone:
-// phase 1 recomputes the push (V2) as straight-line arithmetic, phase 1b redoes the particles pass A flagged
+// phase 1 recomputes the push as straight-line arithmetic, phase 1b redoes the particles pass A flagged
 // through the full advance(), phase 2 ranks inside (warp, cell), deposits and scatters.  One CTA barrier per
 // tile (it frees the stage); the tile's deposit is double-buffered and flushed after it.
 __global__ void __launch_bounds__(kThreads, kMinBlocks)
@@ -1183,13 +1183,15 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
   }
   tot = block_sum_128(tot, s_warp);
   wsum = block_sum_128(wsum, s_warp);
-  if (threadIdx.x == 0) { part[b] = tot; part[G + b] = wsum; }
-  __threadfence();
-  grid_or_cta_sync(grid);
-  tot = 0; wsum = 0;
-  for (int i = threadIdx.x; i < G; i += kFieldThreads) { tot += part[i]; wsum += part[G + i]; }
-  tot = block_sum_128(tot, s_warp);
-  wsum = block_sum_128(wsum, s_warp);
+  if (G > 1) {   // (a one-CTA grid already holds the totals)
+    if (threadIdx.x == 0) { part[b] = tot; part[G + b] = wsum; }
+    __threadfence();
+    grid_or_cta_sync(grid);
+    tot = 0; wsum = 0;
+    for (int i = threadIdx.x; i < G; i += kFieldThreads) { tot += part[i]; wsum += part[G + i]; }
+    tot = block_sum_128(tot, s_warp);
+    wsum = block_sum_128(wsum, s_warp);
+  }
   if (b == 0 && threadIdx.x == 0) st->rho_total = (long long)(tot >> (2 * smooth));   // the filter conserves charge
   const bool frozen = st->freeze_field != 0;
   if (!frozen) {
@@ -1201,27 +1203,33 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
     int per = (jmax + G - 1) / G;
     per = ((per + unit - 1) / unit) * unit;
     const int j_lo = min(1 + b * per, jmax + 1), j_hi = min(j_lo + per - 1, jmax);
-    // phase B
-    i128 A = 0, C = 0;
-    field_range<false>(P, R, Kphi, KE, j_lo, j_hi, tot, Tn, (i128)0, (i128)0, s_warp, &A, &C);
-    if (threadIdx.x == 0) { part[2 * G + b] = A; part[3 * G + b] = C; }
-    __threadfence();
-    grid_or_cta_sync(grid);
-    // phase C: S_{j_lo-1} = sum of A over earlier CTAs; T_{j_lo} = sum over earlier CTAs of (len * S_before + C)
-    i128 myA = 0, myLen = 0, myC = 0;
-    if ((int)threadIdx.x < G) {
-      const int i = threadIdx.x;
-      myA = part[2 * G + i];
-      myC = part[3 * G + i];
-      const int lo = min(1 + i * per, jmax + 1), hi = min(lo + per - 1, jmax);
-      myLen = hi >= lo ? hi - lo + 1 : 0;
+    i128 carryS = 0, carryT = 0, Send = 0;
+    if (G > 1) {
+      // phase B
+      i128 A = 0, C = 0;
+      field_range<false>(P, R, Kphi, KE, j_lo, j_hi, tot, Tn, (i128)0, (i128)0, s_warp, &A, &C);
+      if (threadIdx.x == 0) { part[2 * G + b] = A; part[3 * G + b] = C; }
+      __threadfence();
+      grid_or_cta_sync(grid);
+      // phase C: S_{j_lo-1} = sum of A over earlier CTAs; T_{j_lo} = sum over earlier CTAs of (len * S_before + C)
+      i128 myA = 0, myLen = 0, myC = 0;
+      if ((int)threadIdx.x < G) {
+        const int i = threadIdx.x;
+        myA = part[2 * G + i];
+        myC = part[3 * G + i];
+        const int lo = min(1 + i * per, jmax + 1), hi = min(lo + per - 1, jmax);
+        myLen = hi >= lo ? hi - lo + 1 : 0;
+      }
+      i128 dummy;
+      const i128 Sbefore = block_exclusive_scan_128(myA, s_warp, &dummy);            // S at the start of CTA i
+      const i128 term = ((int)threadIdx.x < b) ? myLen * Sbefore + myC : (i128)0;
+      carryT = block_sum_128(term, s_warp);
+      carryS = block_sum_128(((int)threadIdx.x < b) ? myA : (i128)0, s_warp);
+      Send = block_sum_128(myA, s_warp);                                              // S_jmax
+    } else if (!bc) {
+      // one CTA owns every element: no carries; S_jmax = sum_{j=1}^{nc-1} (nc R_j - tot) = tot - nc R_0
+      Send = tot - (i128)nc * (i128)R[0];
     }
-    i128 dummy;
-    const i128 Sbefore = block_exclusive_scan_128(myA, s_warp, &dummy);            // S at the start of CTA i
-    const i128 term = ((int)threadIdx.x < b) ? myLen * Sbefore + myC : (i128)0;
-    const i128 carryT = block_sum_128(term, s_warp);
-    const i128 carryS = block_sum_128(((int)threadIdx.x < b) ? myA : (i128)0, s_warp);
-    const i128 Send = block_sum_128(myA, s_warp);                                    // S_jmax
     if (b == 0 && threadIdx.x == 0) {
       // node 0
       P.phi[0] = Kphi * dbl128((i128)0);
@@ -1305,7 +1313,12 @@ cudaError_t configure_kernels() {
   return cudaFuncSetAttribute(k_pass_b, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::b_total);
 }
 
+#ifndef BIT1_ONE_CTA_CELLS
+#define BIT1_ONE_CTA_CELLS 1024
+#endif
 static int coop_grid(int work_items, int per_cta) {
+  // small grids: one CTA loops over its chunks with CTA barriers only, instead of a few CTAs meeting at grid barriers
+  if (work_items <= BIT1_ONE_CTA_CELLS + 1) return 1;
   int g = (work_items + per_cta - 1) / per_cta;
   if (g < 1) g = 1;
   const int cap = sm_count() < kFieldThreads ? sm_count() : kFieldThreads;   // co-resident, and G <= threads
@@ -1318,7 +1331,11 @@ int launch_mid(const Params& P, const Particles& cur, int2* desc_out, int do_col
   int2* dout = desc_out;
   int dc = do_colscan;
   void* args[] = {&Pc, &pc, &dout, &dc};
-  cudaLaunchCooperativeKernel((const void*)k_mid, dim3(coop_grid(P.nc, kMidThreads)), dim3(kMidThreads), args, 0, s);
+  const int g = coop_grid(P.nc, kMidThreads);
+  // a one-CTA grid synchronises with CTA barriers only (grid_or_cta_sync): a plain launch, without the cooperative
+  // launch's residency bookkeeping on the stream
+  if (g == 1) k_mid<<<1, kMidThreads, 0, s>>>(Pc, pc, dout, dc);
+  else cudaLaunchCooperativeKernel((const void*)k_mid, dim3(g), dim3(kMidThreads), args, 0, s);
   return 1;
 }
 
@@ -1326,8 +1343,9 @@ int launch_field(const Params& P, int commit_step, cudaStream_t s) {
   Params Pc = P;
   int cs = commit_step;
   void* args[] = {&Pc, &cs};
-  cudaLaunchCooperativeKernel((const void*)k_field, dim3(coop_grid(P.ng, kFieldThreads * kFieldItems)),
-                              dim3(kFieldThreads), args, 0, s);
+  const int g = coop_grid(P.ng, kFieldThreads * kFieldItems);
+  if (g == 1) k_field<<<1, kFieldThreads, 0, s>>>(Pc, cs);
+  else cudaLaunchCooperativeKernel((const void*)k_field, dim3(g), dim3(kFieldThreads), args, 0, s);
   return 1;
 }
 
