@@ -221,7 +221,7 @@ struct bit1_ctx {
   int cur;
   char* ws;
   cudaStream_t cs, ss;
-  cudaEvent_t ev_snap, ev_done, ev_load0, ev_load1;
+  cudaEvent_t ev_snap, ev_done, ev_load0, ev_load1[3];
   bool ckpt_pending, staging, loaded;
   bool ckpt_reads_live;   // a checkpoint without staging is still copying out of the live half of the store
   uint64_t launches, cfg_hash, cfg_hash_base;
@@ -488,7 +488,7 @@ bit1_status bit1_create(const bit1_grid* g, const bit1_species* sp, int ns, doub
   ok = ok && cudaEventCreateWithFlags(&c->ev_snap, cudaEventDisableTiming) == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&c->ev_done, cudaEventDisableTiming) == cudaSuccess;
   ok = ok && cudaEventCreateWithFlags(&c->ev_load0, cudaEventDisableTiming) == cudaSuccess;
-  ok = ok && cudaEventCreateWithFlags(&c->ev_load1, cudaEventDisableTiming) == cudaSuccess;
+  for (int k = 0; k < 3; ++k) ok = ok && cudaEventCreateWithFlags(&c->ev_load1[k], cudaEventDisableTiming) == cudaSuccess;
   if (!ok) { delete c; return BIT1_ERR_CUDA; }
   *out = c;
   return BIT1_OK;
@@ -508,7 +508,7 @@ void bit1_destroy(bit1_ctx* c) {
   cudaEventDestroy(c->ev_snap);
   cudaEventDestroy(c->ev_done);
   cudaEventDestroy(c->ev_load0);
-  cudaEventDestroy(c->ev_load1);
+  for (int k = 0; k < 3; ++k) cudaEventDestroy(c->ev_load1[k]);
   for (cudaEvent_t e : c->prof_ev) cudaEventDestroy(e);
   delete c;
 }
@@ -794,9 +794,11 @@ bit1_status bit1_load_particles(bit1_ctx* c, uint64_t n, const double* x, const 
       CUDA_OK(cudaStreamWaitEvent(c->ss, c->ev_load0, 0));
     }
     CUDA_OK(cudaMemcpyAsync(in.vx, vx, n * 8, kind, vs));
+    if (split) CUDA_OK(cudaEventRecord(c->ev_load1[0], c->ss));
     CUDA_OK(cudaMemcpyAsync(in.vy, vy, n * 8, kind, vs));
+    if (split) CUDA_OK(cudaEventRecord(c->ev_load1[1], c->ss));
     CUDA_OK(cudaMemcpyAsync(in.vz, vz, n * 8, kind, vs));
-    if (split) CUDA_OK(cudaEventRecord(c->ev_load1, c->ss));
+    if (split) CUDA_OK(cudaEventRecord(c->ev_load1[2], c->ss));
   }
   const unsigned n32 = (unsigned)n;
   // validate before anything indexes by species or cell: a bad species tag or a position outside [0, L) is refused

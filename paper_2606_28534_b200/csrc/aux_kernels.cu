@@ -235,12 +235,18 @@ __global__ void __launch_bounds__(256) k_radix_scatter(const unsigned* keys, con
   }
 }
 
-__global__ void __launch_bounds__(256) k_gather(Particles in, Particles out, const unsigned* perm, unsigned n) {
+// out[i] = in[perm[i]], split so that each velocity array can follow its own host-to-device copy: positions, ids and
+// species (on the device before the sort starts) in one kernel, one kernel per velocity component
+__global__ void __launch_bounds__(256) k_gather_keys(Particles in, Particles out, const unsigned* perm, unsigned n) {
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
     const unsigned j = perm[i];
-    out.x[i] = in.x[j]; out.vx[i] = in.vx[j]; out.vy[i] = in.vy[j]; out.vz[i] = in.vz[j];
-    out.pid[i] = in.pid[j]; out.sp[i] = in.sp[j];
+    out.x[i] = in.x[j]; out.pid[i] = in.pid[j]; out.sp[i] = in.sp[j];
   }
+}
+__global__ void __launch_bounds__(256) k_gather_f64(const double* __restrict__ in, double* __restrict__ out,
+                                                    const unsigned* __restrict__ perm, unsigned n) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    out[i] = in[perm[i]];
 }
 
 // Stable LSD radix sort (8-bit digits over key bits [0, bits)) of n (key, value) pairs of 32-bit words.
@@ -269,7 +275,7 @@ int launch_radix_sort_u32(unsigned n, unsigned stride, int bits, void* scratch, 
 }
 
 int launch_load_sort(const Params& P, const Particles& in, const Particles& out, unsigned n, int have_pid,
-                     void* scratch, cudaStream_t s, cudaEvent_t before_gather) {
+                     void* scratch, cudaStream_t s, const cudaEvent_t* velocity_ready) {
   if (n == 0) return 0;
   int launches = 0;
   unsigned* k0 = reinterpret_cast<unsigned*>(scratch);
@@ -280,9 +286,15 @@ int launch_load_sort(const Params& P, const Particles& in, const Particles& out,
   while ((1ll << bits) < (long long)P.nc) ++bits;
   unsigned *ks = nullptr, *vs = nullptr;
   launches += launch_radix_sort_u32(n, P.capacity, bits, scratch, s, &ks, &vs);
-  if (before_gather) cudaStreamWaitEvent(s, before_gather, 0);   // the velocity arrays arrive on another stream
-  k_gather<<<148 * 8, 256, 0, s>>>(in, out, vs, n);
-  return launches + 1;
+  k_gather_keys<<<148 * 8, 256, 0, s>>>(in, out, vs, n);
+  // the velocity arrays arrive on another stream, one event each: a component is gathered as soon as it has landed
+  const double* vin[3] = {in.vx, in.vy, in.vz};
+  double* vout[3] = {out.vx, out.vy, out.vz};
+  for (int k = 0; k < 3; ++k) {
+    if (velocity_ready) cudaStreamWaitEvent(s, velocity_ready[k], 0);
+    k_gather_f64<<<148 * 8, 256, 0, s>>>(vin[k], vout[k], vs, n);
+  }
+  return launches + 4;
 }
 
 size_t load_scratch_bytes(unsigned capacity) {

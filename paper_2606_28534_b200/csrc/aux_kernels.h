@@ -8,9 +8,10 @@ namespace bit1 {
 int launch_load_validate(const Params& P, const Particles& in, unsigned n, cudaStream_t s);
 int launch_state_validate(const Params& P, const Particles& p, unsigned n, cudaStream_t s);
 // validate + cell index + general stable sort by cell of `in` (n particles) into `out`
-// before_gather: NULL, or an event the final gather waits for (arrays other than x, sp, pid still being copied)
+// velocity_ready: NULL, or three events (vx, vy, vz still being copied on another stream): each component's gather waits
+// for its own
 int launch_load_sort(const Params& P, const Particles& in, const Particles& out, unsigned n, int have_pid,
-                     void* scratch, cudaStream_t s, cudaEvent_t before_gather);
+                     void* scratch, cudaStream_t s, const cudaEvent_t* velocity_ready);
 size_t load_scratch_bytes(unsigned capacity);
 // exclusive scan of n words in place (tmp: n / 4096 + 2 words)
 int launch_scan_u32(unsigned* a, size_t n, unsigned* tmp, cudaStream_t s);
