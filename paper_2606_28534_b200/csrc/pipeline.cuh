@@ -50,6 +50,16 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
 // orders this thread's generic-proxy accesses to shared memory before later async-proxy (TMA) writes
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// Split CTA barrier (named barriers 1 and 2): every warp but one announces that it is done with a tile and goes on; the
+// one warp that owns the tile's hand-over waits for all of them.  Shared-memory accesses made before bar.arrive are
+// visible after the matching bar.sync.
+__device__ __forceinline__ void named_bar_arrive(int id, int nthreads) {
+  asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
 // window of E that a tile with old cells [clo, chi] gathers from: E[clo .. chi+1]
 __device__ __forceinline__ bool e_window(int clo, int chi, int& e0, int& ne) {
   e0 = clo & ~1;

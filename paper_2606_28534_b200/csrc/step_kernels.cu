@@ -201,10 +201,11 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
     if (cnt == (unsigned)kTile) tile_body(std::true_type{});
     else tile_body(std::false_type{});
     __syncthreads();
+    const int kfirst = threadIdx.x, kstep = kThreads;
     // per window cell: the warps' counts become exclusive prefixes (tile_pre, read back by pass B: this warp's
     // particles for that cell start that far into the tile's run), their sum is the tile's count
     const size_t rowo = tile_row_offset(clo, tile, R);
-    for (int k = threadIdx.x; k < tw.W; k += kThreads) {
+    for (int k = kfirst; k < tw.W; k += kstep) {
       unsigned run = 0;
       unsigned* pre = P.tile_pre + BIT1_CHECK(P.st, rowo + (size_t)k, tile_row_words(P.nc, P.max_tiles, P.R_max)) * kWarps;
 #pragma unroll
@@ -746,8 +747,11 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
 // first particle of every window cell, from k_mid) and its row of tile_pre (how many of those belong to
 // earlier warps, from pass A).  So every warp knows where its own particles of each cell start and works alone:
 // phase 1 recomputes the push as straight-line arithmetic, phase 1b redoes the particles pass A flagged
-// through the full advance(), phase 2 ranks inside (warp, cell), deposits and scatters.  One CTA barrier per
-// tile (it frees the stage); the tile's deposit is double-buffered and flushed after it.
+// through the full advance(), phase 2 ranks inside (warp, cell), deposits and scatters.  The hand-over of a tile
+// (flush of its double-buffered deposit, reload of its stage) is a split barrier: seven warps announce that they are
+// done (bar.arrive) and go on to the tile waiting in the other stage; the eighth, taking turns, waits for them
+// (bar.sync), flushes and reloads.  A warp can run one tile ahead of the slowest, never two: the stage it would need
+// is only reloaded after every warp has left it, which also keeps the mbarrier phases and the two barrier ids apart.
 __global__ void __launch_bounds__(kThreads, kMinBlocks)
 k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
   constexpr int kWarpSpan = 32 * kItems;
@@ -792,7 +796,8 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     const unsigned cnt = min((unsigned)kTile, n - base);
     int2 dn = make_int2(0, 0);
     const int tnext = tile + 2 * G;
-    if (threadIdx.x == 0 && tnext < ntiles) dn = cur.desc[tnext];
+    const bool owner = warp == (it & (kWarps - 1));
+    if (owner && lane == 0 && tnext < ntiles) dn = cur.desc[tnext];
     mbar_wait(&bar[it & 1], (unsigned)(it >> 1) & 1u);
     // the stage's descriptor is only valid once its barrier has completed
     const int2 d = S->d;
@@ -920,11 +925,13 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     };   // tile_body
     if (cnt == (unsigned)kTile) tile_body(std::true_type{});
     else tile_body(std::false_type{});
-    __syncthreads();  // the stage may be overwritten; the tile's deposit is complete
-    if (threadIdx.x == 0 && tnext < ntiles)
-      issue_tile(P, cur, S, &bar[it & 1], tnext, dn, R, true, true, true);
+    // one warp (taking turns) hands the tile over: it waits for the others, flushes the tile's deposit and only then
+    // reloads the stage (the tile after next deposits into this buffer once its load has landed)
+    if (!owner) { named_bar_arrive(1 + (it & 1), kThreads); continue; }
+    named_bar_sync(1 + (it & 1), kThreads);
+    const int kfirst = lane, kstep = 32;
     if (P.dep_u32) {
-      for (int k = threadIdx.x; k < ns * (tw.W + 1); k += kThreads) {
+      for (int k = kfirst; k < ns * (tw.W + 1); k += kstep) {
         const unsigned v = s_dens[k];
         if (v) {
           s_dens[k] = 0;
@@ -935,6 +942,8 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
         }
       }
     }
+    __syncwarp();
+    if (lane == 0 && tnext < ntiles) issue_tile(P, cur, S, &bar[it & 1], tnext, dn, R, true, true, true);
   }
 
   // side list: far movers and births go to the slots k_mid computed for them
