@@ -1277,6 +1277,12 @@ bit1_status bit1_stream_publish(bit1_ctx* c, uint64_t* seq_out) {
     c->slot_state[slot].store(kSlotFilling, std::memory_order_release);
   }
   if (slot < 0) return BIT1_ERR_CAPACITY;   // every slot is held by the consumer
+  // a failure below (a CUDA error, a slot too small) hands the claimed slot back instead of leaving it "filling" for good
+  struct SlotClaim {
+    std::atomic<int>* state;
+    bool armed;
+    ~SlotClaim() { if (armed) state->store(kSlotFree, std::memory_order_release); }
+  } claim{&c->slot_state[slot], true};
   const Params& P = c->P;
   const int nc = P.nc, ns = P.ns;
   char* sg = c->ws + c->lay.scratch;   // device staging, payload layout (offsets relative to the end of the header)
@@ -1302,7 +1308,7 @@ bit1_status bit1_stream_publish(bit1_ctx* c, uint64_t* seq_out) {
     hd.off_vy[s] = hsz + o; o += align_up(n * 8);
     hd.off_vz[s] = hsz + o; o += align_up(n * 8);
     hd.off_pid[s] = hsz + o; o += align_up(n * 4);
-    if (hsz + o > c->slot_bytes) { c->slot_state[slot].store(kSlotFree); return BIT1_ERR_CAPACITY; }
+    if (hsz + o > c->slot_bytes) return BIT1_ERR_CAPACITY;
     CUDA_OK(cudaMemcpyAsync(sg + (hd.off_counts[s] - hsz), ex + 256, (size_t)nc * 4, cudaMemcpyDeviceToDevice, c->cs));
     Particles out;
     memset(&out, 0, sizeof(out));
@@ -1323,6 +1329,7 @@ bit1_status bit1_stream_publish(bit1_ctx* c, uint64_t* seq_out) {
   if (o) CUDA_OK(cudaMemcpyAsync(hs + hsz, sg, o, cudaMemcpyDeviceToHost, c->ss));
   c->done_arg[slot].c = c; c->done_arg[slot].slot = slot; c->done_arg[slot].seq = seq;
   CUDA_OK(cudaLaunchHostFunc(c->ss, stream_done_cb, &c->done_arg[slot]));
+  claim.armed = false;   // from here on the host function publishes the slot
   CUDA_OK(cudaEventRecord(c->ev_done, c->ss));
   c->ckpt_pending = true;
   if (seq_out) *seq_out = seq;

@@ -239,6 +239,33 @@ def test_capacity_hit_matches_oracle_and_raises_the_sticky_flag():
     g.close()
 
 
+def test_particle_id_counter_wrap_matches_the_oracle_and_raises_the_flag():
+    """Reading R-pid: ids are 32-bit on both sides.  Loaded with ids that end five short of 2^32, the ionisation births
+    of the next steps take ids that wrap through 0: the CUDA path hands out the same ids as the oracle (which has the
+    same counter and no flag) and raises BIT1_FLAG_PID_WRAP so that the shared random streams do not go unnoticed."""
+    from oracle.oracle import Oracle
+    from paper_2606_28534_b200.binding import Bit1, FLAG_PID_WRAP
+
+    w = W.make_config(3, scale=1 / 256, n0_scale=300.0)
+    pid = (np.arange(w.n, dtype=np.uint64) + (2 ** 32 - 5 - w.n)).astype(np.uint32)
+    g = Bit1(w)
+    g.load_particles(w.x, w.vx, w.vy, w.vz, w.sp, pid=pid)
+    o = Oracle(w, load=False)
+    o.load(w.x, w.vx, w.vy, w.vz, w.sp, pid=pid)
+    g.step(3)
+    o.step(3)
+    g.sync(check_flags=False)
+    m = g.get_moments()
+    assert m["births"] > 5, "the workload was meant to create more births than ids were left"
+    pg, po = g.get_particles(), o.particles()
+    for k in ("pid", "sp", "cell", "x", "vx", "vy", "vz"):
+        assert np.array_equal(pg[k], po[k]), k
+    assert m["next_pid"] == o.next_pid and m["next_pid"] < 2 ** 31
+    assert m["flags"] == (o.flagword | FLAG_PID_WRAP)
+    assert np.array_equal(g.get_rho(), o.rho())
+    g.close()
+
+
 @pytest.mark.parametrize("R", [0, 2, 4, 17, 60])
 def test_sort_window_radius_does_not_change_the_result(R):
     """Reading R-win: the radius only moves particles between the windowed path and the side list."""
