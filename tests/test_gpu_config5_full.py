@@ -4,7 +4,7 @@ oracle after 2 steps and 240 000 sampled particles after a third.
 
 Opt-in (BIT1_FULL_C5=1): it needs ~130 GB of HBM, ~130 GB of host memory and about eight minutes, which does not
 belong in the default `pytest -m gpu` run.  The result of the run made for this round is recorded in
-profiles/r1e_config5_full.md.  State digests are taken array by array (8 GB at a time) through the C ABI."""
+profiles/r2_full_runs.md (round 1: profiles/r1e_config5_full.md).  State digests are taken array by array (8 GB at a time) through the C ABI."""
 import ctypes as C
 import hashlib
 import json
@@ -180,7 +180,7 @@ def test_config5_full_size_checkpoint_every_50_steps_and_bit_identical_restart()
               "far_movers_per_step": far, "n_final": want["n"], "bit_identical": got == want,
               "sampled_particles_bit_identical_to_oracle": n_sampled,
               "all_elements_bit_identical_to_oracle_after_2_steps": True, "oracle_load_and_2_steps_s": t_oracle}
-    if os.environ.get("BIT1_REPORT_DIR"):   # where to leave the figures (profiles/r1e_config5_full.md was made from them)
+    if os.environ.get("BIT1_REPORT_DIR"):   # where to leave the figures (profiles/r2_full_runs.md was made from them)
         os.makedirs(os.environ["BIT1_REPORT_DIR"], exist_ok=True)
         with open(os.path.join(os.environ["BIT1_REPORT_DIR"], "config5_full.json"), "w") as f:
             json.dump(report, f, indent=1)
