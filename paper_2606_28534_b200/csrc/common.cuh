@@ -27,6 +27,7 @@ constexpr int kTile = kThreads * kItems;  // particles per tile (one TMA stage)
 constexpr int kWCap = BIT1_WCAP;          // max cells in a tile's window (smem histogram bins)
 constexpr int kWarps = kThreads / 32;
 static_assert(kWCap <= kThreads && (32 % kWarps == 0 || kWarps % 32 == 0), "pass geometry");
+static_assert((kWarps & (kWarps - 1)) == 0, "pass B rotates the tile hand-over among the warps by it & (kWarps - 1)");
 
 // side-list ("far mover" / birth) key: cell | cls(2) | ord(Params::ord_bits), packed so that the radix sort of a long
 // list only visits the bits in use (Params::key_bits)
