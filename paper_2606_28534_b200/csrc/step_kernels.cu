@@ -874,12 +874,8 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
       old[r] = 0;
       if (key[r] >= 0 && lane == __ffs(m[r]) - 1) {
         unsigned* slot = &wc[BIT1_CHECK(P.st, key[r], tw.W)];
-#ifdef BIT1_EXP_ATOMIC_WC
-        old[r] = atomicAdd(slot, (unsigned)__popc(m[r]));
-#else
         old[r] = *slot;
         *slot = old[r] + (unsigned)__popc(m[r]);
-#endif
       }
       __syncwarp();
     }
