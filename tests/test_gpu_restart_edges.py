@@ -100,6 +100,53 @@ def test_restart_rejects_a_blob_of_another_configuration():
     h.close()
 
 
+def test_restart_refuses_a_blob_whose_body_was_tampered_with_and_create_refuses_a_bad_source_interval():
+    """The blob's header and hash vouch for the configuration only: a species tag that does not exist, a position
+    outside the domain and positions out of cell order are caught on the device before anything indexes by them
+    (BIT1_ERR_CHECKPOINT, no device fault; the context can be loaded again).  bit1_create refuses re-injection
+    intervals that are empty or reach outside [0, L) when a species re-injects."""
+    import torch
+    from paper_2606_28534_b200.binding import Bit1, Bit1Error, ERR_CHECKPOINT, ERR_INVALID_ARG
+
+    w = W.make_config(2, scale=1 / 64)
+    g = Bit1(w)
+    g.load()
+    g.step(3)
+    blob = torch.empty(g.checkpoint_size(), dtype=torch.uint8).pin_memory()
+    written = g.checkpoint(blob)
+    g.checkpoint_wait()
+    n = g.n_live()
+    x = g.get_particles()["x"]
+    raw = blob.numpy()
+    sp_off = written - (n + 255) // 256 * 256          # the species tags are the blob's last section
+    x_off = raw[:written].tobytes().find(x[:4].tobytes())
+    assert x_off > 0 and x_off % 256 == 0, "the positions' section was not found"
+    for what in ("species", "position", "order"):
+        bad = blob.clone()
+        b = bad.numpy()
+        if what == "species":
+            b[sp_off + 3] = 200
+        elif what == "position":
+            b[x_off + 8 * 5: x_off + 8 * 6] = np.frombuffer(np.float64(-1.0).tobytes(), np.uint8)
+        else:   # the first and the last particle change places: no longer sorted by cell
+            first = b[x_off: x_off + 8].copy()
+            b[x_off: x_off + 8] = b[x_off + 8 * (n - 1): x_off + 8 * n]
+            b[x_off + 8 * (n - 1): x_off + 8 * n] = first
+        with pytest.raises(Bit1Error) as e:
+            g.restart(bad)
+        assert e.value.status == ERR_CHECKPOINT, what
+    g.restart(blob)   # the untouched blob still restarts, and the run goes on
+    g.step(2)
+    g.sync()
+    g.close()
+    L = w.nc * w.dx
+    for lo, hi in ((0.5 * L, 0.5 * L), (0.75 * L, 0.25 * L), (-0.1 * L, 0.5 * L), (0.5 * L, 1.5 * L)):
+        w.src_lo, w.src_hi = lo, hi
+        with pytest.raises(Bit1Error) as e:
+            Bit1(w)
+        assert e.value.status == ERR_INVALID_ARG, (lo, hi)
+
+
 def test_two_runs_give_identical_bits():
     w = W.make_config(3, scale=1 / 64, n0_scale=100.0)
     a, _ = None, None
