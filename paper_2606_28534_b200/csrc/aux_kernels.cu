@@ -2,6 +2,7 @@
 // cell-index fill (the store's cell array is cell_of(x) by construction and only materialised when asked for).
 // The load-time sort is a multi-pass LSD radix sort (8-bit digits) on (cell, original index); it is the
 // general counterpart of the banded single-scatter sort of the step kernels and is not timed.
+#include "block_ops.cuh"
 #include "aux_kernels.h"
 #include "device_math.cuh"
 
@@ -79,41 +80,19 @@ __global__ void __launch_bounds__(256) k_radix_hist(const unsigned* keys, unsign
 __global__ void __launch_bounds__(1024) k_scan_u32(unsigned* a, size_t n) {
   __shared__ unsigned s_warp[33];
   unsigned carry = 0;
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (size_t i0 = 0; i0 < n; i0 += 4096) {
     const size_t i = i0 + (size_t)threadIdx.x * 4;
     unsigned v[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) v[k] = i + k < n ? a[i + k] : 0u;
-    const unsigned t = v[0] + v[1] + v[2] + v[3];
-    unsigned inc = t;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const unsigned u = __shfl_up_sync(0xffffffffu, inc, d);
-      if (lane >= d) inc += u;
-    }
-    if (lane == 31) s_warp[warp] = inc;
-    __syncthreads();
-    if (warp == 0) {
-      const unsigned w = s_warp[lane];
-      unsigned winc = w;
-#pragma unroll
-      for (int d = 1; d < 32; d <<= 1) {
-        const unsigned u = __shfl_up_sync(0xffffffffu, winc, d);
-        if (lane >= d) winc += u;
-      }
-      s_warp[lane] = winc - w;
-      if (lane == 31) s_warp[32] = winc;
-    }
-    __syncthreads();
-    unsigned ex = carry + s_warp[warp] + inc - t;
+    unsigned chunk;
+    unsigned ex = carry + block_exclusive_scan<unsigned>(v[0] + v[1] + v[2] + v[3], s_warp, &chunk);
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       if (i + k < n) a[i + k] = ex;
       ex += v[k];
     }
-    carry += s_warp[32];
-    __syncthreads();
+    carry += chunk;
   }
 }
 
@@ -121,50 +100,22 @@ __global__ void __launch_bounds__(1024) k_scan_u32(unsigned* a, size_t n) {
 // every chunk scanned with its carry.  (The one-CTA k_scan_u32 took 12 ms per radix pass at 2e8 particles.)
 constexpr int kScanChunk = 4096;
 __global__ void __launch_bounds__(1024) k_scan_chunk_sums(const unsigned* a, size_t n, unsigned* sums) {
-  __shared__ unsigned s_warp[32];
+  __shared__ unsigned s_warp[33];
   const size_t i = (size_t)blockIdx.x * kScanChunk + (size_t)threadIdx.x * 4;
   unsigned t = 0;
 #pragma unroll
   for (int k = 0; k < 4; ++k) t += i + k < n ? a[i + k] : 0u;
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-  if ((threadIdx.x & 31) == 0) s_warp[threadIdx.x >> 5] = t;
-  __syncthreads();
-  if (threadIdx.x < 32) {
-    unsigned v = s_warp[threadIdx.x];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    if (threadIdx.x == 0) sums[blockIdx.x] = v;
-  }
+  t = block_sum<unsigned>(t, s_warp);
+  if (threadIdx.x == 0) sums[blockIdx.x] = t;
 }
 __global__ void __launch_bounds__(1024) k_scan_chunks(unsigned* a, size_t n, const unsigned* carry_in) {
   __shared__ unsigned s_warp[33];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const size_t i = (size_t)blockIdx.x * kScanChunk + (size_t)threadIdx.x * 4;
   unsigned v[4];
 #pragma unroll
   for (int k = 0; k < 4; ++k) v[k] = i + k < n ? a[i + k] : 0u;
-  const unsigned t = v[0] + v[1] + v[2] + v[3];
-  unsigned inc = t;
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const unsigned u = __shfl_up_sync(0xffffffffu, inc, d);
-    if (lane >= d) inc += u;
-  }
-  if (lane == 31) s_warp[warp] = inc;
-  __syncthreads();
-  if (warp == 0) {
-    const unsigned w = s_warp[lane];
-    unsigned winc = w;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const unsigned u = __shfl_up_sync(0xffffffffu, winc, d);
-      if (lane >= d) winc += u;
-    }
-    s_warp[lane] = winc - w;
-  }
-  __syncthreads();
-  unsigned ex = carry_in[blockIdx.x] + s_warp[warp] + inc - t;
+  unsigned chunk;
+  unsigned ex = carry_in[blockIdx.x] + block_exclusive_scan<unsigned>(v[0] + v[1] + v[2] + v[3], s_warp, &chunk);
 #pragma unroll
   for (int k = 0; k < 4; ++k) {
     if (i + k < n) a[i + k] = ex;

@@ -14,6 +14,7 @@
 #include <type_traits>
 
 #include "advance.cuh"
+#include "block_ops.cuh"
 #include "step_kernels.h"
 
 namespace cg = cooperative_groups;
@@ -293,54 +294,6 @@ __device__ __forceinline__ void grid_or_cta_sync(cg::grid_group& grid) {
   else { __threadfence(); grid.sync(); }
 }
 
-__device__ int block_exclusive_scan_int(int v, int* s_warp, int* total) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  int inc = v;
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const int t = __shfl_up_sync(0xffffffffu, inc, d);
-    if (lane >= d) inc += t;
-  }
-  if (lane == 31) s_warp[warp] = inc;
-  __syncthreads();
-  if (warp == 0) {
-    int w = lane < (int)(blockDim.x >> 5) ? s_warp[lane] : 0;
-    int winc = w;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const int t = __shfl_up_sync(0xffffffffu, winc, d);
-      if (lane >= d) winc += t;
-    }
-    s_warp[lane] = winc - w;
-    if (lane == 31) s_warp[32] = winc;
-  }
-  __syncthreads();
-  const int res = s_warp[warp] + inc - v;
-  *total = s_warp[32];
-  __syncthreads();
-  return res;
-}
-
-// block-wide sum of one int per thread (every thread gets it)
-__device__ int block_sum_int(int v, int* s_warp) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  if (lane == 0) s_warp[warp] = v;
-  __syncthreads();
-  int t = 0;
-  if (warp == 0) {
-    t = lane < (int)(blockDim.x >> 5) ? s_warp[lane] : 0;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-    if (lane == 0) s_warp[32] = t;
-  }
-  __syncthreads();
-  t = s_warp[32];
-  __syncthreads();
-  return t;
-}
-
 // Stable LSD radix sort (8-bit digits over key bits [0, nbits)) of n (key, val) pairs over the whole cooperative
 // grid; (k1, v1) is scratch of the same size; the result ends in (k0, v0).  Side lists of 1e5..1e7 entries (a hot
 // tail, a sheath start-up, a pinned small radius) cost a few passes over 12 B per entry instead of the
@@ -387,7 +340,7 @@ __device__ void grid_radix_sort(cg::grid_group& grid, const Params& P, unsigned 
       }
     }
     int dummy;
-    const int ex = block_exclusive_scan_int(tot, s_warp, &dummy);   // entries with a smaller digit, all CTAs
+    const int ex = block_exclusive_scan<int>(tot, s_warp, &dummy);   // entries with a smaller digit, all CTAs
     if (threadIdx.x < 256) {
       unsigned run = (unsigned)(ex + mine);
       for (int w = 0; w < kMidWarps; ++w) {
@@ -637,7 +590,7 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
   {
     int sum = 0;
     for (int c = c_lo + (int)threadIdx.x; c < c_hi; c += kMidThreads) sum += P.cell_count[c];
-    sum = block_sum_int(sum, s_warp);
+    sum = block_sum<int>(sum, s_warp);
     if (threadIdx.x == 0) P.scan_part[b] = sum;
   }
   grid_or_cta_sync(grid);
@@ -649,8 +602,8 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
       all += v;
       if (i < b) mine += v;
     }
-    carry = block_sum_int(mine, s_warp);
-    total = block_sum_int(all, s_warp);
+    carry = block_sum<int>(mine, s_warp);
+    total = block_sum<int>(all, s_warp);
   }
   for (int c0 = c_lo; c0 < c_hi; c0 += kMidThreads * 4) {
     const int c = c0 + (int)threadIdx.x * 4;
@@ -663,7 +616,7 @@ __global__ void __launch_bounds__(kMidThreads) k_mid(const __grid_constant__ Par
     }
     const int tsum = (v[0] + v[1]) + (v[2] + v[3]);
     int chunk;
-    int ex = carry + block_exclusive_scan_int(tsum, s_warp, &chunk);
+    int ex = carry + block_exclusive_scan<int>(tsum, s_warp, &chunk);
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
       if (c + k < c_hi) {
@@ -994,71 +947,9 @@ __global__ void __launch_bounds__(kAuxThreads) k_deposit(const __grid_constant__
 }
 
 // ---------------------------------------------------------------------------------------------
-// k_field helpers: 128-bit shuffles, block scans and sums (the kernel itself is cooperative, see below).
+// k_field helpers (the kernel itself is cooperative, see below); the 128-bit block scans and sums are block_ops.cuh's.
 constexpr int kFieldThreads = 256;
 constexpr int kFieldItems = 4;
-typedef __int128 i128;
-
-__device__ __forceinline__ i128 shfl_up_128(i128 v, int d) {
-  unsigned long long lo = (unsigned long long)v, hi = (unsigned long long)((unsigned __int128)v >> 64);
-  lo = __shfl_up_sync(0xffffffffu, lo, d);
-  hi = __shfl_up_sync(0xffffffffu, hi, d);
-  return (i128)(((unsigned __int128)hi << 64) | (unsigned __int128)lo);
-}
-__device__ __forceinline__ i128 shfl_xor_128(i128 v, int d) {
-  unsigned long long lo = (unsigned long long)v, hi = (unsigned long long)((unsigned __int128)v >> 64);
-  lo = __shfl_xor_sync(0xffffffffu, lo, d);
-  hi = __shfl_xor_sync(0xffffffffu, hi, d);
-  return (i128)(((unsigned __int128)hi << 64) | (unsigned __int128)lo);
-}
-
-// exclusive scan over the CTA of one int128 per thread; *total = sum over the CTA
-__device__ i128 block_exclusive_scan_128(i128 v, i128* s_warp, i128* total) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  i128 inc = v;
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const i128 t = shfl_up_128(inc, d);
-    if (lane >= d) inc += t;
-  }
-  if (lane == 31) s_warp[warp] = inc;
-  __syncthreads();
-  if (warp == 0) {
-    const i128 w = lane < (int)(blockDim.x >> 5) ? s_warp[lane] : (i128)0;
-    i128 winc = w;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const i128 t = shfl_up_128(winc, d);
-      if (lane >= d) winc += t;
-    }
-    s_warp[lane] = winc - w;
-    if (lane == 31) s_warp[32] = winc;
-  }
-  __syncthreads();
-  const i128 res = s_warp[warp] + inc - v;
-  *total = s_warp[32];
-  __syncthreads();
-  return res;
-}
-
-__device__ i128 block_sum_128(i128 v, i128* s_warp) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += shfl_xor_128(v, o);
-  if (lane == 0) s_warp[warp] = v;
-  __syncthreads();
-  i128 t = 0;
-  if (warp == 0) {
-    t = lane < (int)(blockDim.x >> 5) ? s_warp[lane] : (i128)0;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) t += shfl_xor_128(t, o);
-    if (lane == 0) s_warp[32] = t;
-  }
-  __syncthreads();
-  t = s_warp[32];
-  __syncthreads();
-  return t;
-}
 
 // One pass of CTA b over its elements j in [j_lo, j_hi] (a sub-range of 1..jmax), in chunks of
 // kFieldThreads * kFieldItems.  carryS = S_{j_lo-1}, carryT = T_{j_lo} on entry.  APPLY = false: only the sums
@@ -1085,7 +976,7 @@ __device__ void field_range(const Params& P, const long long* __restrict__ R_in,
       Sl[k] = run;  // inclusive local
     }
     i128 chunkS;
-    const i128 exS = carryS + block_exclusive_scan_128(run, s_warp, &chunkS);
+    const i128 exS = carryS + block_exclusive_scan<i128>(run, s_warp, &chunkS);
     i128 tsumS = 0;
 #pragma unroll
     for (int k = 0; k < kFieldItems; ++k) {
@@ -1094,7 +985,7 @@ __device__ void field_range(const Params& P, const long long* __restrict__ R_in,
       if (j <= j_hi) tsumS += Sl[k];
     }
     i128 chunkSS;
-    i128 T = carryT + block_exclusive_scan_128(tsumS, s_warp, &chunkSS);  // T at this thread's first element
+    i128 T = carryT + block_exclusive_scan<i128>(tsumS, s_warp, &chunkSS);  // T at this thread's first element
     if (APPLY) {
 #pragma unroll
       for (int k = 0; k < kFieldItems; ++k) {
@@ -1186,16 +1077,16 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
       if (j >= 1 && j <= nc - 1) wsum += (i128)(nc - j) * (i128)r;
     }
   }
-  tot = block_sum_128(tot, s_warp);
-  wsum = block_sum_128(wsum, s_warp);
+  tot = block_sum<i128>(tot, s_warp);
+  wsum = block_sum<i128>(wsum, s_warp);
   if (G > 1) {   // (a one-CTA grid already holds the totals)
     if (threadIdx.x == 0) { part[b] = tot; part[G + b] = wsum; }
     __threadfence();
     grid_or_cta_sync(grid);
     tot = 0; wsum = 0;
     for (int i = threadIdx.x; i < G; i += kFieldThreads) { tot += part[i]; wsum += part[G + i]; }
-    tot = block_sum_128(tot, s_warp);
-    wsum = block_sum_128(wsum, s_warp);
+    tot = block_sum<i128>(tot, s_warp);
+    wsum = block_sum<i128>(wsum, s_warp);
   }
   if (b == 0 && threadIdx.x == 0) st->rho_total = (long long)(tot >> (2 * smooth));   // the filter conserves charge
   const bool frozen = st->freeze_field != 0;
@@ -1226,11 +1117,11 @@ __global__ void __launch_bounds__(kFieldThreads) k_field(const __grid_constant__
         myLen = hi >= lo ? hi - lo + 1 : 0;
       }
       i128 dummy;
-      const i128 Sbefore = block_exclusive_scan_128(myA, s_warp, &dummy);            // S at the start of CTA i
+      const i128 Sbefore = block_exclusive_scan<i128>(myA, s_warp, &dummy);            // S at the start of CTA i
       const i128 term = ((int)threadIdx.x < b) ? myLen * Sbefore + myC : (i128)0;
-      carryT = block_sum_128(term, s_warp);
-      carryS = block_sum_128(((int)threadIdx.x < b) ? myA : (i128)0, s_warp);
-      Send = block_sum_128(myA, s_warp);                                              // S_jmax
+      carryT = block_sum<i128>(term, s_warp);
+      carryS = block_sum<i128>(((int)threadIdx.x < b) ? myA : (i128)0, s_warp);
+      Send = block_sum<i128>(myA, s_warp);                                              // S_jmax
     } else if (!bc) {
       // one CTA owns every element: no carries; S_jmax = sum_{j=1}^{nc-1} (nc R_j - tot) = tot - nc R_0
       Send = tot - (i128)nc * (i128)R[0];
