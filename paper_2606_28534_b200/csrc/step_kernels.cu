@@ -40,8 +40,8 @@ struct PassSmem {
   static constexpr size_t a_bar = (a_sp + kMaxSpecies * sizeof(SpeciesP) + 15) & ~(size_t)15;  // 2 x u64
   static constexpr size_t a_exc = a_bar + 16;                               // unsigned[kMaxR + 2]
   static constexpr size_t a_total = a_exc + (((size_t)(kMaxR + 2) * 4 + 15) & ~(size_t)15);
-  static constexpr size_t b_wc = stages;                                    // unsigned[kWarps][kWCap]
-  static constexpr size_t b_dens = b_wc + (size_t)kWCap * kWarps * 4;       // unsigned[2][kWCap + 1][kMaxSpecies]
+  static constexpr size_t b_wc = stages;                                    // unsigned[kWarps][2][kWCap]: destinations, row counts
+  static constexpr size_t b_dens = b_wc + 2 * (size_t)kWCap * kWarps * 4;   // unsigned[2][kWCap + 1][kMaxSpecies]
   static constexpr size_t b_sp = b_dens + 2 * (size_t)kDensWords * 4;
   static constexpr size_t b_bar = (b_sp + kMaxSpecies * sizeof(SpeciesP) + 15) & ~(size_t)15;
   static constexpr size_t b_total = b_bar + 16;
@@ -725,7 +725,9 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
   const int ntiles = (int)((n + kTile - 1) / kTile);
   const int G = gridDim.x;
   const int ns = P.ns;
-  unsigned* wc = s_wc + warp * kWCap;
+  unsigned* wc = s_wc + warp * (2 * kWCap);   // destination of the warp's first particle of every window cell
+  unsigned* cw = wc + kWCap;                  // per window cell, one byte per row of the warp: the row's particles for it
+  static_assert(kItems <= 4, "one byte per row in a 32-bit word");
 
   if (threadIdx.x == 0) {
     mbar_init(&bar[0], 1);
@@ -757,7 +759,10 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     const TileWin tw = make_window(d.x, d.y, R);
 
     // destination of this warp's first particle of every window cell
-    for (int k = lane; k < tw.W; k += 32) wc[k] = (unsigned)S->tb[k] + S->pre[k * kWarps + warp];
+    for (int k = lane; k < tw.W; k += 32) {
+      wc[k] = (unsigned)S->tb[k] + S->pre[k * kWarps + warp];
+      cw[k] = 0;
+    }
     __syncwarp();
 
     int e0, ne;
@@ -812,7 +817,7 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     // same operation over the kItems particles so that the shared-memory and warp-wide operations of different
     // particles overlap instead of forming one long dependent chain.
     int sp[kItems];
-    unsigned m[kItems], a[kItems], old[kItems];
+    unsigned m[kItems], a[kItems];
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
       const bool valid = key[r] >= 0;
@@ -820,18 +825,17 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
       m[r] = __match_any_sync(0xffffffffu, valid ? (unsigned)key[r] : (0x80000000u | (unsigned)lane));
       a[r] = valid ? deposit_a(x[r], tw.wlo + key[r], P.inv_dx, (unsigned)s_sp[sp[r]].Q) : 0u;
     }
-    // the leader of every (item, cell) group reserves the group's destinations; items in order (stability).  The
-    // counters are this warp's own: plain loads and stores, ordered by the warp barrier
+    // stable order inside (warp, cell) is row by row, lane by lane: the leader of every (row, cell) group writes the
+    // group's size into the cell's byte for that row -- distinct bytes, no read-modify-write, no ordering between the
+    // rows -- and after one warp barrier every lane adds up the earlier rows' bytes of its own cell
+    {
+      unsigned char* cb = reinterpret_cast<unsigned char*>(cw);
 #pragma unroll
-    for (int r = 0; r < kItems; ++r) {
-      old[r] = 0;
-      if (key[r] >= 0 && lane == __ffs(m[r]) - 1) {
-        unsigned* slot = &wc[BIT1_CHECK(P.st, key[r], tw.W)];
-        old[r] = *slot;
-        *slot = old[r] + (unsigned)__popc(m[r]);
-      }
-      __syncwarp();
+      for (int r = 0; r < kItems; ++r)
+        if (key[r] >= 0 && lane == __ffs(m[r]) - 1)
+          cb[BIT1_CHECK(P.st, key[r], tw.W) * 4 + r] = (unsigned char)__popc(m[r]);   // 32 is written as 32: fits a byte
     }
+    __syncwarp();
     // deposit (SURVEY 8(c) "D"): one shared-memory atomic pair per (cell, species) run of the warp
     if (P.dep_u32) {
       // Q < 2^21: the sum of a over a warp stays below 2^26
@@ -862,9 +866,12 @@ k_pass_b(const __grid_constant__ Params P, Particles cur, Particles nxt) {
     }
 #pragma unroll
     for (int r = 0; r < kItems; ++r) {
-      const unsigned o = __shfl_sync(0xffffffffu, old[r], __ffs(m[r]) - 1);
       if (key[r] >= 0) {
         const int off = warp * kWarpSpan + r * 32 + lane;
+        const unsigned rows = cw[key[r]];
+        unsigned o = wc[key[r]];
+#pragma unroll
+        for (int q = 0; q < r; ++q) o += (rows >> (8 * q)) & 0xffu;
         const unsigned dst = BIT1_CHECK(P.st, o + (unsigned)__popc(m[r] & lt), P.st->n_next);
         nxt.x[dst] = x[r]; nxt.vx[dst] = vx[r]; nxt.vy[dst] = vy[r]; nxt.vz[dst] = vz[r];
         nxt.pid[dst] = S->pid[off]; nxt.sp[dst] = (unsigned char)sp[r];
