@@ -60,6 +60,7 @@ __device__ __forceinline__ unsigned long long w52(unsigned a, unsigned b) {
 // builds the banded histogram.  One CTA barrier per tile: the histogram is double-buffered.
 __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_constant__ Params P, Particles cur) {
   constexpr int kWarpSpan = 32 * kItems;
+  static_assert(kItems <= 4, "the (cell, warp) histogram counter holds one byte per row of the warp");
   if (P.st->stalled) return;
   typedef PassSmem SM;
   extern __shared__ __align__(128) unsigned char smem[];
@@ -181,10 +182,12 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
         const unsigned eb = __ballot_sync(0xffffffffu, (evm >> r) & 1u);
         if (lane == 0) P.evt[BIT1_CHECK(P.st, (base >> 5) + (unsigned)(warp * kItems + r), (unsigned)(P.max_tiles + 1) * (kTile / 32))] = eb;
       }
+      // the (window cell, warp) counter is four bytes, one per row of the warp: the leader of every (row, cell) group
+      // writes the group's size into its own byte -- no read-modify-write, no ordering between the rows
       const unsigned m = __match_any_sync(0xffffffffu, key);
       if (!(key & 0x80000000u) && lane == __ffs(m) - 1)
-        s_hist[BIT1_CHECK(P.st, key, (unsigned)tw.W) * kWarps + warp] += (unsigned)__popc(m);
-      __syncwarp();
+        reinterpret_cast<unsigned char*>(s_hist)[(BIT1_CHECK(P.st, key, (unsigned)tw.W) * kWarps + warp) * 4 + r] =
+            (unsigned char)__popc(m);
     }
     // how far outside the tile's old cell range the windowed particles land: k_mid picks the next step's radius from
     // these counts and the far movers' (phase 2).  At radius 1 a windowed particle is at most one cell outside and
@@ -211,7 +214,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) k_pass_a(const __grid_co
       unsigned* pre = P.tile_pre + BIT1_CHECK(P.st, rowo + (size_t)k, tile_row_words(P.nc, P.max_tiles, P.R_max)) * kWarps;
 #pragma unroll
       for (int w = 0; w < kWarps; ++w) {
-        const unsigned t = s_hist[k * kWarps + w];
+        const unsigned t = __dp4a(s_hist[k * kWarps + w], 0x01010101u, 0u);   // sum of the four rows' bytes
         s_hist[k * kWarps + w] = 0;
         pre[w] = run;
         run += t;
