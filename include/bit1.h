@@ -52,7 +52,8 @@ typedef enum {
   BIT1_ERR_STATE = 4,       /* call out of order (e.g. step before load) */
   BIT1_ERR_CUDA = 5,        /* a CUDA runtime call failed / no device */
   BIT1_ERR_CHECKPOINT = 6,  /* blob does not match this context */
-  BIT1_ERR_DEVICE_FLAG = 7  /* sticky device flag set; see bit1_moments.flags */
+  BIT1_ERR_DEVICE_FLAG = 7, /* sticky device flag set; see bit1_moments.flags */
+  BIT1_ERR_STATIC_LIMIT = 8 /* bit1_field_solve_static only: more cells than BIT1_FIELD_STATIC_MAX_CELLS */
 } bit1_status;
 
 /* sticky device flag bits (bit1_moments.flags) */
@@ -277,6 +278,43 @@ bit1_status bit1_stream_publish(bit1_ctx *ctx, uint64_t *seq_or_null);
 bit1_status bit1_stream_acquire(bit1_ctx *ctx, uint64_t after_seq, const void **slot, uint64_t *seq);
 bit1_status bit1_stream_release(bit1_ctx *ctx, uint64_t seq);
 bit1_status bit1_stream_close(bit1_ctx *ctx);
+
+/* The field solve on its own, for callers that cannot allocate device memory.
+ *
+ * Every other call of this library works out of the workspace handed to bit1_create, which somebody had to cudaMalloc.
+ * Not every caller can: a plug-in inside a host application whose GPU memory comes from the host's own pool, a callback
+ * that runs while that pool is locked, a job whose device-memory budget was fixed when it started.  Such a caller owns
+ * the arrays it was given and nothing more, and cudaMalloc is either forbidden to it or would stall the whole device
+ * under somebody else's pipeline.  For them this one entry point runs the step's field solve -- `smoothing_passes`
+ * (0..8) passes of the 1-2-1 filter of bit1_set_smoothing over rho, then the exact integer-scan Poisson solve
+ * ("(iii) field solver", "density smoothing") -- with no context, no
+ * workspace, and no cudaMalloc / cudaFree / allocating library routine anywhere inside: the temporaries the solve needs
+ * (per-CTA partial sums, two int64 arrays for the filter) live in an array that is part of the library image itself.
+ *
+ *   rho_fixed  DEVICE, in: ng int64 entries (ng = nc + 1 with walls, nc periodic), unit 2^-40 C, what bit1_get_rho returns
+ *   phi, E     DEVICE, out: nc + 1 doubles each (periodic: entry nc repeats entry 0); must not overlap rho_fixed
+ *   nc, bc, dx, area   as in bit1_grid
+ *   stream     cudaStream_t, borrowed; NULL = default stream.  The call enqueues one kernel and returns without waiting.
+ * phi and E are bit-identical to what a context with the same grid and bit1_set_smoothing(passes) computes from the
+ * same rho (bit1_get_phi / bit1_get_E).
+ *
+ * Limits and rules that follow from the built-in array:
+ *  - nc <= BIT1_FIELD_STATIC_MAX_CELLS (1 048 576, the largest grid of BASELINE.json).  A larger grid is refused with
+ *    BIT1_ERR_STATIC_LIMIT and nothing is launched; use a context (bit1_create) for it.
+ *  - The array (about 16 MiB) occupies device memory on every GPU of the process that loads this library, from load
+ *    until the process exits, whether or not this call is ever made.
+ *  - The first call on each device looks up the array's device address (cudaGetSymbolAddress) and the SM count and
+ *    remembers them; make that first call with the device current and outside any CUDA stream capture.  Later calls on
+ *    that device do no set-up.  The device current at the call must be the one `stream` belongs to.
+ *  - All calls on one device share the one array, which still holds whatever the previous call left there.  The kernel
+ *    writes every entry before it reads it, so nothing needs clearing and a call never sees an earlier call's data; but two
+ *    calls that run on the GPU at the same time (different streams, or different threads) overwrite each other's
+ *    temporaries and both results are garbage.  Keep the calls of one device on one stream, or order them with events.
+ * BIT1_ERR_INVALID_ARG: a NULL pointer, nc < 2, bc not 0/1, dx or area not positive, passes outside 0..8.
+ * BIT1_ERR_CUDA: no device, the address look-up or the launch failed. */
+#define BIT1_FIELD_STATIC_MAX_CELLS 1048576
+bit1_status bit1_field_solve_static(const int64_t *rho_fixed, double *phi, double *E, int32_t nc, int32_t bc, double dx,
+                                    double area, int32_t smoothing_passes, void *stream);
 
 void bit1_destroy(bit1_ctx *ctx);
 const char *bit1_error_string(bit1_status s);

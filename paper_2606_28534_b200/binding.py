@@ -17,6 +17,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libbit1.so")
 
 OK, ERR_INVALID_ARG, ERR_RANGE, ERR_CAPACITY, ERR_STATE, ERR_CUDA, ERR_CHECKPOINT, ERR_DEVICE_FLAG = range(8)
+ERR_STATIC_LIMIT = 8
+FIELD_STATIC_MAX_CELLS = 1 << 20   # BIT1_FIELD_STATIC_MAX_CELLS
 FLAG_CAPACITY, FLAG_ESCAPE, FLAG_PID_WRAP = 1, 2, 8
 
 c_f64p = C.POINTER(C.c_double)
@@ -154,6 +156,8 @@ def load_library(path: Optional[str] = None):
     L.bit1_build_is_checked.argtypes = []
     L.bit1_check_selftest.restype = C.c_int
     L.bit1_check_selftest.argtypes = [vp]
+    L.bit1_field_solve_static.restype = C.c_int
+    L.bit1_field_solve_static.argtypes = [vp, vp, vp, C.c_int32, C.c_int32, C.c_double, C.c_double, C.c_int32, vp]
     if path is None:
         _lib = L
     return L
@@ -182,6 +186,30 @@ def _ptr(a):
     if isinstance(a, np.ndarray):
         return a.ctypes.data
     return a.data_ptr()
+
+
+def field_solve_static(rho, phi, E, nc: int, bc: int, dx: float, area: float, passes: int = 0, stream=None, lib=None):
+    """bit1_field_solve_static: smoothing + Poisson solve of one rho array with no context and no workspace.
+
+    For code that may not allocate GPU memory (a plug-in fed from its host's memory pool, a callback that runs while
+    that pool is locked, a job with a fixed device-memory budget): the library allocates nothing in this call; its
+    temporaries live in an array built into libbit1.so, which is why nc may not exceed FIELD_STATIC_MAX_CELLS
+    (Bit1Error with status ERR_STATIC_LIMIT beyond it).  rho (int64[ng]), phi and E (float64[nc + 1]) are torch CUDA
+    tensors the caller already owns, all on the current device; stream is a torch.cuda.Stream or None (the current
+    stream).  The kernel is enqueued, not waited for.  Calls on one device share the built-in array: keep them on one
+    stream (include/bit1.h has the full list of rules).  Marshalling only."""
+    import torch
+
+    L = lib if lib is not None else load_library()
+    ng = nc + 1 if bc else nc
+    for t, n, dt, name in ((rho, ng, torch.int64, "rho"), (phi, nc + 1, torch.float64, "phi"), (E, nc + 1, torch.float64, "E")):
+        if not (t.is_cuda and t.dtype == dt and t.is_contiguous() and t.numel() == n):
+            raise ValueError(f"{name}: need a contiguous CUDA tensor of {n} x {dt}")
+    s = stream if stream is not None else torch.cuda.current_stream(rho.device)
+    with torch.cuda.device(rho.device):
+        st = L.bit1_field_solve_static(rho.data_ptr(), phi.data_ptr(), E.data_ptr(), int(nc), int(bc), float(dx), float(area),
+                                       int(passes), s.cuda_stream)
+    _check(st, "bit1_field_solve_static")
 
 
 class Bit1:

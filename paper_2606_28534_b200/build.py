@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libbit1.so")
 LIB_CHECKED = os.path.join(_HERE, "libbit1_checked.so")   # -DBIT1_CHECKED: index checks in the step kernels (common.cuh)
-SOURCES = ["api.cu", "step_kernels.cu", "general_kernels.cu", "aux_kernels.cu"]
+SOURCES = ["api.cu", "step_kernels.cu", "general_kernels.cu", "aux_kernels.cu", "field_static.cu"]
 HEADERS = ["common.cuh", "device_math.cuh", "advance.cuh", "pipeline.cuh", "block_ops.cuh", "step_kernels.h", "aux_kernels.h",
            os.path.join("..", "..", "include", "bit1.h")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-fmad=false", "-lineinfo",

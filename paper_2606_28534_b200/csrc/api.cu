@@ -293,6 +293,8 @@ const char* bit1_error_string(bit1_status s) {
     case BIT1_ERR_CUDA: return "CUDA runtime error or no device";
     case BIT1_ERR_CHECKPOINT: return "checkpoint blob does not match this context";
     case BIT1_ERR_DEVICE_FLAG: return "sticky device flag set";
+    case BIT1_ERR_STATIC_LIMIT:
+      return "grid has more cells than the built-in scratch of bit1_field_solve_static holds (BIT1_FIELD_STATIC_MAX_CELLS = 1048576)";
   }
   return "unknown";
 }
