@@ -234,6 +234,7 @@ def _measure(sim, steps: int, warmup: int, peak: float, barrier=None, sampler_in
     sim.step(warmup)
     sim.sync()
     n_start = sim.n_live()
+    general0 = sim.get_moments()["general_steps"]
     launches0 = sim.launch_count()
     ev0 = torch.cuda.Event(enable_timing=True)
     ev1 = torch.cuda.Event(enable_timing=True)
@@ -255,6 +256,13 @@ def _measure(sim, steps: int, warmup: int, peak: float, barrier=None, sampler_in
     launches = sim.launch_count() - launches0
     sim.sync()
     ms_settled = 1e3 * (time.perf_counter() - t_wall0)   # wall clock incl. any step redone by the general path
+    # A step whose side list overflowed is a device no-op inside the event pair; its real work (the general path) runs in
+    # the sync above.  If that happened in the timed leg the event time undercounts: the wall clock up to the end of the
+    # settle is the honest figure, and every number derived from `ms` (headline value, workloads list) uses it.
+    general_timed = int(sim.get_moments()["general_steps"] - general0)
+    ms_events = ms
+    if general_timed > 0:
+        ms = ms_settled
     n_end = sim.n_live()
     units = 0.5 * (n_start + n_end) * steps
     psteps_want = min(steps, 50)
@@ -266,7 +274,9 @@ def _measure(sim, steps: int, warmup: int, peak: float, barrier=None, sampler_in
     n_prof = 0.5 * (n_end + sim.n_live())
     mom = sim.get_moments()
     kern = {k: v / max(psteps, 1) for k, v in prof.items()}
-    return dict(ms=ms, ms_settled=ms_settled, units=units, launches=int(launches), clocks=clocks, n_end=n_end,
+    return dict(ms=ms, ms_events=ms_events, ms_settled=ms_settled, general_timed=general_timed,
+                timed="wall clock incl. settle of redone steps" if general_timed else "CUDA events",
+                units=units, launches=int(launches), clocks=clocks, n_end=n_end,
                 n_prof=n_prof, kern=kern, psteps=int(psteps), mom=mom)
 
 
@@ -287,6 +297,7 @@ def _summary(r, steps: int, peak: float, n0: int):
                  "state larger than L2 (no flush)",
            "far_movers_per_step": r["mom"]["far_movers"] / max(r["mom"]["step"], 1),
            "window_radius": r["mom"]["window_radius"], "general_steps": r["mom"]["general_steps"],
+           "general_steps_in_timed_region": r["general_timed"], "timed": r["timed"],
            "flags": r["mom"]["flags"], "gpu_launches": r["launches"]}
     return out
 
@@ -459,7 +470,8 @@ def run_cuda(args):
                               "frac_on_82B_minimum": MIN_BPP * n_mean / (ms_step * 1e-3) / 1e9 / peak},
                      "kernel_ms_per_step": kernels},
         "state": {"n_live": n_end, "births": mom["births"], "far_movers_per_step": mom["far_movers"] / max(mom["step"], 1),
-                  "window_radius": mom["window_radius"], "general_steps": mom["general_steps"], "flags": mom["flags"]},
+                  "window_radius": mom["window_radius"], "general_steps": mom["general_steps"],
+                  "general_steps_in_timed_region": r["general_timed"], "timed": r["timed"], "flags": mom["flags"]},
     }
     sim.close()
     del sim, pin, host
@@ -499,7 +511,7 @@ def run_sweep(args):
             r = _measure(sim, steps, args.warmup, peak)
             m = r["mom"]
             # steps redone by the general path run when the host next waits: their time is in the wall clock only
-            ms = r["ms_settled"] if m["general_steps"] else r["ms"]
+            ms = r["ms_settled"] if m["general_steps"] else r["ms_events"]
             print(json.dumps({"workload": wname + ("" if not args.noisy else " (independent load)"), "vscale": vs,
                               "radius": "adaptive" if radius is None else radius, "ms_per_step": round(ms / steps, 3),
                               "timed": "wall clock incl. settle" if m["general_steps"] else "CUDA events",
