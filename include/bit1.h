@@ -259,7 +259,10 @@ bit1_status bit1_export_species(bit1_ctx *ctx, int species, uint64_t capacity_ou
  * number > after_seq (BIT1_ERR_STATE if there is none yet; it never blocks) and keeps the producer off it until
  * bit1_stream_release(seq).  The slot starts with a bit1_stream_header; offsets are bytes from the slot's start.
  * A reader in another process that maps the same memory follows the seqlock: a slot is complete iff
- * seq == seq_begin != 0, before and after it has copied what it needs. */
+ * seq == seq_begin != 0, before and after it has copied what it needs.
+ *   bit1_stream_close (producer thread) waits for the copy in flight and detaches the ring.  Consumer threads must be
+ * out of bit1_stream_acquire / bit1_stream_release, and hold no slot they still read, before it is called: the ring
+ * pointer and slot count are plain fields, and the memory goes back to the caller. */
 #define BIT1_STREAM_MAX_SLOTS 8
 typedef struct {
   char magic[8];                       /* "BIT1STRM" */

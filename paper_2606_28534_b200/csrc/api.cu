@@ -1352,8 +1352,18 @@ bit1_status bit1_stream_acquire(bit1_ctx* c, uint64_t after_seq, const void** sl
     if (best < 0) return BIT1_ERR_STATE;   // nothing newer than after_seq yet
     int expect = kSlotReady;
     if (c->slot_state[best].compare_exchange_strong(expect, kSlotHeld, std::memory_order_acq_rel)) {
+      // The slot is ours now and the producer keeps off it, so its sequence number can no longer change.  Read it
+      // again: between the scan above and the exchange the producer may have reclaimed the slot and published a newer
+      // snapshot into it (state Ready again, so the exchange still succeeded).  What the slot holds is then that newer
+      // snapshot, complete (the number is stored before the state), and its number is the one bit1_stream_release
+      // will be given -- the number seen by the scan would match no slot and the slot would stay held for good.
+      const uint64_t now = c->slot_seq[best].load(std::memory_order_acquire);
+      if (now <= after_seq) {   // cannot happen with increasing numbers; never hand out what the caller has seen
+        c->slot_state[best].store(kSlotReady, std::memory_order_release);
+        continue;
+      }
       *slot_out = c->ring + (size_t)best * c->slot_bytes;
-      *seq_out = bs;
+      *seq_out = now;
       return BIT1_OK;
     }
     // the producer took it back for the next snapshot in the meantime: look again
