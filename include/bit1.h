@@ -215,7 +215,8 @@ bit1_status bit1_set_averaging(bit1_ctx *ctx, int window, int interval);
 bit1_status bit1_get_average(bit1_ctx *ctx, int64_t *dens_sum, double *phi_sum, uint64_t *count, uint64_t *step);
 
 /* Prescribed field: overwrite E (HOST, nc+1 entries) and optionally freeze the field solve (E stays as set while rho
- * keeps being deposited): test-particle runs in a given field; the closed-form push tests use it too. */
+ * keeps being deposited): test-particle runs in a given field; the closed-form push tests use it too.  While the field
+ * is frozen bit1_checkpoint is refused (see there). */
 bit1_status bit1_set_E(bit1_ctx *ctx, const double *E, int freeze_field);
 /* Set the step counter (Philox counter words 1-2), e.g. to continue a run that was loaded from exported records. */
 bit1_status bit1_set_step(bit1_ctx *ctx, uint64_t step);
@@ -227,7 +228,10 @@ bit1_status bit1_set_step(bit1_ctx *ctx, uint64_t step);
  * every later step overlaps the copy; without it the copy reads the store directly, the next step overlaps it and the
  * one after waits.  *written <= bit1_checkpoint_size() (the size at full capacity).  The blob is valid after
  * bit1_checkpoint_wait.  bit1_restart needs a context created with the identical configuration, validates the blob
- * (BIT1_ERR_CHECKPOINT) and reproduces the run bit-identically (BASELINE.json north_star). */
+ * (BIT1_ERR_CHECKPOINT) and reproduces the run bit-identically (BASELINE.json north_star).
+ * The blob carries no E (restart solves it from rho), so a run under a prescribed frozen field (bit1_set_E with
+ * freeze_field != 0) cannot be checkpointed: bit1_checkpoint returns BIT1_ERR_STATE until the field is released by
+ * bit1_set_E(E, 0).  Such a run is continued by reloading its particles and calling bit1_set_E again. */
 size_t bit1_checkpoint_size(bit1_ctx *ctx);
 bit1_status bit1_checkpoint(bit1_ctx *ctx, void *pinned_host, size_t cap, size_t *written);
 bit1_status bit1_checkpoint_wait(bit1_ctx *ctx);

@@ -1086,6 +1086,10 @@ bit1_status bit1_checkpoint(bit1_ctx* c, void* host, size_t cap, size_t* written
   // (the expensive part) runs on the side stream behind an event and overlaps the steps that follow
   DevState h;
   BIT1_OK_OR_RETURN(settle(c, &h));
+  // The blob holds no E: bit1_restart rebuilds the field from rho.  Under a prescribed, frozen field (bit1_set_E with
+  // freeze_field) that rebuild would silently swap the caller's field for the self-consistent one, and the restarted
+  // run would no longer be the run that was saved.  Refuse rather than write a checkpoint that cannot keep the promise.
+  if (h.freeze_field) return BIT1_ERR_STATE;
   const size_t n = h.n;
   const CkptLayout cl = ckpt_layout(c->P.nc, c->P.ng, c->P.ns, n);
   if (cap < cl.bytes) return BIT1_ERR_CAPACITY;

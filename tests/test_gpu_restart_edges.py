@@ -446,3 +446,42 @@ def test_eight_species():
     assert_moments = __import__("parity").assert_moments_close
     assert_moments(g, o, tol=1e-9)
     g.close()
+
+
+def test_checkpoint_is_refused_while_the_field_is_frozen():
+    """The blob holds no E (restart solves it from rho): under bit1_set_E(E, freeze) a restart would continue with the
+    self-consistent field instead of the prescribed one, so bit1_checkpoint says BIT1_ERR_STATE until the field is
+    released, and the context stays usable."""
+    import torch
+    from paper_2606_28534_b200.binding import Bit1, Bit1Error, ERR_STATE
+
+    w = W.make_config(2, scale=1 / 64)
+    g = Bit1(w)
+    g.load()
+    blob = torch.empty(g.checkpoint_size(), dtype=torch.uint8).pin_memory()
+    E = np.linspace(-50.0, 50.0, w.nc + 1)
+    g.set_E(E, freeze_field=True)
+    g.step(3)
+    with pytest.raises(Bit1Error) as e:
+        g.checkpoint(blob)
+    assert e.value.status == ERR_STATE
+    assert np.array_equal(g.get_E(), E), "the refusal must not touch the prescribed field"
+    g.step(2)                              # still running under the frozen field
+    assert np.array_equal(g.get_E(), E)
+    g.set_E(g.get_E(), freeze_field=False)  # released: the next step solves the field again
+    g.step(1)
+    g.checkpoint(blob)
+    g.checkpoint_wait()
+    g.step(4)
+    g.sync()
+    want = g.get_particles()
+    h = Bit1(w)
+    h.restart(blob)
+    h.step(4)
+    h.sync()
+    got = h.get_particles()
+    for k in want:
+        assert np.array_equal(want[k], got[k]), k
+    assert np.array_equal(g.get_E(), h.get_E())
+    g.close()
+    h.close()
