@@ -243,7 +243,12 @@ bit1_status bit1_restart(bit1_ctx *ctx, const void *blob_host, size_t bytes);
  * order (HOST, *n_out entries each; any of them may be NULL; pid is the library's own addition, needed to continue a
  * run with the same random streams).  With all record pointers NULL it only returns *n_out and the counts (size
  * query); BIT1_ERR_CAPACITY (with *n_out set) if capacity_out < *n_out.  Waits for a pending checkpoint and for the
- * compute stream; uses the idle half of the particle store as staging, the live state is untouched. */
+ * compute stream; uses the idle half of the particle store as staging, the live state is untouched.
+ * These records (and the slots of bit1_stream_*) are for analysis and for starting a NEW run from a saved plasma: loaded
+ * back with bit1_load_particles + bit1_set_step they give the same charge, counts per cell and particle ids, but not a
+ * bit-identical continuation -- concatenating species changes the order inside a cell, hence which newborn particle gets
+ * which id, and next_pid, the wall / event counters and the averaging sums are not part of them.  For a continuation
+ * that repeats the original run use bit1_checkpoint / bit1_restart. */
 bit1_status bit1_export_species(bit1_ctx *ctx, int species, uint64_t capacity_out, uint64_t *n_out,
                                 int64_t *counts_per_cell, double *x, double *vx, double *vy, double *vz,
                                 uint32_t *pid_or_null);
