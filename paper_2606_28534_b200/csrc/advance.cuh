@@ -8,10 +8,14 @@
 //   SinkStore  general path (general_kernels.cu): counters are left alone (pass A has already counted this step),
 //              births are handed back to the caller, which ranks them itself.
 #pragma once
+#include <cooperative_groups.h>
+
 #include "device_math.cuh"
 #include "pipeline.cuh"
 
 namespace bit1 {
+
+namespace cg_adv = cooperative_groups;
 
 __device__ __forceinline__ unsigned long long make_key(const Params& P, int cell, unsigned cls,
                                                        unsigned long long ord) {
@@ -19,9 +23,16 @@ __device__ __forceinline__ unsigned long long make_key(const Params& P, int cell
 }
 
 // Append one record (far mover or birth) to the side list.  Order of arrival is irrelevant: k_mid sorts by key.
+// Warp-aggregated (BASELINE.json north_star, "warp-aggregated append of newborn particles"): the lanes of a warp that
+// arrive here together take their slots with ONE atomic on the list's counter -- the lowest of them adds their number,
+// everybody gets the base by shuffle and adds its rank among them -- instead of one atomic per record on a single
+// address, which is what serialises a step with many far movers (profiles/r2_far_mover_sweep.md).
 static __device__ __noinline__ void emit_record(const Params& P, unsigned long long key, double x, double vx, double vy,
                                          double vz, unsigned pid, int sp) {
-  const unsigned slot = atomicAdd(&P.st->ovf_count, 1u);
+  const cg_adv::coalesced_group together = cg_adv::coalesced_threads();
+  unsigned base = 0;
+  if (together.thread_rank() == 0) base = atomicAdd(&P.st->ovf_count, (unsigned)together.size());
+  const unsigned slot = together.shfl(base, 0) + together.thread_rank();
   if (slot >= P.ovf_cap) return;   // k_mid sees ovf_count > ovf_cap and stalls the step: the general path takes it
   P.ovf_key[BIT1_CHECK(P.st, slot, P.ovf_cap)] = key;
   OvfRec r;
