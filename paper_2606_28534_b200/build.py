@@ -5,7 +5,9 @@ particle state is bit-identical to the CPU oracle's.
 """
 from __future__ import annotations
 
+import hashlib
 import os
+import socket
 import subprocess
 import sys
 
@@ -27,12 +29,38 @@ def _nvcc() -> str:
     return "nvcc"
 
 
+def _fingerprint(checked: bool = False) -> str:
+    """sha256 over everything the library is made from: sources, headers, flags, this file."""
+    h = hashlib.sha256()
+    for d in [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]:
+        with open(d, "rb") as f:
+            h.update(os.path.basename(d).encode() + b"\0" + f.read() + b"\0")
+    h.update(" ".join(NVCC_FLAGS + (["-DBIT1_CHECKED"] if checked else [])).encode())
+    return h.hexdigest()
+
+
+def _stamp(lib: str):
+    """(hostname, fingerprint) written next to the library by the build that made it, or (None, None)."""
+    try:
+        with open(lib + ".stamp") as f:
+            host, fp = f.read().split()
+        return host, fp
+    except (OSError, ValueError):
+        return None, None
+
+
 def stale(lib: str = LIB) -> bool:
+    """True unless `lib` exists and was built from exactly the present sources and flags (content hash, not mtimes: a
+    tree that arrives with its library -- a gpurun snapshot, a fresh checkout next to an old build -- has arbitrary
+    file times)."""
     if not os.path.exists(lib):
         return True
-    t = os.path.getmtime(lib)
-    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]
-    return any(os.path.getmtime(d) > t for d in deps)
+    return _stamp(lib)[1] != _fingerprint(checked=(lib == LIB_CHECKED))
+
+
+def built_here(lib: str = LIB) -> bool:
+    """The library was compiled on this host (its stamp says so)."""
+    return os.path.exists(lib) and _stamp(lib)[0] == socket.gethostname()
 
 
 def build(force: bool = False, verbose: bool = False, checked: bool = False) -> str:
@@ -58,6 +86,8 @@ def build(force: bool = False, verbose: bool = False, checked: bool = False) -> 
         raise RuntimeError("link failed")
     with open(os.path.join(CSRC, "ptxas_checked.log" if checked else "ptxas.log"), "w") as f:
         f.write("\n".join(log))
+    with open(lib + ".stamp", "w") as f:
+        f.write(f"{socket.gethostname()} {_fingerprint(checked)}\n")
     if verbose:
         print("\n".join(log))
     return lib

@@ -5,8 +5,12 @@
 #include "block_ops.cuh"
 #include "aux_kernels.h"
 #include "device_math.cuh"
+#include "step_kernels.h"
 
 namespace bit1 {
+
+// grid of the grid-stride kernels below: 8 CTAs of 256 threads per SM of the current device
+static int aux_grid() { return sm_count() * 8; }
 
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_load_prepare(const __grid_constant__ Params P, Particles in, unsigned n,
@@ -40,7 +44,7 @@ __global__ void __launch_bounds__(256) k_load_validate(const __grid_constant__ P
 }
 int launch_load_validate(const Params& P, const Particles& in, unsigned n, cudaStream_t s) {
   if (n == 0) return 0;
-  k_load_validate<<<148 * 8, 256, 0, s>>>(P, in, n);
+  k_load_validate<<<aux_grid(), 256, 0, s>>>(P, in, n);
   return 1;
 }
 // bit1_restart: the same, and the positions must be in cell order (the blob's body is data from outside)
@@ -55,7 +59,7 @@ __global__ void __launch_bounds__(256) k_state_validate(const __grid_constant__ 
 }
 int launch_state_validate(const Params& P, const Particles& p, unsigned n, cudaStream_t s) {
   if (n == 0) return 0;
-  k_state_validate<<<148 * 8, 256, 0, s>>>(P, p, n);
+  k_state_validate<<<aux_grid(), 256, 0, s>>>(P, p, n);
   return 1;
 }
 
@@ -231,19 +235,19 @@ int launch_load_sort(const Params& P, const Particles& in, const Particles& out,
   int launches = 0;
   unsigned* k0 = reinterpret_cast<unsigned*>(scratch);
   unsigned* v0 = k0 + P.capacity;
-  k_load_prepare<<<148 * 8, 256, 0, s>>>(P, in, n, have_pid, k0, v0);
+  k_load_prepare<<<aux_grid(), 256, 0, s>>>(P, in, n, have_pid, k0, v0);
   ++launches;
   int bits = 0;
   while ((1ll << bits) < (long long)P.nc) ++bits;
   unsigned *ks = nullptr, *vs = nullptr;
   launches += launch_radix_sort_u32(n, P.capacity, bits, scratch, s, &ks, &vs);
-  k_gather_keys<<<148 * 8, 256, 0, s>>>(in, out, vs, n);
+  k_gather_keys<<<aux_grid(), 256, 0, s>>>(in, out, vs, n);
   // the velocity arrays arrive on another stream, one event each: a component is gathered as soon as it has landed
   const double* vin[3] = {in.vx, in.vy, in.vz};
   double* vout[3] = {out.vx, out.vy, out.vz};
   for (int k = 0; k < 3; ++k) {
     if (velocity_ready) cudaStreamWaitEvent(s, velocity_ready[k], 0);
-    k_gather_f64<<<148 * 8, 256, 0, s>>>(vin[k], vout[k], vs, n);
+    k_gather_f64<<<aux_grid(), 256, 0, s>>>(vin[k], vout[k], vs, n);
   }
   return launches + 4;
 }
@@ -334,7 +338,7 @@ __global__ void __launch_bounds__(256) k_fill_cells(const __grid_constant__ Para
     cur.cell[i] = cell_of(P, cur.x[i]);
 }
 int launch_fill_cells(const Params& P, const Particles& cur, cudaStream_t s) {
-  k_fill_cells<<<148 * 8, 256, 0, s>>>(P, cur);
+  k_fill_cells<<<aux_grid(), 256, 0, s>>>(P, cur);
   return 1;
 }
 
@@ -441,7 +445,7 @@ int launch_export_count(const Params& P, const Particles& cur, int species, unsi
   unsigned* chunk_cnt = reinterpret_cast<unsigned*>(b + 256 + (((size_t)P.nc * 4 + 255) & ~(size_t)255));
   const size_t nchunks_max = ((size_t)capacity + kExpChunk - 1) / kExpChunk;
   cudaMemsetAsync(b, 0, 256 + (((size_t)P.nc * 4 + 255) & ~(size_t)255) + nchunks_max * 4, s);
-  k_export_count<<<148 * 8, 256, 0, s>>>(P, cur, species, chunk_cnt, cell_cnt, total);
+  k_export_count<<<aux_grid(), 256, 0, s>>>(P, cur, species, chunk_cnt, cell_cnt, total);
   return 1 + launch_scan_u32(chunk_cnt, nchunks_max, chunk_cnt + nchunks_max, s);
 }
 
@@ -449,7 +453,7 @@ int launch_export_scatter(const Params& P, const Particles& cur, const Particles
                           cudaStream_t s) {
   char* b = static_cast<char*>(scratch);
   const unsigned* chunk_off = reinterpret_cast<const unsigned*>(b + 256 + (((size_t)P.nc * 4 + 255) & ~(size_t)255));
-  k_export_scatter<<<148 * 8, 256, 0, s>>>(P, cur, out, species, chunk_off);
+  k_export_scatter<<<aux_grid(), 256, 0, s>>>(P, cur, out, species, chunk_off);
   return 1;
 }
 }  // namespace bit1

@@ -190,10 +190,7 @@ int launch_general_step(const Params& P, const Particles& cur, const Particles& 
   unsigned* k0 = reinterpret_cast<unsigned*>(sort_scratch);
   unsigned* v0 = k0 + P.capacity;
   int launches = 0;
-  int dev = 0, sms = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  const int g = sms * 8;
+  const int g = sm_count() * 8;
   k_gen_begin<<<1, 1, 0, s>>>(P, hdr);
   k_gen_count<<<g, kGenThreads, 0, s>>>(P, cur, hdr, chunk);
   launches += 2;

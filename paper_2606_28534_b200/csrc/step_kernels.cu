@@ -1195,15 +1195,18 @@ __global__ void __launch_bounds__(kAuxThreads) k_average(const __grid_constant__
 
 // ---------------------------------------------------------------------------------------------
 // host-side launchers
-static int g_sms = 0;
-static int sm_count() {
-  if (!g_sms) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev);
-    if (g_sms <= 0) g_sms = 148;
+// SMs of the current device, asked once per device (grids are sized from it everywhere; step_kernels.h)
+int sm_count() {
+  constexpr int kMaxDev = 64, kB200Sms = 148;   // the fallback only if the attribute query itself fails
+  static int cache[kMaxDev] = {0};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDev) return kB200Sms;
+  if (cache[dev] <= 0) {
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) return kB200Sms;
+    cache[dev] = sms;
   }
-  return g_sms;
+  return cache[dev];
 }
 
 // persistent grid: kMinBlocks CTAs per SM (or one per tile when there are fewer tiles than that)

@@ -4,6 +4,8 @@
 
 namespace bit1 {
 cudaError_t configure_kernels();
+// SMs of the current device (cudaDevAttrMultiProcessorCount, remembered per device); every grid is sized from it
+int sm_count();
 // one timestep on stream s; returns the number of kernels launched
 // ev: NULL, or 5 events recorded before/between/after the four kernels (per-kernel timing)
 int launch_step(const Params& P, const Particles& cur, const Particles& nxt, cudaStream_t s, cudaEvent_t* ev);
