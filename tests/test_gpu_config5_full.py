@@ -4,7 +4,7 @@ oracle after 2 steps and 240 000 sampled particles after a third.
 
 Opt-in (BIT1_FULL_C5=1): it needs ~130 GB of HBM, ~130 GB of host memory and about eight minutes, which does not
 belong in the default `pytest -m gpu` run.  The result of the run made for this round is recorded in
-profiles/r2_full_runs.md (round 1: profiles/r1e_config5_full.md).  State digests are taken array by array (8 GB at a time) through the C ABI."""
+profiles/r2_full_runs.md.  State digests are taken array by array (8 GB at a time) through the C ABI."""
 import ctypes as C
 import hashlib
 import json

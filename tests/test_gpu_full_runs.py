@@ -2,7 +2,7 @@
 oracle time).  Configs 1-3: every element of the final state against the oracle (SURVEY.md section 4 "100-step on configs
 1-3 in full"; config 2 over its whole 1000 steps, config 3 over 300 of its 1000 by default and over all of them with
 BIT1_FULL_C3_STEPS=1000, five minutes of oracle time).  Config 4: its whole 500 steps, flags
-clean, exact invariants at the end.  The run made for this round is recorded in profiles/r2_full_runs.md (round 1: profiles/r1e_full_runs.md)."""
+clean, exact invariants at the end.  The run made for this round is recorded in profiles/r2_full_runs.md."""
 import json
 import os
 import time
