@@ -280,6 +280,40 @@ def _measure(sim, steps: int, warmup: int, peak: float, barrier=None, sampler_in
                 n_prof=n_prof, kern=kern, psteps=int(psteps), mom=mom)
 
 
+def _sustained(sim, steps: int, sampler_index: int):
+    """What a long run gets: `steps` more steps of the loaded workload (its own length, e.g. configs[3]'s 500) in one
+    bit1_step call, timed by CUDA events on the compute stream, with the clock sampler running throughout (a 20-step
+    burst is over before nvidia-smi's 100 ms poll fires twice; under the power cap the SM clock, and the step time with
+    it, drifts during the first seconds)."""
+    import torch
+
+    sampler = ClockSampler(sampler_index)
+    time.sleep(0.3)   # the sampler's first rows
+    general0 = sim.get_moments()["general_steps"]
+    n_start = sim.n_live()
+    ev0 = torch.cuda.Event(enable_timing=True)
+    ev1 = torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    with torch.cuda.stream(sim.compute_stream):
+        ev0.record(sim.compute_stream)
+        sim.step(steps)
+        ev1.record(sim.compute_stream)
+    torch.cuda.synchronize()
+    t1 = time.perf_counter()
+    clocks = sampler.stop(t0, t1)
+    ms = ev0.elapsed_time(ev1)
+    sim.sync()
+    ms_settled = 1e3 * (time.perf_counter() - t0)
+    general = int(sim.get_moments()["general_steps"] - general0)
+    if general > 0:   # redone steps ran in the sync, outside the event pair (see _measure)
+        ms = ms_settled
+    units = 0.5 * (n_start + sim.n_live()) * steps
+    return {"steps": steps, "ms_per_step": ms / steps, "value": units / (ms * 1e-3), "unit": UNIT,
+            "seconds": ms * 1e-3, "sm_mhz_median": clocks.get("sm_mhz"), "sm_max_mhz": clocks.get("sm_max_mhz"),
+            "reasons": clocks.get("reasons"), "clock_samples": clocks.get("samples"),
+            "general_steps": general, "timed": "wall clock incl. settle of redone steps" if general else "CUDA events"}
+
+
 def _summary(r, steps: int, peak: float, n0: int):
     """Figures of one workload for the `workloads` list."""
     ms_step = r["ms"] / steps
@@ -406,6 +440,10 @@ def run_cuda(args):
     ms, units, launches, clocks, n_end = r["ms"], r["units"], r["launches"], r["clocks"], r["n_end"]
     prof, psteps, n_prof, mom = r["kern"], r["psteps"], r["n_prof"], r["mom"]
     ms_max, units_all = aggregate(ms, units, world, dev)
+    sustained = None
+    if world == 1 and args.sustained_steps != 0:
+        k = args.sustained_steps if args.sustained_steps > 0 else min(int(w.steps), 1000)
+        sustained = _sustained(sim, k, local)
 
     # ---- end-to-end leg: host buffers in, rho out, copies inside the timed region ----------------------
     barrier()
@@ -473,6 +511,10 @@ def run_cuda(args):
                   "window_radius": mom["window_radius"], "general_steps": mom["general_steps"],
                   "general_steps_in_timed_region": r["general_timed"], "timed": r["timed"], "flags": mom["flags"]},
     }
+    if sustained is not None:
+        sustained["what"] = (f"{sustained['steps']} further steps of the same loaded state in one bit1_step call (the "
+                             "workload's own run length), after the timed region and the per-kernel leg")
+        line["sustained"] = sustained
     sim.close()
     del sim, pin, host
     torch.cuda.empty_cache()
@@ -635,6 +677,8 @@ def main():
     ap.add_argument("--radius", type=int, default=None, help="pin the sort-window radius (default: adaptive)")
     ap.add_argument("--radius-max", type=int, default=0)
     ap.add_argument("--side-list", type=int, default=0, help="side-list capacity (entries)")
+    ap.add_argument("--sustained-steps", type=int, default=-1,
+                    help="length of the `sustained` leg (default: the workload's own step count, at most 1000; 0 = skip)")
     ap.add_argument("--sweep", default=None, choices=["far-movers", "stream"],
                     help="print the far-mover sweep / the checkpoint-overlap table instead of the bench line")
     ap.add_argument("--every", type=int, nargs="+", default=[200, 100, 50], help="--sweep stream: snapshot intervals")
