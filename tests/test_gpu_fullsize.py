@@ -10,7 +10,9 @@ pytestmark = pytest.mark.gpu
 
 
 def _scale_for_this_box():
-    """Full size needs ~30 GB of host memory for the input arrays and two copies of the state."""
+    """Full size or nothing: the test's name promises configs[3] at its full 2e8 particles, which needs about 30 GB of
+    host memory for the input arrays and 30 GB of HBM for two copies of the state.  A smaller box skips, with the
+    reason in the report, instead of quietly testing a quarter-size case under the full-size name."""
     try:
         import psutil
         avail = psutil.virtual_memory().available
@@ -20,7 +22,10 @@ def _scale_for_this_box():
     free, _ = torch.cuda.mem_get_info()
     if avail > 48e9 and free > 30e9:
         return 1.0
-    return 0.25
+    reason = (f"full size needs > 48 GB of free host memory and > 30 GB of free HBM; this box has "
+              f"{avail / 1e9:.0f} GB and {free / 1e9:.0f} GB")
+    print("SKIPPED test_gpu_fullsize: " + reason)
+    pytest.skip(reason)
 
 
 def _check_invariants(w, p, rho, dens, m, n_expected, where):
